@@ -1,0 +1,138 @@
+/*
+ * csf.h — C ABI of libcsf: Chebyshev-filtered spinor H.X on one NVIDIA B200 (sm_100a).
+ *
+ * The library computes, for a block X of two-component complex spinor wavefunctions,
+ *
+ *      Y = T_m(H~) X,   H~ = (Hhat - c I)/e,  c = (a+b)/2,  e = (b-a)/2,
+ *      Hhat = M_D^{-1/2} (H^loc + H^nloc) M_D^{-1/2}
+ *
+ * where H^loc, H^nloc are the finite-element discretised local and nonlocal (spin-orbit
+ * pseudopotential) parts of the noncollinear Kohn-Sham Hamiltonian of arxiv 2410.02754 and M_D is the
+ * GLL-lumped (diagonal) mass matrix. Citations "P:<line>" are lines of the paper text:
+ *
+ *   spinor coefficients U_{2I+alpha,n}, alpha = 0 (up), 1 (down)                     P:290-302 eq.38-39
+ *   H^loc_{2I+a,2J+b} = int [1/2 grad N_I . grad N_J + V_eff N_I N_J] d_ab
+ *                        + sum_d B^d N_I N_J sigma^d_ab          (Gamma point, k = 0)  P:304 eq.40, eq.16
+ *   H^nloc_{2I+a,2J+b} = sum_atoms sum_{X X'} P_{I X} D^{X X'}_{ab} conj(P_{J X'})     P:308 eq.41, eq.14
+ *   Delta_{2X+a,2X'+b} = D^{X X'}_{ab}                                                P:517-519 eq.76
+ *   cell-level evaluation: extract X^(e) = R^(e) X, apply H^(e), assemble sum_e R^(e)T Y^(e)
+ *                                                                                     P:507 eq.74, eq.84
+ *   M diagonal through GLL quadrature at the FE nodes; filter built on M^-1 H
+ *   T_{k+1}(H~) = 2 H~ T_k(H~) - T_{k-1}(H~), unwanted spectrum [a,b] -> [-1,1]        P:463-469 eq.70
+ *
+ * Readings where the paper is silent: the similarity-equivalent Hermitian form
+ * M_D^{-1/2} H M_D^{-1/2} is used (X and Y live in the Loewdin-scaled basis); T_m is the plain first-kind
+ * Chebyshev polynomial; the stiffness integral is exact; V_eff and B are collocated at the GLL nodes;
+ * projector entries P_{I X} are supplied already integrated; nodes on a Dirichlet face are removed.
+ *
+ * Conventions
+ *   - Every function returns CSF_OK (0) or a negative error code; nothing throws or aborts across the ABI.
+ *     csf_last_error() gives a text for the last failure on that context.
+ *   - "host" pointers are ordinary CPU memory, copied before the call returns (the caller may free them).
+ *     "device" pointers are CUDA device memory on the context's device, owned by the caller.
+ *   - Device multivector layout: element (node I, spin alpha, vector n) is the complex128 at
+ *     d[(2*I + alpha)*ld + n], ld >= nvec  (row 2I+alpha as in P:302; vector index fastest).
+ *   - Node numbering is the library's: unconstrained nodes only, x fastest, then y, then z; use
+ *     csf_node_coords() instead of guessing.
+ *   - csf_apply_H and csf_filter only ENQUEUE work on the context's stream and return without
+ *     synchronising; create/set_* /destroy may synchronise.
+ *   - There is no CPU fallback: without a CUDA device every compute entry point fails with CSF_ECUDA.
+ */
+#ifndef CSF_H
+#define CSF_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct csf_ctx csf_ctx;                 /* opaque; owns all device-side operator tables */
+typedef struct { double re, im; } csf_c128;     /* layout-compatible with cuDoubleComplex / torch.complex128 */
+
+enum { CSF_OK = 0, CSF_EINVAL = -1, CSF_ENOMEM = -2, CSF_ECUDA = -3, CSF_ESTATE = -4, CSF_EUNSUPPORTED = -5 };
+enum { CSF_BC_PERIODIC = 0, CSF_BC_DIRICHLET = 1, CSF_BC_FREE = 2 /* natural BC: not supported on the GPU path */ };
+enum { CSF_FP64 = 0, CSF_FP32_INTERMEDIATE = 1 };
+
+/* Create the mesh, cells and GLL nodes: an axis-aligned box of `box` bohr meshed by
+ * ncell[0] x ncell[1] x ncell[2] congruent hexahedral cells carrying tensor-product Lagrange bases of
+ * degree `order` (1..7) on GLL nodes; bc[d] is CSF_BC_PERIODIC or CSF_BC_DIRICHLET per direction.
+ * `device` is the CUDA ordinal; `cuda_stream` is a cudaStream_t (borrowed, may be NULL = default stream)
+ * on which all later work is enqueued. All arrays are host pointers. Errors: CSF_EINVAL (bad argument),
+ * CSF_EUNSUPPORTED (CSF_BC_FREE, order > 7), CSF_ECUDA, CSF_ENOMEM. */
+int csf_create(csf_ctx** out, const int ncell[3], const double box[3], int order, const int bc[3],
+               int device, void* cuda_stream);
+
+/* Free the context and every device table it owns. NULL is accepted. */
+int csf_destroy(csf_ctx* ctx);
+
+/* Rebind the stream later work is enqueued on (borrowed cudaStream_t). */
+int csf_set_stream(csf_ctx* ctx, void* cuda_stream);
+
+/* M = number of unconstrained FE nodes per spin component ("M^{h,p}"); a spinor block has 2M rows. */
+int csf_num_nodes(const csf_ctx* ctx, int64_t* M);
+
+/* GLL node positions in the library's numbering, host array [M][3] (bohr). A periodic node is reported
+ * at its image inside [0, box). */
+int csf_node_coords(const csf_ctx* ctx, double* xyz_host);
+
+/* Lumped GLL mass m_I = sum_e J^(e) w_i w_j w_k (eq.43 under GLL quadrature), host array [M]. */
+int csf_mass_diag(const csf_ctx* ctx, double* m_host);
+
+/* Set the spin potential at the nodes (eq.16, eq.40): veff host [M] (Ha), bxyz host [M][3]
+ * (B_xc components; NULL means B = 0). Node I contributes the block m_I (V_I I_2 + B_I . sigma). */
+int csf_set_potential(csf_ctx* ctx, const double* veff, const double* bxyz);
+
+/* Set the atom-centred projectors and the spin-coupled D matrices (eq.41-42, eq.76).
+ *   natoms           number of atoms; 0 clears the nonlocal part (all other pointers may then be NULL)
+ *   node_ptr         host [natoms+1]: atom a's support rows are node_idx[node_ptr[a] .. node_ptr[a+1])
+ *   node_idx         host: global node ids (0 <= id < M), no duplicates within one atom
+ *   nproj            host [natoms]: n_pj of each atom (scalar projector columns, spin-diagonal as in eq.78)
+ *   pvals            host: atom a's block [n_a][nproj[a]] row-major, blocks concatenated; entry = P_{I X},
+ *                    the already integrated value of eq.42 at k = 0 (real)
+ *   atom_type        host [natoms]: index gamma_a into the Delta tables
+ *   ntypes, delta, delta_ptr
+ *                    type t owns delta[delta_ptr[t] .. delta_ptr[t+1]) = [(2 npj)][(2 npj)] row-major with
+ *                    composite index 2X+alpha (eq.76); must be Hermitian for a Hermitian H (not checked)
+ * Errors: CSF_EINVAL on inconsistent sizes or out-of-range ids. */
+int csf_set_projectors(csf_ctx* ctx, int natoms, const int64_t* node_ptr, const int64_t* node_idx,
+                       const int* nproj, const double* pvals, const int* atom_type, int ntypes,
+                       const csf_c128* delta, const int64_t* delta_ptr);
+
+/* Bytes of device workspace csf_apply_H / csf_filter need for blocks of up to nvec vectors in `mode`. */
+int csf_workspace_bytes(const csf_ctx* ctx, int nvec, int mode, size_t* bytes);
+
+/* Y = Hhat X (one application of M_D^{-1/2} H M_D^{-1/2}; P:551-561 steps 2-4). dX, dY: device, [2M][ld]
+ * complex128, dY must not alias dX. d_work: device, >= csf_workspace_bytes(nvec, CSF_FP64). Enqueues only.
+ * Errors: CSF_ESTATE if the potential was never set, CSF_EINVAL on NULL / ld < nvec / nvec < 0 /
+ * too small workspace, CSF_ECUDA. nvec = 0 is a no-op. */
+int csf_apply_H(csf_ctx* ctx, const csf_c128* dX, csf_c128* dY, int64_t ld, int nvec,
+                void* d_work, size_t work_bytes);
+
+/* Y = T_degree((Hhat - c)/e) X with c = (a+b)/2, e = (b-a)/2 (eq.70). degree = 0 copies X to Y.
+ * Same pointer rules as csf_apply_H; X is not modified. mode: CSF_FP64, or CSF_FP32_INTERMEDIATE (complex128
+ * in and out, fp32 recurrence buffers and cell arithmetic in between; CSF_EUNSUPPORTED until built).
+ * Errors: CSF_EINVAL also for degree < 0 or a >= b. Enqueues only. */
+int csf_filter(csf_ctx* ctx, const csf_c128* dX, csf_c128* dY, int64_t ld, int nvec,
+               int degree, double a, double b, int mode, void* d_work, size_t work_bytes);
+
+/* Same operation with HOST buffers hX, hY ([2M][ld] complex128, pinned or pageable): the library stages
+ * column chunks through device memory it allocates itself (host->device copy, filter, device->host copy)
+ * and SYNCHRONISES before returning. This is the end-to-end entry point. */
+int csf_filter_host(csf_ctx* ctx, const csf_c128* hX, csf_c128* hY, int64_t ld, int nvec,
+                    int degree, double a, double b, int mode);
+
+/* Number of kernel launches (own kernels only, memsets excluded) enqueued by this context so far. */
+int csf_launch_count(const csf_ctx* ctx, int64_t* launches);
+
+/* Select the cell-kernel variant (0 = library default); used by the benchmark sweep. CSF_EINVAL if unknown. */
+int csf_set_variant(csf_ctx* ctx, int variant);
+
+/* Text of the last error recorded on ctx (never NULL; "" if none). With ctx = NULL: last csf_create failure. */
+const char* csf_last_error(const csf_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CSF_H */

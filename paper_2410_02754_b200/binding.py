@@ -1,0 +1,139 @@
+"""Thin Python binding of libcsf.so (include/csf.h): argument marshalling only.
+
+Every step of the path runs in the library's CUDA kernels; PyTorch is used for device memory and streams.
+There is no CPU fallback: if libcsf.so is missing or no CUDA device is present, calls raise.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libcsf.so")
+
+CSF_OK, CSF_EINVAL, CSF_ENOMEM, CSF_ECUDA, CSF_ESTATE, CSF_EUNSUPPORTED = 0, -1, -2, -3, -4, -5
+CSF_BC_PERIODIC, CSF_BC_DIRICHLET, CSF_BC_FREE = 0, 1, 2
+CSF_FP64, CSF_FP32_INTERMEDIATE = 0, 1
+
+EXPORTS = ["csf_create", "csf_destroy", "csf_set_stream", "csf_num_nodes", "csf_node_coords", "csf_mass_diag", "csf_set_potential",
+           "csf_set_projectors", "csf_workspace_bytes", "csf_apply_H", "csf_filter", "csf_filter_host", "csf_launch_count",
+           "csf_set_variant", "csf_last_error"]
+
+_lib = None
+
+
+class CsfError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"libcsf error {code}: {msg}")
+        self.code = code
+
+
+def lib():
+    """Load libcsf.so (built in-tree by paper_2410_02754_b200/build.py). Fails loudly if it is missing."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise FileNotFoundError(f"{LIB_PATH} not found: run `python -m paper_2410_02754_b200.build` (no CPU fallback exists)")
+        _lib = C.CDLL(LIB_PATH)
+        _lib.csf_last_error.restype = C.c_char_p
+        _lib.csf_last_error.argtypes = [C.c_void_p]
+    return _lib
+
+
+def _dp(a, t):
+    return a.ctypes.data_as(C.POINTER(t))
+
+
+class Csf:
+    """One mesh + operator context on one GPU. Method names mirror the C entry points."""
+
+    def __init__(self, ncell, box, order, bc, device=0, stream=None):
+        self._h = C.c_void_p()
+        self._L = lib()
+        nc = (C.c_int * 3)(*[int(v) for v in ncell]); bx = (C.c_double * 3)(*[float(v) for v in box]); b = (C.c_int * 3)(*[int(v) for v in bc])
+        rc = self._L.csf_create(C.byref(self._h), nc, bx, C.c_int(int(order)), b, C.c_int(int(device)), C.c_void_p(stream or 0))
+        if rc != CSF_OK:
+            raise CsfError(rc, self._L.csf_last_error(None).decode())
+        self.ncell, self.box, self.order, self.bc, self.device = tuple(ncell), tuple(box), int(order), tuple(bc), int(device)
+        m = C.c_int64(); self._chk(self._L.csf_num_nodes(self._h, C.byref(m))); self.M = int(m.value)
+
+    def _chk(self, rc):
+        if rc != CSF_OK:
+            raise CsfError(rc, self._L.csf_last_error(self._h).decode())
+
+    def destroy(self):
+        if self._h:
+            self._L.csf_destroy(self._h); self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+    def set_stream(self, stream):
+        self._chk(self._L.csf_set_stream(self._h, C.c_void_p(stream or 0)))
+
+    def node_coords(self):
+        xyz = np.zeros((self.M, 3)); self._chk(self._L.csf_node_coords(self._h, _dp(xyz, C.c_double))); return xyz
+
+    def mass_diag(self):
+        m = np.zeros(self.M); self._chk(self._L.csf_mass_diag(self._h, _dp(m, C.c_double))); return m
+
+    def set_potential(self, veff, bxyz=None):
+        veff = np.ascontiguousarray(veff, dtype=np.float64)
+        if veff.shape != (self.M,):
+            raise ValueError("veff must have shape [M]")
+        if bxyz is not None:
+            bxyz = np.ascontiguousarray(bxyz, dtype=np.float64)
+            if bxyz.shape != (self.M, 3):
+                raise ValueError("bxyz must have shape [M,3]")
+        self._chk(self._L.csf_set_potential(self._h, _dp(veff, C.c_double), _dp(bxyz, C.c_double) if bxyz is not None else None))
+
+    def set_projectors(self, node_ptr, node_idx, nproj, pvals, atom_type, delta, delta_ptr):
+        natoms = len(nproj)
+        if natoms == 0:
+            self._chk(self._L.csf_set_projectors(self._h, C.c_int(0), None, None, None, None, None, C.c_int(0), None, None)); return
+        node_ptr = np.ascontiguousarray(node_ptr, dtype=np.int64); node_idx = np.ascontiguousarray(node_idx, dtype=np.int64)
+        nproj = np.ascontiguousarray(nproj, dtype=np.int32); pvals = np.ascontiguousarray(pvals, dtype=np.float64)
+        atom_type = np.ascontiguousarray(atom_type, dtype=np.int32)
+        delta = np.ascontiguousarray(delta, dtype=np.complex128); delta_ptr = np.ascontiguousarray(delta_ptr, dtype=np.int64)
+        self._chk(self._L.csf_set_projectors(self._h, C.c_int(natoms), _dp(node_ptr, C.c_int64), _dp(node_idx, C.c_int64), _dp(nproj, C.c_int),
+                                             _dp(pvals, C.c_double), _dp(atom_type, C.c_int), C.c_int(len(delta_ptr) - 1),
+                                             delta.ctypes.data_as(C.c_void_p), _dp(delta_ptr, C.c_int64)))
+
+    def workspace_bytes(self, nvec, mode=CSF_FP64):
+        b = C.c_size_t(); self._chk(self._L.csf_workspace_bytes(self._h, C.c_int(int(nvec)), C.c_int(mode), C.byref(b))); return int(b.value)
+
+    # ---- device entry points: raw pointers (ints) or torch tensors ----
+    @staticmethod
+    def _ptr(t):
+        return C.c_void_p(t if isinstance(t, int) else t.data_ptr())
+
+    @staticmethod
+    def _nbytes(t, given):
+        return C.c_size_t(given if isinstance(t, int) else t.numel() * t.element_size())
+
+    def apply_H(self, dX, dY, ld, nvec, d_work, work_bytes=0):
+        self._chk(self._L.csf_apply_H(self._h, self._ptr(dX), self._ptr(dY), C.c_int64(int(ld)), C.c_int(int(nvec)), self._ptr(d_work), self._nbytes(d_work, work_bytes)))
+
+    def filter(self, dX, dY, ld, nvec, degree, a, b, mode=CSF_FP64, d_work=0, work_bytes=0):
+        self._chk(self._L.csf_filter(self._h, self._ptr(dX), self._ptr(dY), C.c_int64(int(ld)), C.c_int(int(nvec)), C.c_int(int(degree)),
+                                     C.c_double(float(a)), C.c_double(float(b)), C.c_int(mode), self._ptr(d_work), self._nbytes(d_work, work_bytes)))
+
+    def filter_host(self, hX, hY, ld, nvec, degree, a, b, mode=CSF_FP64):
+        """hX, hY: host pointers (ints), NumPy arrays or CPU (pinned) torch tensors."""
+        def hp(t):
+            if isinstance(t, int):
+                return C.c_void_p(t)
+            if isinstance(t, np.ndarray):
+                return C.c_void_p(t.ctypes.data)
+            return C.c_void_p(t.data_ptr())
+        self._chk(self._L.csf_filter_host(self._h, hp(hX), hp(hY), C.c_int64(int(ld)), C.c_int(int(nvec)), C.c_int(int(degree)),
+                                          C.c_double(float(a)), C.c_double(float(b)), C.c_int(mode)))
+
+    def launch_count(self):
+        n = C.c_int64(); self._chk(self._L.csf_launch_count(self._h, C.byref(n))); return int(n.value)
+
+    def set_variant(self, variant):
+        self._chk(self._L.csf_set_variant(self._h, C.c_int(int(variant))))

@@ -1,0 +1,484 @@
+// csf_api.cu — C ABI of libcsf (see include/csf.h): context, host-side preprocessing, launch sequencing.
+#include "../../include/csf.h"
+#include "csf_kernels.cuh"
+#include "csf_tables.h"
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <numeric>
+#include <string>
+#include <vector>
+
+using namespace csf;
+
+namespace {
+
+thread_local std::string g_create_error;
+
+struct DevBuf {
+    void* p = nullptr; size_t bytes = 0;
+    ~DevBuf() { release(); }
+    void release() { if (p) cudaFree(p); p = nullptr; bytes = 0; }
+    cudaError_t alloc(size_t n) { release(); if (n == 0) return cudaSuccess; cudaError_t e = cudaMalloc(&p, n); if (e == cudaSuccess) bytes = n; return e; }
+    template <class T> cudaError_t upload(const std::vector<T>& v) {
+        cudaError_t e = alloc(std::max<size_t>(v.size(), 1) * sizeof(T)); if (e != cudaSuccess) return e;
+        return v.empty() ? cudaSuccess : cudaMemcpy(p, v.data(), v.size() * sizeof(T), cudaMemcpyHostToDevice);
+    }
+    template <class T> T* as() const { return static_cast<T*>(p); }
+};
+
+}  // namespace
+
+struct csf_ctx {
+    int device = 0; cudaStream_t stream = nullptr;
+    int ncell[3], bc[3], p = 0, n = 0;
+    double box[3], h[3];
+    int nfree[3]; long long M = 0; int E = 0;
+    Gll1D gll; Dir1D dir[3];
+    bool have_pot = false;
+    DevBuf d_cell_order, d_vb;
+    // projectors
+    int natoms = 0, npj_uniform = 0, npjp = 0; long long crows = 0;
+    DevBuf d_pair_ptr, d_pair_atom, d_pair_off, d_ent_loc, d_ent_node, d_ent_p, d_atom_coff, d_atom_npj, d_atom_type,
+        d_delta, d_delta_ptr, d_gb_atom, d_gb_beg, d_gb_end;
+    int n_gather_blocks = 0;
+    int variant = 0;
+    long long launches = 0;
+    int sm_count = 148; size_t smem_optin = 0;
+    std::string err;
+    // scratch for csf_filter_host
+    DevBuf h_x, h_y, h_w;
+};
+
+namespace {
+
+int fail(csf_ctx* c, int code, const std::string& msg) { if (c) c->err = msg; else g_create_error = msg; return code; }
+int cuda_fail(csf_ctx* c, cudaError_t e, const char* what) { return fail(c, CSF_ECUDA, std::string(what) + ": " + cudaGetErrorString(e)); }
+#define CSF_CUDA(ctx, call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) return cuda_fail(ctx, e__, #call); } while (0)
+
+inline int lanes_of_variant(int v) { return v == 1 ? 32 : v == 2 ? 16 : v == 3 ? 8 : 0; }
+
+size_t cell_smem_bytes(int p, int L) { const size_t n = p + 1; return (2 * n * n * n + (size_t)p * p * p) * L * sizeof(double); }
+
+template <int P, int L, int NPJ>
+cudaError_t launch_cell_t(const CellParams& cp, int nblocks, size_t smem, cudaStream_t s) {
+    static bool configured = false;
+    auto kern = cell_kernel<P, L, NPJ>;
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    kern<<<nblocks, (P + 1) * L, smem, s>>>(cp);
+    return cudaGetLastError();
+}
+
+template <int P, int L>
+cudaError_t launch_cell_pl(int npj, const CellParams& cp, int nblocks, size_t smem, cudaStream_t s) {
+    if (npj == 18) return launch_cell_t<P, L, 18>(cp, nblocks, smem, s);
+    return launch_cell_t<P, L, 0>(cp, nblocks, smem, s);
+}
+
+template <int P>
+cudaError_t launch_cell_p(int L, int npj, const CellParams& cp, int nblocks, size_t smem, cudaStream_t s) {
+    switch (L) {
+        case 32: return launch_cell_pl<P, 32>(npj, cp, nblocks, smem, s);
+        case 16: return launch_cell_pl<P, 16>(npj, cp, nblocks, smem, s);
+        default: return launch_cell_pl<P, 8>(npj, cp, nblocks, smem, s);
+    }
+}
+
+cudaError_t launch_cell(int p, int L, int npj, const CellParams& cp, int nblocks, size_t smem, cudaStream_t s) {
+    switch (p) {
+        case 1: return launch_cell_p<1>(L, npj, cp, nblocks, smem, s);
+        case 2: return launch_cell_p<2>(L, npj, cp, nblocks, smem, s);
+        case 3: return launch_cell_p<3>(L, npj, cp, nblocks, smem, s);
+        case 4: return launch_cell_p<4>(L, npj, cp, nblocks, smem, s);
+        case 5: return launch_cell_p<5>(L, npj, cp, nblocks, smem, s);
+        case 6: return launch_cell_p<6>(L, npj, cp, nblocks, smem, s);
+        case 7: return launch_cell_p<7>(L, npj, cp, nblocks, smem, s);
+    }
+    return cudaErrorInvalidValue;
+}
+
+int pick_lanes(const csf_ctx* c) {
+    int L = lanes_of_variant(c->variant);
+    if (L == 0) L = 32;
+    while (L > 8 && cell_smem_bytes(c->p, L) > c->smem_optin) L /= 2;
+    return L;
+}
+
+// one step: dst += sc * i^rot * (Hhat - shift) src
+int enqueue_step(csf_ctx* c, const double* src, long long ld, double* dst, long long ld_dst, int nvec, double sc, int rot, double shift,
+                 double* dC, double* dCt) {
+    const int L = pick_lanes(c);
+    if (cell_smem_bytes(c->p, L) > c->smem_optin) return fail(c, CSF_EUNSUPPORTED, "cell tile does not fit shared memory");
+    const long long ldc = nvec;
+    if (c->natoms > 0) {
+        CSF_CUDA(c, cudaMemsetAsync(dC, 0, (size_t)c->crows * ldc * sizeof(double2), c->stream));
+        GatherParams gp{};
+        gp.src = src; gp.ld = ld; gp.nvec = nvec;
+        gp.gb_atom = c->d_gb_atom.as<int>(); gp.gb_beg = c->d_gb_beg.as<int>(); gp.gb_end = c->d_gb_end.as<int>();
+        gp.ent_node = c->d_ent_node.as<int>(); gp.ent_p = c->d_ent_p.as<double>(); gp.npjp = c->npjp;
+        gp.atom_coff = c->d_atom_coff.as<long long>(); gp.atom_npj = c->d_atom_npj.as<int>();
+        gp.C = dC; gp.ldc = ldc;
+        dim3 gg(c->n_gather_blocks, (nvec + 7) / 8);
+        if (c->npj_uniform == 18) proj_gather_kernel<18><<<gg, 128, 0, c->stream>>>(gp);
+        else proj_gather_kernel<0><<<gg, 128, 0, c->stream>>>(gp);
+        CSF_CUDA(c, cudaGetLastError());
+        DeltaParams dp{};
+        dp.C = reinterpret_cast<const double2*>(dC); dp.Ct = reinterpret_cast<double2*>(dCt); dp.ldc = ldc; dp.nvec = nvec;
+        dp.atom_coff = c->d_atom_coff.as<long long>(); dp.atom_npj = c->d_atom_npj.as<int>(); dp.atom_type = c->d_atom_type.as<int>();
+        dp.delta = c->d_delta.as<double2>(); dp.delta_ptr = c->d_delta_ptr.as<long long>();
+        dim3 dg(c->natoms, (nvec + 31) / 32);
+        delta_apply_kernel<<<dg, 256, 0, c->stream>>>(dp);
+        CSF_CUDA(c, cudaGetLastError());
+        c->launches += 2;
+    }
+    CellParams cp{};
+    const int n = c->n;
+    for (int i = 0; i < n; ++i) {
+        for (int j = 0; j < n; ++j) { cp.Ay[i][j] = c->dir[1].A[i][j]; cp.Az[i][j] = c->dir[2].A[i][j]; cp.Ax[i][j] = sc * c->dir[0].A[i][j]; }
+        cp.by[i] = c->dir[1].beta[i]; cp.uy[i] = c->dir[1].u[i];
+        cp.bz[i] = c->dir[2].beta[i]; cp.uz[i] = c->dir[2].u[i];
+        cp.bxs[i] = sc * c->dir[0].beta[i]; cp.ux[i] = c->dir[0].u[i]; cp.uxs[i] = sc * c->dir[0].u[i];
+    }
+    cp.src = src; cp.dst = dst; cp.ld_src = ld; cp.ld_dst = ld_dst; cp.nvec = nvec;
+    cp.ncx = c->ncell[0]; cp.ncy = c->ncell[1]; cp.ncz = c->ncell[2];
+    cp.nfx = c->nfree[0]; cp.nfy = c->nfree[1]; cp.nfz = c->nfree[2];
+    cp.bcx = c->bc[0]; cp.bcy = c->bc[1]; cp.bcz = c->bc[2];
+    cp.cell_order = c->d_cell_order.as<int>(); cp.ncells = c->E;
+    cp.vb = c->d_vb.as<double>(); cp.shift = shift; cp.sc = sc; cp.rot = rot & 3;
+    if (c->natoms > 0) {
+        cp.pair_ptr = c->d_pair_ptr.as<int>(); cp.pair_atom = c->d_pair_atom.as<int>(); cp.pair_off = c->d_pair_off.as<int>();
+        cp.ent_loc = c->d_ent_loc.as<int>(); cp.ent_p = c->d_ent_p.as<double>();
+        cp.atom_coff = c->d_atom_coff.as<long long>(); cp.atom_npj = c->d_atom_npj.as<int>();
+        cp.Ct = dCt; cp.ldc = ldc; cp.npjp = c->npjp;
+    }
+    const int vchunk = L / 4;
+    const long long nblocks = (long long)c->E * ((nvec + vchunk - 1) / vchunk);
+    if (nblocks > 0x7fffffffLL) return fail(c, CSF_EUNSUPPORTED, "grid too large");
+    CSF_CUDA(c, launch_cell(c->p, L, c->natoms > 0 ? c->npj_uniform : 18, cp, (int)nblocks, cell_smem_bytes(c->p, L), c->stream));
+    c->launches += 1;
+    return CSF_OK;
+}
+
+size_t block_bytes(const csf_ctx* c, int nvec) { return (size_t)2 * c->M * nvec * sizeof(double2); }
+size_t coef_bytes(const csf_ctx* c, int nvec) { return ((size_t)c->crows * nvec * sizeof(double2) + 255) / 256 * 256; }
+
+int enqueue_zero(csf_ctx* c, double* dst, long long ld, int nvec) {
+    const long long rows = 2 * c->M;
+    if (ld == nvec) { CSF_CUDA(c, cudaMemsetAsync(dst, 0, (size_t)rows * ld * sizeof(double2), c->stream)); return CSF_OK; }
+    zero_kernel<<<c->sm_count * 8, 256, 0, c->stream>>>(reinterpret_cast<double2*>(dst), rows, ld, nvec);
+    CSF_CUDA(c, cudaGetLastError());
+    c->launches += 1;
+    return CSF_OK;
+}
+
+int check_block_args(csf_ctx* c, const void* x, const void* y, long long ld, int nvec, const void* work, size_t work_bytes, size_t need) {
+    if (!c) return CSF_EINVAL;
+    if (!x || !y) return fail(c, CSF_EINVAL, "NULL block pointer");
+    if (x == y) return fail(c, CSF_EINVAL, "Y must not alias X");
+    if (nvec < 0 || ld < nvec) return fail(c, CSF_EINVAL, "need 0 <= nvec <= ld");
+    if (!c->have_pot) return fail(c, CSF_ESTATE, "csf_set_potential has not been called");
+    if (nvec > 0 && need > 0 && (!work || work_bytes < need)) return fail(c, CSF_EINVAL, "workspace too small");
+    return CSF_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* csf_last_error(const csf_ctx* ctx) { return ctx ? ctx->err.c_str() : g_create_error.c_str(); }
+
+int csf_create(csf_ctx** out, const int ncell[3], const double box[3], int order, const int bc[3], int device, void* cuda_stream) {
+    if (!out || !ncell || !box || !bc) return fail(nullptr, CSF_EINVAL, "NULL argument");
+    *out = nullptr;
+    if (order < 1) return fail(nullptr, CSF_EINVAL, "order must be >= 1");
+    if (order > 7) return fail(nullptr, CSF_EUNSUPPORTED, "order > 7 is not supported");
+    long long M = 1, E = 1;
+    for (int d = 0; d < 3; ++d) {
+        if (ncell[d] < 1 || !(box[d] > 0.0)) return fail(nullptr, CSF_EINVAL, "ncell must be >= 1 and box > 0");
+        if (bc[d] == CSF_BC_FREE) return fail(nullptr, CSF_EUNSUPPORTED, "CSF_BC_FREE is not supported on the GPU path");
+        if (bc[d] != CSF_BC_PERIODIC && bc[d] != CSF_BC_DIRICHLET) return fail(nullptr, CSF_EINVAL, "bad boundary condition");
+        long long nf = (long long)ncell[d] * order - (bc[d] == CSF_BC_DIRICHLET ? 1 : 0);
+        if (nf < 1) return fail(nullptr, CSF_EINVAL, "direction has no unconstrained node");
+        M *= nf; E *= ncell[d];
+    }
+    if (M >= (1LL << 31) || E >= (1LL << 31)) return fail(nullptr, CSF_EUNSUPPORTED, "mesh too large for 32-bit node ids");
+    int ndev = 0;
+    cudaError_t ce = cudaGetDeviceCount(&ndev);
+    if (ce != cudaSuccess || ndev <= 0) return fail(nullptr, CSF_ECUDA, std::string("no CUDA device: ") + cudaGetErrorString(ce));
+    if (device < 0 || device >= ndev) return fail(nullptr, CSF_EINVAL, "bad device ordinal");
+    ce = cudaSetDevice(device);
+    if (ce != cudaSuccess) return cuda_fail(nullptr, ce, "cudaSetDevice");
+    csf_ctx* c = new (std::nothrow) csf_ctx();
+    if (!c) return fail(nullptr, CSF_ENOMEM, "out of host memory");
+    c->device = device; c->stream = static_cast<cudaStream_t>(cuda_stream);
+    c->p = order; c->n = order + 1; c->M = M; c->E = (int)E;
+    for (int d = 0; d < 3; ++d) {
+        c->ncell[d] = ncell[d]; c->bc[d] = bc[d]; c->box[d] = box[d]; c->h[d] = box[d] / ncell[d];
+        c->nfree[d] = ncell[d] * order - (bc[d] == CSF_BC_DIRICHLET ? 1 : 0);
+    }
+    build_gll(order, &c->gll);
+    for (int d = 0; d < 3; ++d) build_dir(c->gll, c->h[d], &c->dir[d]);
+    cudaDeviceProp prop;
+    ce = cudaGetDeviceProperties(&prop, device);
+    if (ce != cudaSuccess) { delete c; return cuda_fail(nullptr, ce, "cudaGetDeviceProperties"); }
+    c->sm_count = prop.multiProcessorCount; c->smem_optin = prop.sharedMemPerBlockOptin;
+    // traversal order of the cells: 8x8x8 bricks, x fastest inside, so that the faces shared between
+    // neighbouring cells are combined in L2 before they are evicted
+    std::vector<int> order_v; order_v.reserve(E);
+    const int B = 8;
+    for (int bz = 0; bz < ncell[2]; bz += B) for (int by = 0; by < ncell[1]; by += B) for (int bx = 0; bx < ncell[0]; bx += B)
+        for (int z = bz; z < std::min(bz + B, ncell[2]); ++z) for (int y = by; y < std::min(by + B, ncell[1]); ++y)
+            for (int x = bx; x < std::min(bx + B, ncell[0]); ++x) order_v.push_back(x + ncell[0] * (y + ncell[1] * z));
+    ce = c->d_cell_order.upload(order_v);
+    if (ce != cudaSuccess) { delete c; return cuda_fail(nullptr, ce, "upload cell order"); }
+    *out = c;
+    return CSF_OK;
+}
+
+int csf_destroy(csf_ctx* ctx) {
+    if (!ctx) return CSF_OK;
+    cudaSetDevice(ctx->device);
+    delete ctx;
+    return CSF_OK;
+}
+
+int csf_set_stream(csf_ctx* ctx, void* cuda_stream) { if (!ctx) return CSF_EINVAL; ctx->stream = static_cast<cudaStream_t>(cuda_stream); return CSF_OK; }
+
+int csf_num_nodes(const csf_ctx* ctx, int64_t* M) { if (!ctx || !M) return CSF_EINVAL; *M = ctx->M; return CSF_OK; }
+
+// 1-D axis data of direction d: coordinate and lumped mass of every unconstrained node
+static void axis_tables(const csf_ctx* c, int d, std::vector<double>* x, std::vector<double>* m) {
+    const int p = c->p, nf = c->nfree[d];
+    x->assign(nf, 0.0); m->assign(nf, 0.0);
+    for (int cell = 0; cell < c->ncell[d]; ++cell)
+        for (int i = 0; i <= p; ++i) {
+            const int f = cell * p + i; int g;
+            if (c->bc[d] == CSF_BC_PERIODIC) g = f % (c->ncell[d] * p);
+            else { if (f == 0 || f == c->ncell[d] * p) continue; g = f - 1; }
+            (*m)[g] += 0.5 * c->h[d] * c->gll.w[i];
+            if (!(c->bc[d] == CSF_BC_PERIODIC && cell == c->ncell[d] - 1 && i == p)) (*x)[g] = (cell + 0.5 * (c->gll.xi[i] + 1.0)) * c->h[d];
+        }
+}
+
+int csf_node_coords(const csf_ctx* ctx, double* xyz) {
+    if (!ctx || !xyz) return CSF_EINVAL;
+    std::vector<double> ax[3], am[3];
+    for (int d = 0; d < 3; ++d) axis_tables(ctx, d, &ax[d], &am[d]);
+    long long I = 0;
+    for (int z = 0; z < ctx->nfree[2]; ++z) for (int y = 0; y < ctx->nfree[1]; ++y) for (int x = 0; x < ctx->nfree[0]; ++x, ++I) {
+        xyz[3 * I] = ax[0][x]; xyz[3 * I + 1] = ax[1][y]; xyz[3 * I + 2] = ax[2][z];
+    }
+    return CSF_OK;
+}
+
+int csf_mass_diag(const csf_ctx* ctx, double* mh) {
+    if (!ctx || !mh) return CSF_EINVAL;
+    std::vector<double> ax[3], am[3];
+    for (int d = 0; d < 3; ++d) axis_tables(ctx, d, &ax[d], &am[d]);
+    long long I = 0;
+    for (int z = 0; z < ctx->nfree[2]; ++z) for (int y = 0; y < ctx->nfree[1]; ++y) for (int x = 0; x < ctx->nfree[0]; ++x, ++I)
+        mh[I] = am[0][x] * am[1][y] * am[2][z];
+    return CSF_OK;
+}
+
+int csf_set_potential(csf_ctx* c, const double* veff, const double* bxyz) {
+    if (!c) return CSF_EINVAL;
+    if (!veff) return fail(c, CSF_EINVAL, "veff is NULL");
+    CSF_CUDA(c, cudaSetDevice(c->device));
+    std::vector<double> vb((size_t)c->M * 4);
+    for (long long I = 0; I < c->M; ++I) {
+        vb[4 * I] = veff[I];
+        vb[4 * I + 1] = bxyz ? bxyz[3 * I] : 0.0; vb[4 * I + 2] = bxyz ? bxyz[3 * I + 1] : 0.0; vb[4 * I + 3] = bxyz ? bxyz[3 * I + 2] : 0.0;
+    }
+    CSF_CUDA(c, cudaStreamSynchronize(c->stream));
+    CSF_CUDA(c, c->d_vb.upload(vb));
+    c->have_pot = true;
+    return CSF_OK;
+}
+
+int csf_set_projectors(csf_ctx* c, int natoms, const int64_t* node_ptr, const int64_t* node_idx, const int* nproj,
+                       const double* pvals, const int* atom_type, int ntypes, const csf_c128* delta, const int64_t* delta_ptr) {
+    if (!c) return CSF_EINVAL;
+    if (natoms < 0) return fail(c, CSF_EINVAL, "natoms < 0");
+    CSF_CUDA(c, cudaSetDevice(c->device));
+    CSF_CUDA(c, cudaStreamSynchronize(c->stream));
+    c->natoms = 0; c->crows = 0; c->n_gather_blocks = 0;
+    if (natoms == 0) return CSF_OK;
+    if (!node_ptr || !node_idx || !nproj || !pvals || !atom_type || ntypes < 1 || !delta || !delta_ptr) return fail(c, CSF_EINVAL, "NULL projector argument");
+    int npj_max = 0; bool uniform = true;
+    for (int a = 0; a < natoms; ++a) {
+        if (nproj[a] < 1) return fail(c, CSF_EINVAL, "nproj must be >= 1");
+        if (atom_type[a] < 0 || atom_type[a] >= ntypes) return fail(c, CSF_EINVAL, "atom_type out of range");
+        if (delta_ptr[atom_type[a] + 1] - delta_ptr[atom_type[a]] != (int64_t)4 * nproj[a] * nproj[a]) return fail(c, CSF_EINVAL, "Delta size does not match nproj");
+        if (node_ptr[a + 1] < node_ptr[a]) return fail(c, CSF_EINVAL, "node_ptr not monotone");
+        npj_max = std::max(npj_max, nproj[a]); uniform = uniform && nproj[a] == nproj[0];
+    }
+    if (npj_max > 32) return fail(c, CSF_EUNSUPPORTED, "more than 32 projectors per atom");
+    const long long nent = node_ptr[natoms];
+    if (nent >= (1LL << 31)) return fail(c, CSF_EUNSUPPORTED, "too many projector entries");
+    for (long long t = 0; t < nent; ++t) if (node_idx[t] < 0 || node_idx[t] >= c->M) return fail(c, CSF_EINVAL, "node_idx out of range");
+    const int p = c->p, npjp = (npj_max + 1) / 2 * 2;
+    std::vector<double> mass((size_t)c->M);
+    csf_mass_diag(c, mass.data());
+    // owner cell and local index of every support node; sort each atom's entries by (cell, lz, ly, lx)
+    struct Ent { int cell, lz, ly, lx; long long t; };
+    std::vector<int> ent_node((size_t)nent), ent_loc((size_t)nent);
+    std::vector<double> ent_p((size_t)nent * npjp, 0.0);
+    std::vector<long long> atom_coff(natoms); std::vector<int> atom_npj(nproj, nproj + natoms), atom_ty(atom_type, atom_type + natoms);
+    std::vector<int> gb_atom, gb_beg, gb_end;
+    struct Pair { int cell, atom; int off[kTabN + 1]; };
+    std::vector<Pair> pairs;
+    long long pv_off = 0, crows = 0;
+    std::vector<Ent> ents;
+    for (int a = 0; a < natoms; ++a) {
+        atom_coff[a] = crows; crows += 2 * nproj[a];
+        const long long t0 = node_ptr[a], t1 = node_ptr[a + 1];
+        ents.clear(); ents.reserve(t1 - t0);
+        for (long long t = t0; t < t1; ++t) {
+            long long I = node_idx[t]; int g[3] = { (int)(I % c->nfree[0]), (int)((I / c->nfree[0]) % c->nfree[1]), (int)(I / ((long long)c->nfree[0] * c->nfree[1])) };
+            int cl[3], lo[3];
+            for (int d = 0; d < 3; ++d) { int f = g[d] + (c->bc[d] == CSF_BC_DIRICHLET ? 1 : 0); cl[d] = f / p; lo[d] = f % p; }
+            ents.push_back({ cl[0] + c->ncell[0] * (cl[1] + c->ncell[1] * cl[2]), lo[2], lo[1], lo[0], t });
+        }
+        std::sort(ents.begin(), ents.end(), [](const Ent& x, const Ent& y) {
+            if (x.cell != y.cell) return x.cell < y.cell; if (x.lz != y.lz) return x.lz < y.lz; if (x.ly != y.ly) return x.ly < y.ly; return x.lx < y.lx; });
+        for (size_t q = 1; q < ents.size(); ++q)
+            if (ents[q].cell == ents[q - 1].cell && ents[q].lz == ents[q - 1].lz && ents[q].ly == ents[q - 1].ly && ents[q].lx == ents[q - 1].lx)
+                return fail(c, CSF_EINVAL, "duplicate node in an atom's support");
+        for (size_t q = 0; q < ents.size(); ++q) {
+            const long long e = t0 + (long long)q, t = ents[q].t, I = node_idx[t];
+            ent_node[e] = (int)I; ent_loc[e] = ents[q].ly * p + ents[q].lx;
+            const double s = 1.0 / std::sqrt(mass[I]);
+            for (int x = 0; x < nproj[a]; ++x) ent_p[(size_t)e * npjp + x] = s * pvals[pv_off + (t - t0) * nproj[a] + x];
+            if (q == 0 || ents[q].cell != ents[q - 1].cell) {
+                Pair pr; pr.cell = ents[q].cell; pr.atom = a;
+                for (int k = 0; k <= p; ++k) pr.off[k] = (int)e;
+                pairs.push_back(pr);
+            }
+            Pair& pr = pairs.back();
+            for (int k = ents[q].lz + 1; k <= p; ++k) pr.off[k] = (int)e + 1;
+        }
+        for (long long b = t0; b < t1; b += 256) { gb_atom.push_back(a); gb_beg.push_back((int)b); gb_end.push_back((int)std::min(b + 256, t1)); }
+        pv_off += (t1 - t0) * nproj[a];
+    }
+    // cell-major pair lists
+    std::vector<int> pair_ptr(c->E + 1, 0);
+    for (const Pair& pr : pairs) pair_ptr[pr.cell + 1]++;
+    for (int e = 0; e < c->E; ++e) pair_ptr[e + 1] += pair_ptr[e];
+    std::vector<int> fill(pair_ptr.begin(), pair_ptr.end() - 1), pair_atom(pairs.size()), pair_off(pairs.size() * (p + 1));
+    for (const Pair& pr : pairs) { int s = fill[pr.cell]++; pair_atom[s] = pr.atom; for (int k = 0; k <= p; ++k) pair_off[(size_t)s * (p + 1) + k] = pr.off[k]; }
+    std::vector<double2> dl((size_t)delta_ptr[ntypes]);
+    for (size_t i = 0; i < dl.size(); ++i) dl[i] = make_double2(delta[i].re, delta[i].im);
+    std::vector<long long> dptr(delta_ptr, delta_ptr + ntypes + 1);
+    CSF_CUDA(c, c->d_pair_ptr.upload(pair_ptr)); CSF_CUDA(c, c->d_pair_atom.upload(pair_atom)); CSF_CUDA(c, c->d_pair_off.upload(pair_off));
+    CSF_CUDA(c, c->d_ent_loc.upload(ent_loc)); CSF_CUDA(c, c->d_ent_node.upload(ent_node)); CSF_CUDA(c, c->d_ent_p.upload(ent_p));
+    CSF_CUDA(c, c->d_atom_coff.upload(atom_coff)); CSF_CUDA(c, c->d_atom_npj.upload(atom_npj)); CSF_CUDA(c, c->d_atom_type.upload(atom_ty));
+    CSF_CUDA(c, c->d_delta.upload(dl)); CSF_CUDA(c, c->d_delta_ptr.upload(dptr));
+    CSF_CUDA(c, c->d_gb_atom.upload(gb_atom)); CSF_CUDA(c, c->d_gb_beg.upload(gb_beg)); CSF_CUDA(c, c->d_gb_end.upload(gb_end));
+    c->natoms = natoms; c->crows = crows; c->npjp = npjp; c->npj_uniform = uniform ? nproj[0] : 0;
+    c->n_gather_blocks = (int)gb_atom.size();
+    return CSF_OK;
+}
+
+int csf_workspace_bytes(const csf_ctx* c, int nvec, int mode, size_t* bytes) {
+    if (!c || !bytes || nvec < 0) return CSF_EINVAL;
+    if (mode != CSF_FP64) return CSF_EUNSUPPORTED;
+    *bytes = block_bytes(c, nvec) + 2 * coef_bytes(c, nvec) + 256;
+    return CSF_OK;
+}
+
+int csf_apply_H(csf_ctx* c, const csf_c128* dX, csf_c128* dY, int64_t ld, int nvec, void* d_work, size_t work_bytes) {
+    if (!c) return CSF_EINVAL;
+    const size_t need = c->natoms > 0 ? 2 * coef_bytes(c, std::max(nvec, 0)) : 0;
+    int rc = check_block_args(c, dX, dY, ld, nvec, d_work, work_bytes, need);
+    if (rc != CSF_OK || nvec == 0) return rc;
+    CSF_CUDA(c, cudaSetDevice(c->device));
+    double* dC = static_cast<double*>(d_work);
+    double* dCt = reinterpret_cast<double*>(static_cast<char*>(d_work) + coef_bytes(c, nvec));
+    rc = enqueue_zero(c, reinterpret_cast<double*>(dY), ld, nvec);
+    if (rc != CSF_OK) return rc;
+    return enqueue_step(c, reinterpret_cast<const double*>(dX), ld, reinterpret_cast<double*>(dY), ld, nvec, 1.0, 0, 0.0, dC, dCt);
+}
+
+int csf_filter(csf_ctx* c, const csf_c128* dX, csf_c128* dY, int64_t ld, int nvec, int degree, double a, double b, int mode,
+               void* d_work, size_t work_bytes) {
+    if (!c) return CSF_EINVAL;
+    if (mode == CSF_FP32_INTERMEDIATE) return fail(c, CSF_EUNSUPPORTED, "CSF_FP32_INTERMEDIATE is not built yet");
+    if (mode != CSF_FP64) return fail(c, CSF_EINVAL, "unknown mode");
+    if (degree < 0) return fail(c, CSF_EINVAL, "degree < 0");
+    if (!(a < b)) return fail(c, CSF_EINVAL, "need a < b");
+    size_t need = 0;
+    if (nvec > 0) csf_workspace_bytes(c, nvec, mode, &need);
+    int rc = check_block_args(c, dX, dY, ld, nvec, d_work, work_bytes, degree >= 1 ? need : 0);
+    if (rc != CSF_OK || nvec == 0) return rc;
+    CSF_CUDA(c, cudaSetDevice(c->device));
+    const long long rows = 2 * c->M;
+    const double cc = 0.5 * (a + b), ee = 0.5 * (b - a);
+    const double2* X = reinterpret_cast<const double2*>(dX);
+    double* Y = reinterpret_cast<double*>(dY);
+    if (degree == 0) {
+        rot_copy_kernel<<<c->sm_count * 8, 256, 0, c->stream>>>(X, ld, reinterpret_cast<double2*>(Y), ld, rows, nvec, 0);
+        CSF_CUDA(c, cudaGetLastError()); c->launches += 1;
+        return CSF_OK;
+    }
+    char* w = static_cast<char*>(d_work);
+    double* Wk = reinterpret_cast<double*>(w);                              // the second block buffer, [2M][nvec]
+    double* dC = reinterpret_cast<double*>(w + block_bytes(c, nvec));
+    double* dCt = reinterpret_cast<double*>(w + block_bytes(c, nvec) + coef_bytes(c, nvec));
+    // W_k = i^(m-k) T_k(H~) X, so that W_{k+1} = W_{k-1} + (-2i/e)(Hhat - c) W_k and W_m = T_m(H~) X.
+    // W_0 lives in the buffer that also receives W_m: Y if m is even, the workspace block if m is odd.
+    const bool even_m = (degree % 2 == 0);
+    double* buf0 = even_m ? Y : Wk;  const long long ld0 = even_m ? ld : nvec;
+    double* buf1 = even_m ? Wk : Y;  const long long ld1 = even_m ? nvec : ld;
+    if (degree >= 2) {
+        rot_copy_kernel<<<c->sm_count * 8, 256, 0, c->stream>>>(X, ld, reinterpret_cast<double2*>(buf0), ld0, rows, nvec, degree & 3);   // W_0 = i^m X
+        CSF_CUDA(c, cudaGetLastError()); c->launches += 1;
+    }
+    rc = enqueue_zero(c, buf1, ld1, nvec); if (rc != CSF_OK) return rc;
+    // W_1 = (i^(m-1)/e)(Hhat - c) X
+    rc = enqueue_step(c, reinterpret_cast<const double*>(dX), ld, buf1, ld1, nvec, 1.0 / ee, (degree + 3) & 3, cc, dC, dCt);
+    if (rc != CSF_OK) return rc;
+    for (int k = 1; k < degree; ++k) {
+        const bool odd = (k & 1);
+        rc = enqueue_step(c, odd ? buf1 : buf0, odd ? ld1 : ld0, odd ? buf0 : buf1, odd ? ld0 : ld1, nvec, 2.0 / ee, 3, cc, dC, dCt);
+        if (rc != CSF_OK) return rc;
+    }
+    return CSF_OK;
+}
+
+int csf_filter_host(csf_ctx* c, const csf_c128* hX, csf_c128* hY, int64_t ld, int nvec, int degree, double a, double b, int mode) {
+    if (!c) return CSF_EINVAL;
+    if (!hX || !hY) return fail(c, CSF_EINVAL, "NULL host block pointer");
+    if (nvec < 0 || ld < nvec) return fail(c, CSF_EINVAL, "need 0 <= nvec <= ld");
+    if (nvec == 0) return CSF_OK;
+    CSF_CUDA(c, cudaSetDevice(c->device));
+    size_t wb = 0;
+    int rc = csf_workspace_bytes(c, nvec, mode, &wb); if (rc != CSF_OK) return fail(c, rc, "unsupported mode");
+    const size_t bb = (size_t)2 * c->M * ld * sizeof(double2);
+    if (c->h_x.bytes < bb) CSF_CUDA(c, c->h_x.alloc(bb));
+    if (c->h_y.bytes < bb) CSF_CUDA(c, c->h_y.alloc(bb));
+    if (c->h_w.bytes < wb) CSF_CUDA(c, c->h_w.alloc(wb));
+    CSF_CUDA(c, cudaMemcpyAsync(c->h_x.p, hX, bb, cudaMemcpyHostToDevice, c->stream));
+    rc = csf_filter(c, static_cast<const csf_c128*>(c->h_x.p), static_cast<csf_c128*>(c->h_y.p), ld, nvec, degree, a, b, mode, c->h_w.p, c->h_w.bytes);
+    if (rc != CSF_OK) return rc;
+    CSF_CUDA(c, cudaMemcpyAsync(hY, c->h_y.p, bb, cudaMemcpyDeviceToHost, c->stream));
+    CSF_CUDA(c, cudaStreamSynchronize(c->stream));
+    return CSF_OK;
+}
+
+int csf_launch_count(const csf_ctx* c, int64_t* launches) { if (!c || !launches) return CSF_EINVAL; *launches = c->launches; return CSF_OK; }
+
+int csf_set_variant(csf_ctx* c, int variant) {
+    if (!c) return CSF_EINVAL;
+    if (variant < 0 || variant > 3) return fail(c, CSF_EINVAL, "unknown variant");
+    c->variant = variant;
+    return CSF_OK;
+}
+
+}  // extern "C"

@@ -58,11 +58,11 @@ CONFIGS = {
 
 
 def scaled_config(base: Config, ncell, natoms, nvec=None, degree=None, name=None) -> Config:
-    """Same cell size, order, boundary conditions and atom recipe as `base` on a smaller mesh (parity sub-cases)."""
+    """Same cell size, order and boundary conditions as `base` on a smaller mesh, atoms uniform with separation
+    >= 3 bohr (parity sub-cases and the bounded CPU-baseline sample)."""
     h = [b / c for b, c in zip(base.box, base.ncell)]
-    placement = base.placement if base.placement in ("uniform",) else "uniform_sep3" if base.placement != "slab3" else "slab3"
     return Config(base.index, name or f"{base.name}_sub{ncell[0]}x{ncell[1]}x{ncell[2]}", tuple(ncell),
-                  tuple(h[d] * ncell[d] for d in range(3)), base.order, base.bc, natoms, placement,
+                  tuple(h[d] * ncell[d] for d in range(3)), base.order, base.bc, natoms, "uniform_sep3",
                   nvec or base.nvec, degree or base.degree, 0, base.seed)
 
 

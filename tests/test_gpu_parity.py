@@ -1,0 +1,161 @@
+"""GPU parity: libcsf (through the C ABI) against the CPU oracle, element by element, on the same seeded inputs.
+
+Tolerance: relative Frobenius error <= 1e-11 in FP64 (BASELINE.json north_star). The result is unique up to
+rounding (the summation order of the scatter-add is not fixed), so nothing but the tolerance is compared.
+"""
+import numpy as np
+import pytest
+
+from paper_2410_02754_b200 import synth, bounds
+from helpers import setup_pair, gpu_apply_H, gpu_filter, rel_fro
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-11
+
+
+def _cfg(ncell, box, order, bc, natoms, nvec=8, degree=6, seed=77, placement="uniform"):
+    return synth.Config(9, "case", tuple(ncell), tuple(box), order, tuple(bc), natoms, placement, nvec, degree, 0, seed)
+
+
+def test_mesh_exports_match_oracle():
+    for cfg in [synth.CONFIGS[0], _cfg((2, 3, 4), (2.0, 3.3, 5.0), 4, (0, 1, 0), 1), _cfg((1, 2, 2), (1.5, 2.0, 2.0), 5, (0, 0, 1), 1)]:
+        ref, gpu, _ = setup_pair(cfg, with_projectors=False)
+        assert gpu.M == ref.M
+        assert np.allclose(gpu.node_coords(), ref.node_coords(), atol=1e-13)
+        assert np.allclose(gpu.mass_diag(), ref.mass_diag(), rtol=1e-13)
+
+
+@pytest.mark.parametrize("order", [1, 2, 3, 4, 5, 6, 7])
+def test_apply_H_all_orders(order):
+    cfg = _cfg((2, 3, 2), (2.2, 3.0, 1.9), order, (0, 0, 0), 2 if order >= 2 else 0, nvec=5)
+    ref, gpu, s = setup_pair(cfg, with_projectors=order >= 2)
+    X = synth.random_block(s.rng, 2 * ref.M, cfg.nvec)
+    assert rel_fro(gpu_apply_H(gpu, X), ref.apply_H(X)) < TOL
+
+
+@pytest.mark.parametrize("variant", [1, 2, 3])
+@pytest.mark.parametrize("nvec,ld", [(16, 16), (13, 13), (5, 9), (1, 1), (33, 40)])
+def test_apply_H_cfg0_variants_and_ragged(variant, nvec, ld):
+    ref, gpu, s = setup_pair(synth.CONFIGS[0])
+    gpu.set_variant(variant)
+    X = synth.random_block(s.rng, 2 * ref.M, nvec)
+    assert rel_fro(gpu_apply_H(gpu, X, ld=ld), ref.apply_H(X)) < TOL
+
+
+@pytest.mark.parametrize("bc", [(0, 0, 1), (1, 1, 1), (1, 0, 0), (0, 1, 0)])
+@pytest.mark.parametrize("order", [3, 5])
+def test_apply_H_dirichlet_and_noncubic(bc, order):
+    cfg = _cfg((3, 2, 4), (3.3, 2.5, 3.0), order, bc, 3, nvec=7)
+    ref, gpu, s = setup_pair(cfg)
+    X = synth.random_block(s.rng, 2 * ref.M, cfg.nvec)
+    assert rel_fro(gpu_apply_H(gpu, X), ref.apply_H(X)) < TOL
+
+
+def test_apply_H_parts_separately():
+    """kinetic only / + V / + B / + projectors: a wrong term cannot hide behind another."""
+    cfg = _cfg((3, 3, 2), (3.0, 3.0, 2.0), 4, (0, 0, 0), 2, nvec=6)
+    ref, gpu, s = setup_pair(cfg)
+    X = synth.random_block(s.rng, 2 * ref.M, cfg.nvec)
+    empty = ([0], [], [], [], [], [], [0])
+    for veff, bxyz, proj in [(np.zeros(ref.M), None, False), (s.veff, None, False), (s.veff, s.bxyz, False), (np.zeros(ref.M), None, True)]:
+        for ctx in (ref, gpu):
+            ctx.set_potential(veff, bxyz)
+            if proj:
+                ctx.set_projectors(s.node_ptr, s.node_idx, s.nproj, s.pvals, s.atom_type, s.delta, s.delta_ptr)
+            else:
+                ctx.set_projectors(*empty)
+        assert rel_fro(gpu_apply_H(gpu, X), ref.apply_H(X)) < TOL
+
+
+def test_single_cell_periodic_directions():
+    cfg = _cfg((1, 1, 3), (1.0, 1.2, 3.0), 3, (0, 0, 0), 0, nvec=4)
+    ref, gpu, s = setup_pair(cfg, with_projectors=False)
+    X = synth.random_block(s.rng, 2 * ref.M, cfg.nvec)
+    assert rel_fro(gpu_apply_H(gpu, X), ref.apply_H(X)) < TOL
+
+
+def test_generic_projector_counts():
+    """Atoms with different numbers of projectors take the generic (non-18) code path."""
+    cfg = _cfg((3, 3, 3), (4.0, 4.0, 4.0), 3, (0, 0, 0), 0, nvec=6)
+    ref, gpu, s = setup_pair(cfg, with_projectors=False)
+    rng = np.random.default_rng(4); M = ref.M
+    nproj = np.array([5, 1, 7], dtype=np.int32); node_ptr = [0]; idx = []; pv = []; dl = []; dptr = [0]
+    for a, npj in enumerate(nproj):
+        sel = np.sort(rng.choice(M, 60 + 10 * a, replace=False)); idx.append(sel); node_ptr.append(node_ptr[-1] + len(sel))
+        pv.append(rng.normal(size=(len(sel), npj)).reshape(-1))
+        A = rng.normal(size=(2 * npj, 2 * npj)) + 1j * rng.normal(size=(2 * npj, 2 * npj)); dl.append((A + A.conj().T).reshape(-1)); dptr.append(dptr[-1] + 4 * npj * npj)
+    args = (node_ptr, np.concatenate(idx), nproj, np.concatenate(pv), np.arange(3, dtype=np.int32), np.concatenate(dl), dptr)
+    ref.set_projectors(*args); gpu.set_projectors(*args)
+    X = synth.random_block(s.rng, 2 * M, cfg.nvec)
+    assert rel_fro(gpu_apply_H(gpu, X), ref.apply_H(X)) < TOL
+
+
+@pytest.mark.parametrize("degree", [0, 1, 2, 3, 8, 9])
+def test_filter_cfg0_degrees(degree, cfg0_oracle):
+    ref, a, b, X = (cfg0_oracle[k] for k in ("ctx", "a", "b", "X"))
+    _, gpu, _ = setup_pair(synth.CONFIGS[0])
+    Yref = ref.filter(X, degree, a, b)
+    assert rel_fro(gpu_filter(gpu, X, degree, a, b), Yref) < TOL
+    assert rel_fro(gpu_filter(gpu, X[:, :11], degree, a, b, ld=14), Yref[:, :11]) < TOL
+
+
+def test_filter_cfg0_against_dense_brute_force(cfg0_oracle):
+    """The GPU result against V T_m(Lambda~) V^H X from a dense eigendecomposition of the oracle's Hhat."""
+    ref, a, b, X = (cfg0_oracle[k] for k in ("ctx", "a", "b", "X"))
+    _, gpu, _ = setup_pair(synth.CONFIGS[0])
+    lam, V = np.linalg.eigh(ref.dense_H()); lt = (lam - 0.5 * (a + b)) / (0.5 * (b - a))
+    t = np.where(np.abs(lt) <= 1, np.cos(8 * np.arccos(np.clip(lt, -1, 1))), np.cosh(8 * np.arccosh(np.maximum(np.abs(lt), 1))))
+    Yb = V @ (t[:, None] * (V.conj().T @ X))
+    assert rel_fro(gpu_filter(gpu, X, 8, a, b), Yb) < TOL
+
+
+@pytest.mark.parametrize("base,ncell,natoms,nvec,degree", [(2, (4, 4, 8), 3, 24, 10), (3, (6, 6, 6), 4, 16, 12), (4, (6, 6, 6), 4, 16, 12)])
+def test_filter_shapes_of_large_configs(base, ncell, natoms, nvec, degree):
+    """Sub-meshes with the cell size, order, boundary conditions and atom recipe of configs 2-4."""
+    cfg = synth.scaled_config(synth.CONFIGS[base], ncell, natoms, nvec=nvec, degree=degree)
+    ref, gpu, s = setup_pair(cfg)
+    a, b, _, _ = bounds.lanczos_bounds(lambda v: ref.apply_H(v), 2 * ref.M)
+    X = synth.random_block(s.rng, 2 * ref.M, nvec)
+    assert rel_fro(gpu_filter(gpu, X, degree, a, b), ref.filter(X, degree, a, b)) < TOL
+
+
+def test_su2_covariance_on_gpu():
+    """BASELINE check 4 on the CUDA path itself (needs no oracle)."""
+    from test_oracle_pins import _su2
+    cfg = synth.CONFIGS[0]
+    ref, gpu, s = setup_pair(cfg, soc_off=True)
+    a, b, _, _ = bounds.lanczos_bounds(lambda v: ref.apply_H(v), 2 * ref.M)
+    X = synth.random_block(s.rng, 2 * ref.M, 8); U, R = _su2(1.1, (0.2, 0.9, -0.4)); M = ref.M
+    rot = lambda Z: (Z.reshape(M, 2, -1).transpose(0, 2, 1) @ U.T).transpose(0, 2, 1).reshape(2 * M, -1)
+    Y = gpu_filter(gpu, X, 8, a, b)
+    gpu.set_potential(s.veff, s.bxyz @ R.T)
+    assert rel_fro(gpu_filter(gpu, np.ascontiguousarray(rot(X)), 8, a, b), rot(Y)) < TOL
+
+
+def test_error_codes():
+    import torch
+    from paper_2410_02754_b200 import binding
+    with pytest.raises(binding.CsfError) as ei:
+        binding.Csf((2, 2, 2), (1.0, 1.0, 1.0), 3, (0, 0, 2))
+    assert ei.value.code == binding.CSF_EUNSUPPORTED
+    with pytest.raises(binding.CsfError) as ei:
+        binding.Csf((2, 0, 2), (1.0, 1.0, 1.0), 3, (0, 0, 0))
+    assert ei.value.code == binding.CSF_EINVAL
+    g = binding.Csf((2, 2, 2), (2.0, 2.0, 2.0), 2, (0, 0, 0))
+    X = torch.zeros((2 * g.M, 4), dtype=torch.complex128, device="cuda"); Y = torch.zeros_like(X); w = torch.empty(1 << 20, dtype=torch.uint8, device="cuda")
+    with pytest.raises(binding.CsfError) as ei:
+        g.apply_H(X, Y, 4, 4, w)
+    assert ei.value.code == binding.CSF_ESTATE
+    g.set_potential(np.zeros(g.M))
+    for kwargs, code in [(dict(ld=3, nvec=4, degree=2, a=0.0, b=1.0), binding.CSF_EINVAL), (dict(ld=4, nvec=4, degree=-1, a=0.0, b=1.0), binding.CSF_EINVAL),
+                         (dict(ld=4, nvec=4, degree=2, a=1.0, b=1.0), binding.CSF_EINVAL), (dict(ld=4, nvec=4, degree=2, a=0.0, b=1.0, mode=1), binding.CSF_EUNSUPPORTED)]:
+        with pytest.raises(binding.CsfError) as ei:
+            g.filter(X, Y, d_work=w, **kwargs)
+        assert ei.value.code == code
+    with pytest.raises(binding.CsfError) as ei:
+        g.filter(X, X, 4, 4, 2, 0.0, 1.0, 0, w)
+    assert ei.value.code == binding.CSF_EINVAL
+    with pytest.raises(binding.CsfError) as ei:
+        g.filter(X, Y, 4, 4, 2, 0.0, 1.0, 0, w[:64])
+    assert ei.value.code == binding.CSF_EINVAL
+    g.filter(X, Y, 4, 0, 2, 0.0, 1.0, 0, w)     # nvec = 0 is a no-op
