@@ -1,0 +1,361 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the Chebyshev-filtered spinor H.X (csf_filter) on B200, one JSON line.
+
+A "step" is one pass of the whole hot path over one block: Y = T_m(H~) X for B spinor vectors, i.e. m
+applications of [projector gather -> Delta -> gather/cell apply/assembly/recurrence].
+metric = spinor DoF x vectors x degree per second (BASELINE.json). Default workload: BASELINE.json configs[3]
+(periodic bulk, 32^3 cells of order 5, 8.19 M spinor DoF, 500 atoms, block of 256, degree 40), the largest
+single-GPU configuration of the roofline target set; `--config k` selects another.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config k] [--impl ours|reference]
+
+N > 1 (under torchrun): the path does not shard (BASELINE.json north_star), so every rank filters its own block
+of states on its own replica of the operator ("replicas only"; the paper's band groups). No
+data-path collective; the only communication is the timing barrier / max-over-ranks.
+
+--impl reference times the CPU oracle (oracle/) on the host cores on a bounded sample of the same workload.
+"""
+import argparse
+import json
+import math
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_2410_02754_b200 import synth  # noqa: E402
+
+METRIC = "Cheb-filtered spinor HX: DoF*vectors*degree/s"
+UNIT = "DoF*vec*deg/s"
+FP64_FMA_PER_CLK_PER_SM = 64          # 4 SMSPs x 16 FP64 lanes (B200 data sheet: 37-40 TF/s FP64 vector at 1.97 GHz)
+SM_COUNT = 148
+
+
+# ----------------------------------------------------------------------------------------------- helpers
+def algorithmic_flops(p, c_ov):
+    """FP64 flops per unit (one spinor DoF x vector x degree) of the algorithm the kernels implement (DESIGN.md
+    'Roofline'): sum-factorised 1/2 K with the rank-one mass form, nodal 2x2 potential, projector gather + expand,
+    recurrence. Returns (cell kernel, projector gather kernel, total)."""
+    n = p + 1
+    kin = (12.0 * n ** 4 + 40.0 * n ** 3) / p ** 3      # 3 dense + 4 rank-one 1-D contractions, re and im
+    pot, rec = 14.0, 10.0
+    expand = 72.0 * c_ov                                # 18 projectors x 2 flops x (re, im) per support row per spin-vector
+    gather = 72.0 * c_ov
+    return kin + pot + rec + expand, gather, kin + pot + rec + expand + gather
+
+
+def shard_states(nstates, nvec, rank, world):
+    """Block indices (of ceil(nstates / nvec) blocks of `nvec` states) owned by `rank`: round robin, no exchange."""
+    nblocks = max(1, math.ceil(nstates / nvec))
+    return [b for b in range(nblocks) if b % world == rank]
+
+
+def reduce_max_time(ms, dist_mod=None):
+    """Max over ranks of a local duration (the only cross-rank operation of the benchmark)."""
+    if dist_mod is None or not dist_mod.is_initialized():
+        return ms
+    import torch
+    dev = "cuda" if dist_mod.get_backend() == "nccl" else "cpu"
+    t = torch.tensor([ms], dtype=torch.float64, device=dev)
+    dist_mod.all_reduce(t, op=dist_mod.ReduceOp.MAX)
+    return float(t.item())
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks and throttle reasons every 200 ms while the timed region runs."""
+    Q = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
+        "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+
+    def __init__(self, device):
+        self.device, self.proc, self.lines = device, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "200", "-i", str(self.device)],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thr = threading.Thread(target=self._read, daemon=True); self.thr.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for ln in self.proc.stdout:
+            self.lines.append(ln.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "power_w_max": float(max(pw)), "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def build_system(cfg, ctx):
+    """Seeded synthetic operator inputs for `cfg` on node coordinates / masses exported by `ctx` (either side)."""
+    sysm = synth.make_system(cfg, ctx.node_coords(), ctx.mass_diag())
+    ctx.set_potential(sysm.veff, sysm.bxyz)
+    ctx.set_projectors(sysm.node_ptr, sysm.node_idx, sysm.nproj, sysm.pvals, sysm.atom_type, sysm.delta, sysm.delta_ptr)
+    return sysm
+
+
+def cpu_sample_config(cfg):
+    """Bounded sample of the workload for the oracle: same cell size, order, boundary conditions, atom density and
+    degree on an 8x8x8-cell sub-mesh (config 0/1: the whole mesh), 16 columns."""
+    if cfg.index <= 1:
+        return synth.Config(cfg.index, cfg.name, cfg.ncell, cfg.box, cfg.order, cfg.bc, cfg.natoms, cfg.placement, min(cfg.nvec, 16), cfg.degree, 0, cfg.seed)
+    nc = tuple(min(8, c) for c in cfg.ncell)
+    frac = float(np.prod(nc)) / float(np.prod(cfg.ncell))
+    return synth.scaled_config(cfg, nc, max(1, int(round(cfg.natoms * frac))), nvec=16, degree=cfg.degree)
+
+
+def run_oracle_sample(cfg, steps=1, warmup=0):
+    """Times the oracle as it stands (oracle/, OpenMP) on the bounded sample; returns (units/s, description, cores, ms/step)."""
+    from oracle import oracle as O
+    from paper_2410_02754_b200 import bounds
+    sc = cpu_sample_config(cfg)
+    ref = O.RefCtx(sc.ncell, sc.box, sc.order, sc.bc)
+    sysm = build_system(sc, ref)
+    a, b, _, _ = bounds.lanczos_bounds(lambda v: ref.apply_H(v), 2 * ref.M, k=10)
+    X = synth.random_block(sysm.rng, 2 * ref.M, sc.nvec)
+    for _ in range(warmup):
+        ref.filter(X[:, :2], 2, a, b)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        ref.filter(X, sc.degree, a, b)
+    dt = (time.perf_counter() - t0) / steps
+    units = 2.0 * ref.M * sc.nvec * sc.degree
+    desc = f"{sc.ncell[0]}x{sc.ncell[1]}x{sc.ncell[2]} cells of order {sc.order} (same cell size, bc, atom density: {sc.natoms} atoms), " \
+           f"{sc.nvec} columns, degree {sc.degree}: {units:.3g} of the workload's {2.0 * cfg.M * cfg.nvec * cfg.degree:.3g} units"
+    return units / dt, desc, O.num_threads(), dt * 1e3
+
+
+def workload_dict(cfg, sysm=None):
+    d = {"workload": f"BASELINE.json configs[{cfg.index}] {cfg.name}", "ncell": list(cfg.ncell), "order": cfg.order,
+         "bc": ["periodic" if b == 0 else "dirichlet" for b in cfg.bc], "spinor_dof": 2 * cfg.M, "block_vectors": cfg.nvec,
+         "degree": cfg.degree, "atoms": cfg.natoms, "projectors_per_atom": synth.N_PROJ,
+         "l2": "inputs larger than L2 (block buffers of %.2f GB each)" % (2 * cfg.M * cfg.nvec * 16 / 1e9)}
+    if sysm is not None:
+        d["c_ov"] = round(sysm.coverage, 4)
+    return d
+
+
+# ----------------------------------------------------------------------------------------------- reference arm
+def main_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    cfg = synth.CONFIGS[args.config]
+    val, desc, cores, ms = run_oracle_sample(cfg, steps=max(1, args.steps), warmup=min(args.warmup, 1))
+    out = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+           "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+           "config": workload_dict(cfg),
+           "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+           "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}
+    print(json.dumps(out))
+    return 0
+
+
+# ----------------------------------------------------------------------------------------------- our arm
+def main_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2410_02754_b200 import binding, bounds
+
+    world = int(os.environ.get("WORLD_SIZE", "1")); rank = int(os.environ.get("RANK", "0")); local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    cfg = synth.CONFIGS[args.config]
+    nvec = args.nvec or cfg.nvec
+    degree = args.degree or cfg.degree
+    stream = torch.cuda.current_stream()
+    ctx = binding.Csf(cfg.ncell, cfg.box, cfg.order, cfg.bc, device=local, stream=stream.cuda_stream)
+    if args.variant:
+        ctx.set_variant(args.variant)
+    t_setup = time.perf_counter()
+    sysm = build_system(cfg, ctx)
+    M = ctx.M; rows = 2 * M
+    wb = ctx.workspace_bytes(nvec)
+    work = torch.empty(max(wb, 16), dtype=torch.uint8, device="cuda")
+
+    # bounds [a, b]: Lanczos on the library's own apply_H (input generation; see bounds.py)
+    x1 = torch.empty((rows, 1), dtype=torch.complex128, device="cuda"); y1 = torch.empty_like(x1)
+
+    def apply_h_host(v):
+        x1.copy_(torch.from_numpy(np.ascontiguousarray(v)).to("cuda"))
+        ctx.apply_H(x1, y1, 1, 1, work)
+        return y1.cpu().numpy()
+
+    a, b, tmin, tmax = bounds.lanczos_bounds(apply_h_host, rows, k=20)
+    del x1, y1
+
+    # this rank's block of states (band group): a different seed per block index
+    my_blocks = shard_states(max(cfg.nstates, nvec * world), nvec, rank, world)
+    gen = torch.Generator(device="cuda"); gen.manual_seed(cfg.seed * 1000 + my_blocks[0])
+    X = torch.empty((rows, nvec), dtype=torch.complex128, device="cuda")
+    torch.view_as_real(X).normal_(0.0, math.sqrt(0.5), generator=gen)
+    Y = torch.empty_like(X)
+    t_setup = time.perf_counter() - t_setup
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        ctx.filter(X, Y, nvec, nvec, degree, a, b, 0, work)
+    barrier()
+    for k in range(binding.KIND_AUX + 1):
+        ctx.profile_read(k)
+    ctx.profile_enable(not args.no_profile)
+    l0 = ctx.launch_count()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    barrier()
+    e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(args.steps):
+        ctx.filter(X, Y, nvec, nvec, degree, a, b, 0, work)
+    e1.record(stream)
+    barrier()
+    clocks = sampler.stop() if rank == 0 else None
+    ms_local = e0.elapsed_time(e1)
+    ms = reduce_max_time(ms_local, dist if world > 1 else None)
+    launches = ctx.launch_count() - l0
+    kinds = {binding.KIND_NAMES[k]: ctx.profile_read(k) for k in range(binding.KIND_AUX + 1)}
+    ctx.profile_enable(False)
+    ms_per_step = ms / args.steps
+    units_step = float(rows) * nvec * degree
+    value = world * units_step / (ms_per_step * 1e-3)
+    finite = bool(torch.isfinite(torch.view_as_real(Y)).all().item())
+
+    # ---- roofline of the dominant kernel (cell kernel) and of the whole step
+    f_cell, f_gather, f_total = algorithmic_flops(cfg.order, sysm.coverage)
+    peaks = {}
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            peaks = json.load(f)
+    except OSError:
+        pass
+    sm_max = float(peaks.get("sm_max_mhz", 1965.0))
+    peak_alu = SM_COUNT * FP64_FMA_PER_CLK_PER_SM * 2 * sm_max * 1e6 / 1e12
+    hbm = float(peaks.get("hbm_gbs", 6650.0))
+    cell_ms, cell_n = kinds["cell"]
+    roof = None
+    if cell_n > 0:
+        t_cell = cell_ms / cell_n * 1e-3
+        ach = f_cell * rows * nvec / t_cell / 1e12
+        roof = {"kernel": "cell_kernel (a1-a4, a7, a8)", "bound": "alu", "achieved": ach, "peak": peak_alu, "unit": "TFLOP/s", "frac": ach / peak_alu,
+                "peak_source": "148 SMs x 64 FP64 FMA/clk x 2 x %.0f MHz (DESIGN.md)" % sm_max, "traffic": None,
+                "flops_per_unit": f_cell, "avg_launch_ms": t_cell * 1e3, "launches": cell_n,
+                "share_of_step": cell_ms / ms_local,
+                "hbm_achieved_gbs": 48.0 * rows * nvec / t_cell / 1e9, "hbm_peak_gbs": hbm, "hbm_frac": 48.0 * rows * nvec / t_cell / 1e9 / hbm,
+                "hbm_peak_source": "measured (MEASURED_PEAKS.json)" if peaks else "fallback"}
+        if not args.no_probe:
+            pf, pm = binding.probe_fp64_peak(local)
+            roof["peak_measured_dfma"] = pf; roof["peak_measured_dmma"] = pm; roof["frac_of_measured_dfma"] = ach / pf
+    step = {"flops_per_unit": f_total, "tflops": f_total * units_step / (ms_per_step * 1e-3) / 1e12,
+            "frac_alu": f_total * units_step / (ms_per_step * 1e-3) / 1e12 / peak_alu,
+            "hbm_gbs": 48.0 * units_step / (ms_per_step * 1e-3) / 1e9, "frac_hbm": 48.0 * units_step / (ms_per_step * 1e-3) / 1e9 / hbm,
+            "kernel_ms": {k: round(v[0] / args.steps, 3) for k, v in kinds.items()}}
+
+    # ---- end to end: host buffers through csf_filter_host (H2D + filter + D2H inside the timed region)
+    e2e = None
+    if not args.no_e2e:
+        import psutil
+        e2e_nvec = nvec
+        need = 2 * rows * 16
+        avail = psutil.virtual_memory().available / max(1, world)
+        while e2e_nvec > 8 and need * e2e_nvec > 0.7 * avail:
+            e2e_nvec //= 2
+        hX = torch.empty((rows, e2e_nvec), dtype=torch.complex128, pin_memory=True)
+        hX.copy_(X[:, :e2e_nvec])
+        del X, Y, work
+        torch.cuda.empty_cache()
+        hY = torch.empty((rows, e2e_nvec), dtype=torch.complex128, pin_memory=True)
+        ctx.set_host_chunk(args.host_chunk)
+        e2e_steps = max(1, min(args.steps, args.e2e_steps))
+        ctx.filter_host(hX, hY, e2e_nvec, min(e2e_nvec, 2 * args.host_chunk), min(degree, 2), a, b, 0)   # warm-up: allocates both staging slots
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(e2e_steps):
+            ctx.filter_host(hX, hY, e2e_nvec, e2e_nvec, degree, a, b, 0)
+        torch.cuda.synchronize()
+        dt_ms = (time.perf_counter() - t0) * 1e3
+        barrier()
+        dt_ms = reduce_max_time(dt_ms, dist if world > 1 else None)
+        ev = world * float(rows) * e2e_nvec * degree / (dt_ms / e2e_steps * 1e-3)
+        e2e = {"value": ev, "unit": UNIT, "h2d_bytes_per_step": rows * e2e_nvec * 16, "d2h_bytes_per_step": rows * e2e_nvec * 16,
+               "steps": e2e_steps, "ms_per_step": dt_ms / e2e_steps, "block_vectors": e2e_nvec, "host_chunk_columns": args.host_chunk,
+               "api": "csf_filter_host (pinned host X, Y; column chunks staged H2D / filtered / D2H on three streams)",
+               "finite": bool(torch.isfinite(torch.view_as_real(hY[::4097])).all().item())}
+        del hX, hY
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        v, desc, cores, _ = run_oracle_sample(cfg)
+        cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
+
+    if rank == 0:
+        conf = workload_dict(cfg, sysm)
+        conf.update({"block_vectors": nvec, "degree": degree, "bounds": [a, b], "lanczos_ritz": [tmin, tmax], "parallelism": f"replicas x{world}" if world > 1 else "single GPU",
+                     "setup_s": round(t_setup, 2)})
+        out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step,
+               "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": conf,
+               "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roof, "step_roofline": step, "cpu_baseline": cpu, "finite": finite}
+        print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=3, choices=sorted(synth.CONFIGS))
+    ap.add_argument("--nvec", type=int, default=0, help="override the block width (not a bench value)")
+    ap.add_argument("--degree", type=int, default=0, help="override the degree (not a bench value)")
+    ap.add_argument("--variant", type=int, default=0)
+    ap.add_argument("--host-chunk", type=int, default=64)
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-profile", action="store_true")
+    ap.add_argument("--no-probe", action="store_true")
+    args = ap.parse_args()
+    return main_reference(args) if args.impl == "reference" else main_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

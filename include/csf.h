@@ -123,6 +123,22 @@ int csf_filter(csf_ctx* ctx, const csf_c128* dX, csf_c128* dY, int64_t ld, int n
 int csf_filter_host(csf_ctx* ctx, const csf_c128* hX, csf_c128* hY, int64_t ld, int nvec,
                     int degree, double a, double b, int mode);
 
+/* Columns per staged chunk of csf_filter_host (default 64; >= 1). */
+int csf_set_host_chunk(csf_ctx* ctx, int ncols);
+
+/* Per-kernel CUDA-event timing. While enabled, every kernel the context launches is bracketed by two events
+ * on the context's stream. csf_profile_read SYNCHRONISES the stream, returns the summed device time (ms) and the
+ * number of launches of `kind` since the last read, and clears that kind. kind: CSF_KIND_CELL (gather -> cell-level
+ * local apply -> assembly and recurrence update, a1-a4, a7, a8), CSF_KIND_PGATHER (a5), CSF_KIND_DELTA (a6),
+ * CSF_KIND_AUX (block copy / zero). */
+enum { CSF_KIND_CELL = 0, CSF_KIND_PGATHER = 1, CSF_KIND_DELTA = 2, CSF_KIND_AUX = 3, CSF_NKINDS = 4 };
+int csf_profile_enable(csf_ctx* ctx, int on);
+int csf_profile_read(csf_ctx* ctx, int kind, double* ms_total, int64_t* launches);
+
+/* Measure the FP64 arithmetic peaks of `device` with register-resident loops (no memory traffic): tflops_fma from
+ * independent DFMA chains, tflops_mma from mma.sync m8n8k4 f64 (DMMA) chains. Synchronises. Either pointer may be NULL. */
+int csf_probe_fp64_peak(int device, double* tflops_fma, double* tflops_mma);
+
 /* Number of kernel launches (own kernels only, memsets excluded) enqueued by this context so far. */
 int csf_launch_count(const csf_ctx* ctx, int64_t* launches);
 

@@ -16,8 +16,10 @@ CSF_BC_PERIODIC, CSF_BC_DIRICHLET, CSF_BC_FREE = 0, 1, 2
 CSF_FP64, CSF_FP32_INTERMEDIATE = 0, 1
 
 EXPORTS = ["csf_create", "csf_destroy", "csf_set_stream", "csf_num_nodes", "csf_node_coords", "csf_mass_diag", "csf_set_potential",
-           "csf_set_projectors", "csf_workspace_bytes", "csf_apply_H", "csf_filter", "csf_filter_host", "csf_launch_count",
-           "csf_set_variant", "csf_last_error"]
+           "csf_set_projectors", "csf_workspace_bytes", "csf_apply_H", "csf_filter", "csf_filter_host", "csf_set_host_chunk",
+           "csf_profile_enable", "csf_profile_read", "csf_probe_fp64_peak", "csf_launch_count", "csf_set_variant", "csf_last_error"]
+KIND_CELL, KIND_PGATHER, KIND_DELTA, KIND_AUX = 0, 1, 2, 3
+KIND_NAMES = ("cell", "proj_gather", "delta", "aux")
 
 _lib = None
 
@@ -132,8 +134,29 @@ class Csf:
         self._chk(self._L.csf_filter_host(self._h, hp(hX), hp(hY), C.c_int64(int(ld)), C.c_int(int(nvec)), C.c_int(int(degree)),
                                           C.c_double(float(a)), C.c_double(float(b)), C.c_int(mode)))
 
+    def set_host_chunk(self, ncols):
+        self._chk(self._L.csf_set_host_chunk(self._h, C.c_int(int(ncols))))
+
+    def profile_enable(self, on=True):
+        self._chk(self._L.csf_profile_enable(self._h, C.c_int(1 if on else 0)))
+
+    def profile_read(self, kind):
+        """(summed device ms, launches) of kernel kind since the last read; synchronises the stream."""
+        ms = C.c_double(); n = C.c_int64()
+        self._chk(self._L.csf_profile_read(self._h, C.c_int(int(kind)), C.byref(ms), C.byref(n)))
+        return float(ms.value), int(n.value)
+
     def launch_count(self):
         n = C.c_int64(); self._chk(self._L.csf_launch_count(self._h, C.byref(n))); return int(n.value)
 
     def set_variant(self, variant):
         self._chk(self._L.csf_set_variant(self._h, C.c_int(int(variant))))
+
+
+def probe_fp64_peak(device=0):
+    """(TFLOP/s of a register-resident DFMA loop, TFLOP/s of a DMMA m8n8k4 loop) measured on `device`."""
+    f = C.c_double(); m = C.c_double()
+    rc = lib().csf_probe_fp64_peak(C.c_int(int(device)), C.byref(f), C.byref(m))
+    if rc != CSF_OK:
+        raise CsfError(rc, lib().csf_last_error(None).decode())
+    return float(f.value), float(m.value)

@@ -48,8 +48,20 @@ struct csf_ctx {
     long long launches = 0;
     int sm_count = 148; size_t smem_optin = 0;
     std::string err;
-    // scratch for csf_filter_host
-    DevBuf h_x, h_y, h_w;
+    // csf_filter_host: two (x, y) column-chunk slots + one workspace, copy streams and events
+    DevBuf h_x[2], h_y[2], h_w;
+    cudaStream_t hs_in = nullptr, hs_out = nullptr;
+    cudaEvent_t ev_in[2] = {nullptr, nullptr}, ev_cmp[2] = {nullptr, nullptr}, ev_out[2] = {nullptr, nullptr};
+    int host_chunk = 64;
+    // per-kernel-kind CUDA-event timing (csf_profile_*)
+    bool prof = false;
+    std::vector<std::pair<cudaEvent_t, cudaEvent_t>> prof_ev[CSF_NKINDS];
+    ~csf_ctx() {
+        for (auto& v : prof_ev) for (auto& pr : v) { cudaEventDestroy(pr.first); cudaEventDestroy(pr.second); }
+        for (int s = 0; s < 2; ++s) { if (ev_in[s]) cudaEventDestroy(ev_in[s]); if (ev_cmp[s]) cudaEventDestroy(ev_cmp[s]); if (ev_out[s]) cudaEventDestroy(ev_out[s]); }
+        if (hs_in) cudaStreamDestroy(hs_in);
+        if (hs_out) cudaStreamDestroy(hs_out);
+    }
 };
 
 namespace {
@@ -57,6 +69,17 @@ namespace {
 int fail(csf_ctx* c, int code, const std::string& msg) { if (c) c->err = msg; else g_create_error = msg; return code; }
 int cuda_fail(csf_ctx* c, cudaError_t e, const char* what) { return fail(c, CSF_ECUDA, std::string(what) + ": " + cudaGetErrorString(e)); }
 #define CSF_CUDA(ctx, call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) return cuda_fail(ctx, e__, #call); } while (0)
+
+// brackets one kernel launch with two events when profiling is on
+struct ProfScope {
+    csf_ctx* c; int kind; cudaEvent_t e0 = nullptr, e1 = nullptr;
+    ProfScope(csf_ctx* c_, int kind_) : c(c_), kind(kind_) {
+        if (!c->prof) return;
+        if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) { e0 = e1 = nullptr; return; }
+        cudaEventRecord(e0, c->stream);
+    }
+    ~ProfScope() { if (e1) { cudaEventRecord(e1, c->stream); c->prof_ev[kind].push_back({e0, e1}); } }
+};
 
 inline int lanes_of_variant(int v) { return v == 1 ? 32 : v == 2 ? 16 : v == 3 ? 8 : 0; }
 
@@ -125,15 +148,18 @@ int enqueue_step(csf_ctx* c, const double* src, long long ld, double* dst, long 
         gp.atom_coff = c->d_atom_coff.as<long long>(); gp.atom_npj = c->d_atom_npj.as<int>();
         gp.C = dC; gp.ldc = ldc;
         dim3 gg(c->n_gather_blocks, (nvec + 7) / 8);
-        if (c->npj_uniform == 18) proj_gather_kernel<18><<<gg, 128, 0, c->stream>>>(gp);
-        else proj_gather_kernel<0><<<gg, 128, 0, c->stream>>>(gp);
+        {
+            ProfScope ps(c, CSF_KIND_PGATHER);
+            if (c->npj_uniform == 18) proj_gather_kernel<18><<<gg, 128, 0, c->stream>>>(gp);
+            else proj_gather_kernel<0><<<gg, 128, 0, c->stream>>>(gp);
+        }
         CSF_CUDA(c, cudaGetLastError());
         DeltaParams dp{};
         dp.C = reinterpret_cast<const double2*>(dC); dp.Ct = reinterpret_cast<double2*>(dCt); dp.ldc = ldc; dp.nvec = nvec;
         dp.atom_coff = c->d_atom_coff.as<long long>(); dp.atom_npj = c->d_atom_npj.as<int>(); dp.atom_type = c->d_atom_type.as<int>();
         dp.delta = c->d_delta.as<double2>(); dp.delta_ptr = c->d_delta_ptr.as<long long>();
         dim3 dg(c->natoms, (nvec + 31) / 32);
-        delta_apply_kernel<<<dg, 256, 0, c->stream>>>(dp);
+        { ProfScope ps(c, CSF_KIND_DELTA); delta_apply_kernel<<<dg, 256, 0, c->stream>>>(dp); }
         CSF_CUDA(c, cudaGetLastError());
         c->launches += 2;
     }
@@ -160,7 +186,10 @@ int enqueue_step(csf_ctx* c, const double* src, long long ld, double* dst, long 
     const int vchunk = L / 4;
     const long long nblocks = (long long)c->E * ((nvec + vchunk - 1) / vchunk);
     if (nblocks > 0x7fffffffLL) return fail(c, CSF_EUNSUPPORTED, "grid too large");
-    CSF_CUDA(c, launch_cell(c->p, L, c->natoms > 0 ? c->npj_uniform : 18, cp, (int)nblocks, cell_smem_bytes(c->p, L), c->stream));
+    {
+        ProfScope ps(c, CSF_KIND_CELL);
+        CSF_CUDA(c, launch_cell(c->p, L, c->natoms > 0 ? c->npj_uniform : 18, cp, (int)nblocks, cell_smem_bytes(c->p, L), c->stream));
+    }
     c->launches += 1;
     return CSF_OK;
 }
@@ -171,7 +200,7 @@ size_t coef_bytes(const csf_ctx* c, int nvec) { return ((size_t)c->crows * nvec 
 int enqueue_zero(csf_ctx* c, double* dst, long long ld, int nvec) {
     const long long rows = 2 * c->M;
     if (ld == nvec) { CSF_CUDA(c, cudaMemsetAsync(dst, 0, (size_t)rows * ld * sizeof(double2), c->stream)); return CSF_OK; }
-    zero_kernel<<<c->sm_count * 8, 256, 0, c->stream>>>(reinterpret_cast<double2*>(dst), rows, ld, nvec);
+    { ProfScope ps(c, CSF_KIND_AUX); zero_kernel<<<c->sm_count * 8, 256, 0, c->stream>>>(reinterpret_cast<double2*>(dst), rows, ld, nvec); }
     CSF_CUDA(c, cudaGetLastError());
     c->launches += 1;
     return CSF_OK;
@@ -423,7 +452,7 @@ int csf_filter(csf_ctx* c, const csf_c128* dX, csf_c128* dY, int64_t ld, int nve
     const double2* X = reinterpret_cast<const double2*>(dX);
     double* Y = reinterpret_cast<double*>(dY);
     if (degree == 0) {
-        rot_copy_kernel<<<c->sm_count * 8, 256, 0, c->stream>>>(X, ld, reinterpret_cast<double2*>(Y), ld, rows, nvec, 0);
+        { ProfScope ps(c, CSF_KIND_AUX); rot_copy_kernel<<<c->sm_count * 8, 256, 0, c->stream>>>(X, ld, reinterpret_cast<double2*>(Y), ld, rows, nvec, 0); }
         CSF_CUDA(c, cudaGetLastError()); c->launches += 1;
         return CSF_OK;
     }
@@ -437,7 +466,7 @@ int csf_filter(csf_ctx* c, const csf_c128* dX, csf_c128* dY, int64_t ld, int nve
     double* buf0 = even_m ? Y : Wk;  const long long ld0 = even_m ? ld : nvec;
     double* buf1 = even_m ? Wk : Y;  const long long ld1 = even_m ? nvec : ld;
     if (degree >= 2) {
-        rot_copy_kernel<<<c->sm_count * 8, 256, 0, c->stream>>>(X, ld, reinterpret_cast<double2*>(buf0), ld0, rows, nvec, degree & 3);   // W_0 = i^m X
+        { ProfScope ps(c, CSF_KIND_AUX); rot_copy_kernel<<<c->sm_count * 8, 256, 0, c->stream>>>(X, ld, reinterpret_cast<double2*>(buf0), ld0, rows, nvec, degree & 3); }   // W_0 = i^m X
         CSF_CUDA(c, cudaGetLastError()); c->launches += 1;
     }
     rc = enqueue_zero(c, buf1, ld1, nvec); if (rc != CSF_OK) return rc;
@@ -456,19 +485,107 @@ int csf_filter_host(csf_ctx* c, const csf_c128* hX, csf_c128* hY, int64_t ld, in
     if (!c) return CSF_EINVAL;
     if (!hX || !hY) return fail(c, CSF_EINVAL, "NULL host block pointer");
     if (nvec < 0 || ld < nvec) return fail(c, CSF_EINVAL, "need 0 <= nvec <= ld");
+    if (degree < 0) return fail(c, CSF_EINVAL, "degree < 0");
+    if (!(a < b)) return fail(c, CSF_EINVAL, "need a < b");
+    if (!c->have_pot) return fail(c, CSF_ESTATE, "csf_set_potential has not been called");
     if (nvec == 0) return CSF_OK;
     CSF_CUDA(c, cudaSetDevice(c->device));
+    const int chunk = std::min(c->host_chunk, nvec);
+    const int nch = (nvec + chunk - 1) / chunk;
     size_t wb = 0;
-    int rc = csf_workspace_bytes(c, nvec, mode, &wb); if (rc != CSF_OK) return fail(c, rc, "unsupported mode");
-    const size_t bb = (size_t)2 * c->M * ld * sizeof(double2);
-    if (c->h_x.bytes < bb) CSF_CUDA(c, c->h_x.alloc(bb));
-    if (c->h_y.bytes < bb) CSF_CUDA(c, c->h_y.alloc(bb));
+    int rc = csf_workspace_bytes(c, chunk, mode, &wb); if (rc != CSF_OK) return fail(c, rc, "unsupported mode");
+    const size_t rows = (size_t)2 * c->M, cb = rows * chunk * sizeof(double2);
+    for (int s = 0; s < (nch > 1 ? 2 : 1); ++s) {
+        if (c->h_x[s].bytes < cb) CSF_CUDA(c, c->h_x[s].alloc(cb));
+        if (c->h_y[s].bytes < cb) CSF_CUDA(c, c->h_y[s].alloc(cb));
+    }
     if (c->h_w.bytes < wb) CSF_CUDA(c, c->h_w.alloc(wb));
-    CSF_CUDA(c, cudaMemcpyAsync(c->h_x.p, hX, bb, cudaMemcpyHostToDevice, c->stream));
-    rc = csf_filter(c, static_cast<const csf_c128*>(c->h_x.p), static_cast<csf_c128*>(c->h_y.p), ld, nvec, degree, a, b, mode, c->h_w.p, c->h_w.bytes);
-    if (rc != CSF_OK) return rc;
-    CSF_CUDA(c, cudaMemcpyAsync(hY, c->h_y.p, bb, cudaMemcpyDeviceToHost, c->stream));
+    if (!c->hs_in) {
+        CSF_CUDA(c, cudaStreamCreateWithFlags(&c->hs_in, cudaStreamNonBlocking));
+        CSF_CUDA(c, cudaStreamCreateWithFlags(&c->hs_out, cudaStreamNonBlocking));
+        for (int s = 0; s < 2; ++s) {
+            CSF_CUDA(c, cudaEventCreateWithFlags(&c->ev_in[s], cudaEventDisableTiming));
+            CSF_CUDA(c, cudaEventCreateWithFlags(&c->ev_cmp[s], cudaEventDisableTiming));
+            CSF_CUDA(c, cudaEventCreateWithFlags(&c->ev_out[s], cudaEventDisableTiming));
+        }
+    }
+    // chunk i: host->device on hs_in, filter on the context's stream, device->host on hs_out; slot i%2 is reused
+    // only after chunk i-2 has been filtered (x slot) and copied out (y slot), so copies overlap the filter.
+    for (int i = 0; i < nch; ++i) {
+        const int s = i & 1, v0 = i * chunk, nv = std::min(chunk, nvec - v0);
+        const size_t wbytes = (size_t)nv * sizeof(double2);
+        if (i >= 2) CSF_CUDA(c, cudaStreamWaitEvent(c->hs_in, c->ev_cmp[s], 0));
+        CSF_CUDA(c, cudaMemcpy2DAsync(c->h_x[s].p, wbytes, hX + v0, (size_t)ld * sizeof(double2), wbytes, rows, cudaMemcpyHostToDevice, c->hs_in));
+        CSF_CUDA(c, cudaEventRecord(c->ev_in[s], c->hs_in));
+        CSF_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_in[s], 0));
+        if (i >= 2) CSF_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_out[s], 0));
+        rc = csf_filter(c, static_cast<const csf_c128*>(c->h_x[s].p), static_cast<csf_c128*>(c->h_y[s].p), nv, nv, degree, a, b, mode, c->h_w.p, c->h_w.bytes);
+        if (rc != CSF_OK) { cudaDeviceSynchronize(); return rc; }
+        CSF_CUDA(c, cudaEventRecord(c->ev_cmp[s], c->stream));
+        CSF_CUDA(c, cudaStreamWaitEvent(c->hs_out, c->ev_cmp[s], 0));
+        CSF_CUDA(c, cudaMemcpy2DAsync(hY + v0, (size_t)ld * sizeof(double2), c->h_y[s].p, wbytes, wbytes, rows, cudaMemcpyDeviceToHost, c->hs_out));
+        CSF_CUDA(c, cudaEventRecord(c->ev_out[s], c->hs_out));
+    }
+    CSF_CUDA(c, cudaStreamSynchronize(c->hs_out));
     CSF_CUDA(c, cudaStreamSynchronize(c->stream));
+    CSF_CUDA(c, cudaStreamSynchronize(c->hs_in));
+    return CSF_OK;
+}
+
+int csf_set_host_chunk(csf_ctx* c, int ncols) {
+    if (!c) return CSF_EINVAL;
+    if (ncols < 1) return fail(c, CSF_EINVAL, "host chunk must be >= 1");
+    c->host_chunk = ncols;
+    return CSF_OK;
+}
+
+int csf_profile_enable(csf_ctx* c, int on) { if (!c) return CSF_EINVAL; c->prof = on != 0; return CSF_OK; }
+
+int csf_profile_read(csf_ctx* c, int kind, double* ms_total, int64_t* launches) {
+    if (!c || kind < 0 || kind >= CSF_NKINDS) return CSF_EINVAL;
+    CSF_CUDA(c, cudaSetDevice(c->device));
+    CSF_CUDA(c, cudaStreamSynchronize(c->stream));
+    double tot = 0.0;
+    for (auto& pr : c->prof_ev[kind]) {
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, pr.first, pr.second) == cudaSuccess) tot += ms;
+        cudaEventDestroy(pr.first); cudaEventDestroy(pr.second);
+    }
+    if (ms_total) *ms_total = tot;
+    if (launches) *launches = (int64_t)c->prof_ev[kind].size();
+    c->prof_ev[kind].clear();
+    return CSF_OK;
+}
+
+int csf_probe_fp64_peak(int device, double* tflops_fma, double* tflops_mma) {
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) return fail(nullptr, CSF_ECUDA, "no such CUDA device");
+    if (cudaSetDevice(device) != cudaSuccess) return fail(nullptr, CSF_ECUDA, "cudaSetDevice failed");
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return fail(nullptr, CSF_ECUDA, "cudaGetDeviceProperties failed");
+    double* sink = nullptr;
+    if (cudaMalloc(&sink, 1 << 20) != cudaSuccess) return fail(nullptr, CSF_ENOMEM, "cudaMalloc failed");
+    cudaEvent_t e0, e1; cudaEventCreate(&e0); cudaEventCreate(&e1);
+    const int blocks = prop.multiProcessorCount * 8, iters = 4096;
+    double out[2] = {0.0, 0.0};
+    for (int which = 0; which < 2; ++which) {
+        float best = 1e30f;
+        for (int rep = 0; rep < 5; ++rep) {
+            cudaEventRecord(e0, 0);
+            if (which == 0) probe_dfma_kernel<<<blocks, 256>>>(sink, iters, 1.0000001);
+            else probe_dmma_kernel<<<blocks, 256>>>(sink, iters, 1.0000001);
+            cudaEventRecord(e1, 0);
+            if (cudaEventSynchronize(e1) != cudaSuccess) { cudaFree(sink); return fail(nullptr, CSF_ECUDA, "probe kernel failed"); }
+            float ms = 0.f; cudaEventElapsedTime(&ms, e0, e1);
+            if (rep > 0 && ms < best) best = ms;
+        }
+        // DFMA: 8 chains x 2 flops per iteration per thread; DMMA m8n8k4: 8 mma x 512 flops per iteration per warp
+        const double flops = which == 0 ? (double)blocks * 256 * iters * 8 * 2 : (double)blocks * 8 * iters * 8 * 512;
+        out[which] = flops / (best * 1e-3) * 1e-12;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(sink);
+    if (tflops_fma) *tflops_fma = out[0];
+    if (tflops_mma) *tflops_mma = out[1];
     return CSF_OK;
 }
 

@@ -338,4 +338,39 @@ __global__ void __launch_bounds__(256) zero_kernel(double2* __restrict__ dst, lo
     }
 }
 
+// ---------------------------------------------------------------------------------------------------
+// FP64 peak probes (csf_probe_fp64_peak): register-resident dependent chains, no memory traffic.
+// ---------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) probe_dfma_kernel(double* sink, int iters, double m) {
+    double a0 = threadIdx.x, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5, a6 = a0 + 6, a7 = a0 + 7;
+    const double c = 1e-9;
+#pragma unroll 4
+    for (int it = 0; it < iters; ++it) {
+        a0 = fma(a0, m, c); a1 = fma(a1, m, c); a2 = fma(a2, m, c); a3 = fma(a3, m, c);
+        a4 = fma(a4, m, c); a5 = fma(a5, m, c); a6 = fma(a6, m, c); a7 = fma(a7, m, c);
+    }
+    const double s = a0 + a1 + a2 + a3 + a4 + a5 + a6 + a7;
+    if (s == 12345.678) sink[threadIdx.x] = s;
+}
+
+__device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double b) {
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
+}
+
+__global__ void __launch_bounds__(256) probe_dmma_kernel(double* sink, int iters, double m) {
+    double d[8][2];
+#pragma unroll
+    for (int q = 0; q < 8; ++q) { d[q][0] = threadIdx.x + q; d[q][1] = threadIdx.x - q; }
+    const double a = m * 1e-3, b = 1e-3 * (threadIdx.x & 3);
+#pragma unroll 2
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int q = 0; q < 8; ++q) dmma884(d[q][0], d[q][1], a, b);
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int q = 0; q < 8; ++q) s += d[q][0] + d[q][1];
+    if (s == 12345.678) sink[threadIdx.x] = s;
+}
+
 }  // namespace csf
