@@ -142,7 +142,8 @@ int csf_probe_fp64_peak(int device, double* tflops_fma, double* tflops_mma);
 /* Number of kernel launches (own kernels only, memsets excluded) enqueued by this context so far. */
 int csf_launch_count(const csf_ctx* ctx, int64_t* launches);
 
-/* Select the cell-kernel variant (0 = library default); used by the benchmark sweep. CSF_EINVAL if unknown. */
+/* Select a kernel variant: 0 = library default; 1 = always take the general (predicated) column kernel, also on
+ * fully periodic meshes where the predicate-free specialisation would be chosen (test hook). CSF_EINVAL if unknown. */
 int csf_set_variant(csf_ctx* ctx, int variant);
 
 /* Text of the last error recorded on ctx (never NULL; "" if none). With ctx = NULL: last csf_create failure. */

@@ -10,8 +10,8 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libcsf.so")
-SOURCES = ["csf_api.cu", "csf_tables.cpp"]
-HEADERS = ["csf_kernels.cuh", "csf_tables.h", os.path.join("..", "..", "include", "csf.h")]
+SOURCES = ["csf_api.cu", "csf_tables.cpp", "csf_column_p.cu"]
+HEADERS = ["csf_kernels.cuh", "csf_column.cuh", "csf_column_launch.h", "csf_tables.h", os.path.join("..", "..", "include", "csf.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "--use_fast_math=false",
               "-Xcompiler", "-fPIC", "-shared", "-Xptxas", "-v"]
 
@@ -23,18 +23,35 @@ def _stale():
     return any(os.path.getmtime(os.path.join(CSRC, f)) > t for f in SOURCES + HEADERS)
 
 
+def _run(cmd):
+    res = subprocess.run(cmd, capture_output=True, text=True)
+    return res.returncode, res.stdout + res.stderr
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
+    """nvcc -c every translation unit in parallel (one per FE order for the column kernel), then link libcsf.so."""
     if not force and not _stale():
         return LIB
-    flags = [f for f in NVCC_FLAGS if f != "--use_fast_math=false"]
-    cmd = ["nvcc"] + flags + ["-o", LIB] + [os.path.join(CSRC, s) for s in SOURCES]
-    res = subprocess.run(cmd, capture_output=True, text=True)
-    if verbose or res.returncode != 0:
-        sys.stderr.write(res.stdout + res.stderr)
-    if res.returncode != 0:
+    from concurrent.futures import ThreadPoolExecutor
+    objdir = os.path.join(HERE, "build")
+    os.makedirs(objdir, exist_ok=True)
+    cflags = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
+    jobs = [(os.path.join(CSRC, "csf_api.cu"), os.path.join(objdir, "csf_api.o"), []),
+            (os.path.join(CSRC, "csf_tables.cpp"), os.path.join(objdir, "csf_tables.o"), [])]
+    jobs += [(os.path.join(CSRC, "csf_column_p.cu"), os.path.join(objdir, f"csf_column_p{p}.o"), [f"-DCSF_P={p}"]) for p in range(1, 8)]
+    with ThreadPoolExecutor(max_workers=min(8, os.cpu_count() or 2)) as ex:
+        results = list(ex.map(lambda j: _run(["nvcc"] + cflags + j[2] + ["-c", j[0], "-o", j[1]]), jobs))
+    log = "".join(out for _, out in results)
+    if verbose or any(rc != 0 for rc, _ in results):
+        sys.stderr.write(log)
+    if any(rc != 0 for rc, _ in results):
         raise RuntimeError("nvcc failed building libcsf.so")
+    rc, out = _run(["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", LIB] + [j[1] for j in jobs])
+    if rc != 0:
+        sys.stderr.write(out)
+        raise RuntimeError("nvcc failed linking libcsf.so")
     with open(os.path.join(HERE, "build_ptxas.log"), "w") as f:
-        f.write(res.stdout + res.stderr)
+        f.write(log + out)
     return LIB
 
 

@@ -1,6 +1,8 @@
 // csf_api.cu — C ABI of libcsf (see include/csf.h): context, host-side preprocessing, launch sequencing.
 #include "../../include/csf.h"
 #include "csf_kernels.cuh"
+#include "csf_column.cuh"
+#include "csf_column_launch.h"
 #include "csf_tables.h"
 
 #include <algorithm>
@@ -38,7 +40,9 @@ struct csf_ctx {
     int nfree[3]; long long M = 0; int E = 0;
     Gll1D gll; Dir1D dir[3];
     bool have_pot = false;
-    DevBuf d_cell_order, d_vb;
+    DevBuf d_cell_order, d_col_order, d_vb;
+    DevBuf d_pair_beg, d_pair_end, d_ent_locf;
+    int seg_len = 8, chunk_group = 4;
     // projectors
     int natoms = 0, npj_uniform = 0, npjp = 0; long long crows = 0;
     DevBuf d_pair_ptr, d_pair_atom, d_pair_off, d_ent_loc, d_ent_node, d_ent_p, d_atom_coff, d_atom_npj, d_atom_type,
@@ -81,63 +85,29 @@ struct ProfScope {
     ~ProfScope() { if (e1) { cudaEventRecord(e1, c->stream); c->prof_ev[kind].push_back({e0, e1}); } }
 };
 
-inline int lanes_of_variant(int v) { return v == 1 ? 32 : v == 2 ? 16 : v == 3 ? 8 : 0; }
-
-size_t cell_smem_bytes(int p, int L) { const size_t n = p + 1; return (2 * n * n * n + (size_t)p * p * p) * L * sizeof(double); }
-
-template <int P, int L, int NPJ>
-cudaError_t launch_cell_t(const CellParams& cp, int nblocks, size_t smem, cudaStream_t s) {
-    static bool configured = false;
-    auto kern = cell_kernel<P, L, NPJ>;
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        configured = true;
-    }
-    kern<<<nblocks, (P + 1) * L, smem, s>>>(cp);
-    return cudaGetLastError();
-}
-
-template <int P, int L>
-cudaError_t launch_cell_pl(int npj, const CellParams& cp, int nblocks, size_t smem, cudaStream_t s) {
-    if (npj == 18) return launch_cell_t<P, L, 18>(cp, nblocks, smem, s);
-    return launch_cell_t<P, L, 0>(cp, nblocks, smem, s);
-}
-
-template <int P>
-cudaError_t launch_cell_p(int L, int npj, const CellParams& cp, int nblocks, size_t smem, cudaStream_t s) {
-    switch (L) {
-        case 32: return launch_cell_pl<P, 32>(npj, cp, nblocks, smem, s);
-        case 16: return launch_cell_pl<P, 16>(npj, cp, nblocks, smem, s);
-        default: return launch_cell_pl<P, 8>(npj, cp, nblocks, smem, s);
-    }
-}
-
-cudaError_t launch_cell(int p, int L, int npj, const CellParams& cp, int nblocks, size_t smem, cudaStream_t s) {
+cudaError_t launch_column(int p, int ks, bool fast, const ColParams& cp, long long nblocks, cudaStream_t s) {
     switch (p) {
-        case 1: return launch_cell_p<1>(L, npj, cp, nblocks, smem, s);
-        case 2: return launch_cell_p<2>(L, npj, cp, nblocks, smem, s);
-        case 3: return launch_cell_p<3>(L, npj, cp, nblocks, smem, s);
-        case 4: return launch_cell_p<4>(L, npj, cp, nblocks, smem, s);
-        case 5: return launch_cell_p<5>(L, npj, cp, nblocks, smem, s);
-        case 6: return launch_cell_p<6>(L, npj, cp, nblocks, smem, s);
-        case 7: return launch_cell_p<7>(L, npj, cp, nblocks, smem, s);
+        case 1: return launch_column_p1(ks, fast, cp, nblocks, s);
+        case 2: return launch_column_p2(ks, fast, cp, nblocks, s);
+        case 3: return launch_column_p3(ks, fast, cp, nblocks, s);
+        case 4: return launch_column_p4(ks, fast, cp, nblocks, s);
+        case 5: return launch_column_p5(ks, fast, cp, nblocks, s);
+        case 6: return launch_column_p6(ks, fast, cp, nblocks, s);
+        case 7: return launch_column_p7(ks, fast, cp, nblocks, s);
     }
     return cudaErrorInvalidValue;
 }
 
-int pick_lanes(const csf_ctx* c) {
-    int L = lanes_of_variant(c->variant);
-    if (L == 0) L = 32;
-    while (L > 8 && cell_smem_bytes(c->p, L) > c->smem_optin) L /= 2;
-    return L;
+ColInfo column_info(int p) {
+    switch (p) {
+        case 1: return column_info_p1(); case 2: return column_info_p2(); case 3: return column_info_p3(); case 4: return column_info_p4();
+        case 5: return column_info_p5(); case 6: return column_info_p6(); default: return column_info_p7();
+    }
 }
 
 // one step: dst += sc * i^rot * (Hhat - shift) src
 int enqueue_step(csf_ctx* c, const double* src, long long ld, double* dst, long long ld_dst, int nvec, double sc, int rot, double shift,
                  double* dC, double* dCt) {
-    const int L = pick_lanes(c);
-    if (cell_smem_bytes(c->p, L) > c->smem_optin) return fail(c, CSF_EUNSUPPORTED, "cell tile does not fit shared memory");
     const long long ldc = nvec;
     if (c->natoms > 0) {
         CSF_CUDA(c, cudaMemsetAsync(dC, 0, (size_t)c->crows * ldc * sizeof(double2), c->stream));
@@ -163,35 +133,46 @@ int enqueue_step(csf_ctx* c, const double* src, long long ld, double* dst, long 
         CSF_CUDA(c, cudaGetLastError());
         c->launches += 2;
     }
-    CellParams cp{};
-    const int n = c->n;
-    for (int i = 0; i < n; ++i) {
-        for (int j = 0; j < n; ++j) { cp.Ay[i][j] = c->dir[1].A[i][j]; cp.Az[i][j] = c->dir[2].A[i][j]; cp.Ax[i][j] = sc * c->dir[0].A[i][j]; }
-        cp.by[i] = c->dir[1].beta[i]; cp.uy[i] = c->dir[1].u[i];
-        cp.bz[i] = c->dir[2].beta[i]; cp.uz[i] = c->dir[2].u[i];
-        cp.bxs[i] = sc * c->dir[0].beta[i]; cp.ux[i] = c->dir[0].u[i]; cp.uxs[i] = sc * c->dir[0].u[i];
-    }
-    cp.src = src; cp.dst = dst; cp.ld_src = ld; cp.ld_dst = ld_dst; cp.nvec = nvec;
-    cp.ncx = c->ncell[0]; cp.ncy = c->ncell[1]; cp.ncz = c->ncell[2];
-    cp.nfx = c->nfree[0]; cp.nfy = c->nfree[1]; cp.nfz = c->nfree[2];
-    cp.bcx = c->bc[0]; cp.bcy = c->bc[1]; cp.bcz = c->bc[2];
-    cp.cell_order = c->d_cell_order.as<int>(); cp.ncells = c->E;
-    cp.vb = c->d_vb.as<double>(); cp.shift = shift; cp.sc = sc; cp.rot = rot & 3;
-    if (c->natoms > 0) {
-        cp.pair_ptr = c->d_pair_ptr.as<int>(); cp.pair_atom = c->d_pair_atom.as<int>(); cp.pair_off = c->d_pair_off.as<int>();
-        cp.ent_loc = c->d_ent_loc.as<int>(); cp.ent_p = c->d_ent_p.as<double>();
-        cp.atom_coff = c->d_atom_coff.as<long long>(); cp.atom_npj = c->d_atom_npj.as<int>();
-        cp.Ct = dCt; cp.ldc = ldc; cp.npjp = c->npjp;
-    }
-    const int vchunk = L / 4;
-    const long long nblocks = (long long)c->E * ((nvec + vchunk - 1) / vchunk);
-    if (nblocks > 0x7fffffffLL) return fail(c, CSF_EUNSUPPORTED, "grid too large");
     {
-        ProfScope ps(c, CSF_KIND_CELL);
-        CSF_CUDA(c, launch_cell(c->p, L, c->natoms > 0 ? c->npj_uniform : 18, cp, (int)nblocks, cell_smem_bytes(c->p, L), c->stream));
+        const ColInfo ci = column_info(c->p);
+        if (ci.smem > c->smem_optin) return fail(c, CSF_EUNSUPPORTED, "column tile does not fit shared memory");
+        if (4 * ld >= (1LL << 31) || 4 * ld_dst >= (1LL << 31)) return fail(c, CSF_EUNSUPPORTED, "leading dimension too large");
+        const int vpc = ci.lanes / 4;               // spinor vectors per CTA
+        ColParams q{};
+        const int n = c->n;
+        const double hx2 = c->h[0] * c->h[0];
+        for (int i = 0; i < n; ++i) {
+            for (int j = 0; j < n; ++j) q.Ah[i][j] = c->dir[0].A[i][j] * (0.5 * hx2);
+            q.uh[i] = c->dir[0].u[i];
+        }
+        q.ax = 2.0 / hx2; q.rho_y = hx2 / (c->h[1] * c->h[1]); q.rho_z = hx2 / (c->h[2] * c->h[2]);
+        q.src = src; q.dst = dst; q.rs = (int)(4 * ld); q.rd = (int)(4 * ld_dst); q.nvec = nvec;
+        q.ncx = c->ncell[0]; q.ncy = c->ncell[1]; q.ncz = c->ncell[2];
+        q.nfx = c->nfree[0]; q.nfy = c->nfree[1]; q.nfz = c->nfree[2];
+        q.bcx = c->bc[0]; q.bcy = c->bc[1]; q.bcz = c->bc[2];
+        q.col_order = c->d_col_order.as<int>(); q.ncols = c->ncell[0] * c->ncell[1];
+        q.seg_len = std::min(c->seg_len, c->ncell[2]); q.nseg = (c->ncell[2] + q.seg_len - 1) / q.seg_len;
+        q.nchunks = (nvec + vpc - 1) / vpc; q.chunk_group = std::min(c->chunk_group, q.nchunks);
+        q.vb = c->d_vb.as<double>(); q.shift = shift; q.sc = sc; q.rot = rot & 3;
+        if (c->natoms > 0) {
+            q.pair_ptr = c->d_pair_ptr.as<int>(); q.pair_atom = c->d_pair_atom.as<int>();
+            q.pair_beg = c->d_pair_beg.as<int>(); q.pair_end = c->d_pair_end.as<int>();
+            q.ent_loc = c->d_ent_locf.as<int>(); q.ent_p = c->d_ent_p.as<double>();
+            q.atom_coff = c->d_atom_coff.as<long long>(); q.atom_npj = c->d_atom_npj.as<int>();
+            q.Ct = dCt; q.ldc = ldc; q.npjp = c->npjp;
+        }
+        const long long ngroups = (q.nchunks + q.chunk_group - 1) / q.chunk_group;
+        const long long nblocks = (long long)q.chunk_group * q.ncols * q.nseg * ngroups;
+        if (nblocks > 0x7fffffffLL) return fail(c, CSF_EUNSUPPORTED, "grid too large");
+        {
+            ProfScope ps(c, CSF_KIND_CELL);
+            const bool fast = c->bc[0] == CSF_BC_PERIODIC && c->bc[1] == CSF_BC_PERIODIC && c->bc[2] == CSF_BC_PERIODIC && nvec % vpc == 0 &&
+                              q.rho_y == 1.0 && q.rho_z == 1.0 && c->variant != 1;
+            CSF_CUDA(c, launch_column(c->p, c->natoms > 0 ? c->npjp / 4 : 5, fast, q, nblocks, c->stream));
+        }
+        c->launches += 1;
+        return CSF_OK;
     }
-    c->launches += 1;
-    return CSF_OK;
 }
 
 size_t block_bytes(const csf_ctx* c, int nvec) { return (size_t)2 * c->M * nvec * sizeof(double2); }
@@ -266,6 +247,13 @@ int csf_create(csf_ctx** out, const int ncell[3], const double box[3], int order
             for (int x = bx; x < std::min(bx + B, ncell[0]); ++x) order_v.push_back(x + ncell[0] * (y + ncell[1] * z));
     ce = c->d_cell_order.upload(order_v);
     if (ce != cudaSuccess) { delete c; return cuda_fail(nullptr, ce, "upload cell order"); }
+    // traversal order of the (cx, cy) columns: 8x8 tiles, x fastest inside (neighbouring columns run together, so the
+    // x / y faces they share are combined in L2)
+    std::vector<int> col_v; col_v.reserve((size_t)ncell[0] * ncell[1]);
+    for (int by = 0; by < ncell[1]; by += B) for (int bx = 0; bx < ncell[0]; bx += B)
+        for (int y = by; y < std::min(by + B, ncell[1]); ++y) for (int x = bx; x < std::min(bx + B, ncell[0]); ++x) col_v.push_back(x + ncell[0] * y);
+    ce = c->d_col_order.upload(col_v);
+    if (ce != cudaSuccess) { delete c; return cuda_fail(nullptr, ce, "upload column order"); }
     *out = c;
     return CSF_OK;
 }
@@ -352,12 +340,12 @@ int csf_set_projectors(csf_ctx* c, int natoms, const int64_t* node_ptr, const in
     const long long nent = node_ptr[natoms];
     if (nent >= (1LL << 31)) return fail(c, CSF_EUNSUPPORTED, "too many projector entries");
     for (long long t = 0; t < nent; ++t) if (node_idx[t] < 0 || node_idx[t] >= c->M) return fail(c, CSF_EINVAL, "node_idx out of range");
-    const int p = c->p, npjp = (npj_max + 1) / 2 * 2;
+    const int p = c->p, npjp = npj_max <= 20 ? 20 : 32;   // whole DMMA k-steps of 4 projectors
     std::vector<double> mass((size_t)c->M);
     csf_mass_diag(c, mass.data());
     // owner cell and local index of every support node; sort each atom's entries by (cell, lz, ly, lx)
     struct Ent { int cell, lz, ly, lx; long long t; };
-    std::vector<int> ent_node((size_t)nent), ent_loc((size_t)nent);
+    std::vector<int> ent_node((size_t)nent), ent_loc((size_t)nent), ent_locf((size_t)nent);
     std::vector<double> ent_p((size_t)nent * npjp, 0.0);
     std::vector<long long> atom_coff(natoms); std::vector<int> atom_npj(nproj, nproj + natoms), atom_ty(atom_type, atom_type + natoms);
     std::vector<int> gb_atom, gb_beg, gb_end;
@@ -382,7 +370,7 @@ int csf_set_projectors(csf_ctx* c, int natoms, const int64_t* node_ptr, const in
                 return fail(c, CSF_EINVAL, "duplicate node in an atom's support");
         for (size_t q = 0; q < ents.size(); ++q) {
             const long long e = t0 + (long long)q, t = ents[q].t, I = node_idx[t];
-            ent_node[e] = (int)I; ent_loc[e] = ents[q].ly * p + ents[q].lx;
+            ent_node[e] = (int)I; ent_loc[e] = ents[q].ly * p + ents[q].lx; ent_locf[e] = (ents[q].lz * p + ents[q].ly) * p + ents[q].lx;
             const double s = 1.0 / std::sqrt(mass[I]);
             for (int x = 0; x < nproj[a]; ++x) ent_p[(size_t)e * npjp + x] = s * pvals[pv_off + (t - t0) * nproj[a] + x];
             if (q == 0 || ents[q].cell != ents[q - 1].cell) {
@@ -401,11 +389,17 @@ int csf_set_projectors(csf_ctx* c, int natoms, const int64_t* node_ptr, const in
     for (const Pair& pr : pairs) pair_ptr[pr.cell + 1]++;
     for (int e = 0; e < c->E; ++e) pair_ptr[e + 1] += pair_ptr[e];
     std::vector<int> fill(pair_ptr.begin(), pair_ptr.end() - 1), pair_atom(pairs.size()), pair_off(pairs.size() * (p + 1));
-    for (const Pair& pr : pairs) { int s = fill[pr.cell]++; pair_atom[s] = pr.atom; for (int k = 0; k <= p; ++k) pair_off[(size_t)s * (p + 1) + k] = pr.off[k]; }
+    std::vector<int> pair_beg(pairs.size()), pair_end(pairs.size());
+    for (const Pair& pr : pairs) {
+        int s = fill[pr.cell]++; pair_atom[s] = pr.atom;
+        for (int k = 0; k <= p; ++k) pair_off[(size_t)s * (p + 1) + k] = pr.off[k];
+        pair_beg[s] = pr.off[0]; pair_end[s] = pr.off[p];
+    }
     std::vector<double2> dl((size_t)delta_ptr[ntypes]);
     for (size_t i = 0; i < dl.size(); ++i) dl[i] = make_double2(delta[i].re, delta[i].im);
     std::vector<long long> dptr(delta_ptr, delta_ptr + ntypes + 1);
     CSF_CUDA(c, c->d_pair_ptr.upload(pair_ptr)); CSF_CUDA(c, c->d_pair_atom.upload(pair_atom)); CSF_CUDA(c, c->d_pair_off.upload(pair_off));
+    CSF_CUDA(c, c->d_pair_beg.upload(pair_beg)); CSF_CUDA(c, c->d_pair_end.upload(pair_end)); CSF_CUDA(c, c->d_ent_locf.upload(ent_locf));
     CSF_CUDA(c, c->d_ent_loc.upload(ent_loc)); CSF_CUDA(c, c->d_ent_node.upload(ent_node)); CSF_CUDA(c, c->d_ent_p.upload(ent_p));
     CSF_CUDA(c, c->d_atom_coff.upload(atom_coff)); CSF_CUDA(c, c->d_atom_npj.upload(atom_npj)); CSF_CUDA(c, c->d_atom_type.upload(atom_ty));
     CSF_CUDA(c, c->d_delta.upload(dl)); CSF_CUDA(c, c->d_delta_ptr.upload(dptr));
@@ -593,7 +587,7 @@ int csf_launch_count(const csf_ctx* c, int64_t* launches) { if (!c || !launches)
 
 int csf_set_variant(csf_ctx* c, int variant) {
     if (!c) return CSF_EINVAL;
-    if (variant < 0 || variant > 3) return fail(c, CSF_EINVAL, "unknown variant");
+    if (variant < 0 || variant > 1) return fail(c, CSF_EINVAL, "unknown variant");
     c->variant = variant;
     return CSF_OK;
 }

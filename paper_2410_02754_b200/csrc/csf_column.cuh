@@ -1,0 +1,397 @@
+// csf_column.cuh — the column kernel: one recurrence step  dst += gamma (Hhat - c) src  of PAPER.md eq.70/eq.84
+// for one z-segment of a column of cells and L/4 spinor vectors per CTA.
+//
+// Paper steps fused here: a1 extraction X^(e) = R^(e) X with the M_D^{-1/2} scaling folded into the
+// 1-D operators, a2 cell-level product with the sum-factorised 1/2 K^(e), a3 nodal 2x2 spin potential, a7 projector
+// expansion P^a C~^a (FP64 tensor-core tiles, mma.sync m8n8k4 = DMMA), a4 assembly (RED.F64 scatter-add),
+// a8 recurrence update (accumulate form, csf_kernels.cuh).
+//
+// Why a column and not a cell: the L2 <-> SM fabric of B200 is barely faster than HBM, so the (n/p)^3 re-read /
+// re-add of the shared cell faces is real time. A CTA that marches through S cells of one (cx, cy) column keeps the
+// shared z-face on chip: its x-y contracted planes a2, b2 stay in a ring of N = p+1 shared-memory planes (they are
+// identical for the upper cell's bottom plane and the lower cell's top plane), and the partial sums of the top
+// plane are carried in registers into the next cell. Loads, x-y work and REDs all drop by p/(p+1).
+//
+// Operator tables. With the Loewdin scaling the 1-D operators of direction d are (csf_tables.h)
+//     A_d = (2/h_d^2) Ah,   B_d = diag(beta) - uh uh^T,   beta = 1/2 on the two shared end nodes, 1 inside,
+// where Ah and uh depend on the order p only. Ah is symmetric and centro-symmetric, uh is (anti)symmetric, so only
+// N^2/4 + N/2 + N/2 distinct numbers occur; the kernel reads each entry through its canonical index and the whole
+// table set stays resident in uniform registers (sm_100 has no constant-bank operand for DFMA). The kernel computes
+//     out / ax = Bz (By Ah u + rho_y Ah Bx u) + rho_z Ah (By Bx u),   ax = 2/h_x^2, rho_d = h_x^2 / h_d^2.
+//
+// Warp roles. Main threads = (q, lane): L lanes = (spin, vector, re/im) are independent real streams of the same
+// operator (the tables are real); q indexes a plane.
+//   phase A  thread holds the x-y plane u[j][i] of one new z-plane in registers:
+//              a2 = By Ah u + rho_y Ah Bx u,  b2 = rho_z By Bx u  -> ring;
+//              E = (V + B.sigma - c) u on the nodes the plane owns -> E ring (spin partner by shuffle)
+//   phase B  thread j takes the z-lines (j, i): out = ax (Bz a2 + Ah b2) (+ E + X on owned nodes, + carry on k = 0),
+//              RED.F64 into dst for k < p, out[p] becomes the carry.
+// Two auxiliary warps run beside phase A: X = sum_a P~^a C~^a per (cell, atom) pair as DMMA tiles (8 support rows
+// x 8 lanes x 4 projectors each; the tensor pipe works while the FP64 pipe does phase A), and they stage the nodal
+// potential of the next cell into shared memory.
+#pragma once
+#include <cuda_runtime.h>
+#include <cstdint>
+
+namespace csf {
+
+constexpr int kColTab = 8;
+constexpr int kColAux = 64;      // auxiliary threads (2 warps)
+
+struct ColParams {
+    double Ah[kColTab][kColTab];         // h-independent Loewdin-scaled 1-D stiffness (times 1/2), see above
+    double uh[kColTab];                  // rank-one part of the 1-D mass
+    double ax, rho_y, rho_z;             // 2/h_x^2, h_x^2/h_y^2, h_x^2/h_z^2
+    const double* src; double* dst;
+    int rs, rd;                          // doubles per node in src / dst (4 * ld)
+    int nvec;
+    int ncx, ncy, ncz, nfx, nfy, nfz, bcx, bcy, bcz;
+    const int* col_order; int ncols;     // traversal order of the (cx, cy) columns (8x8 tiles)
+    int seg_len, nseg;                   // cells per z-segment, segments per column
+    int chunk_group, nchunks;            // vector chunks of one column scheduled back to back; total chunks
+    const double* vb;                    // [M][4] = V, Bx, By, Bz at the nodes
+    double shift, sc; int rot;           // gamma = sc * i^rot, c = shift
+    // projector expansion: (cell, atom) pairs, entries sorted by local owned index
+    const int* pair_ptr;                 // [ncells+1]
+    const int* pair_atom;                // [npairs]
+    const int* pair_beg;                 // [npairs] entry range of the pair
+    const int* pair_end;
+    const int* ent_loc;                  // [nent] local owned index (lz*p + ly)*p + lx
+    const double* ent_p;                 // [nent][npjp] S_I P_{I chi}, zero padded
+    const long long* atom_coff;          // [natoms] first row of atom a in C / C~ (row = 2 chi + spin)
+    const int* atom_npj;                 // [natoms]
+    const double* Ct;                    // C~ [rows][ldc] complex128
+    long long ldc; int npjp;
+};
+
+__device__ __forceinline__ double col_flip(double x, unsigned mask) {
+    return __hiloint2double(__double2hiint(x) ^ (int)mask, __double2loint(x));
+}
+
+__device__ __forceinline__ int col_free_index(int f, int ncell, int p, int bc) {
+    const int nfull = ncell * p;
+    if (bc == 0) return f >= nfull ? f - nfull : f;
+    return (f == 0 || f == nfull) ? -1 : f - 1;
+}
+
+__device__ __forceinline__ void col_dmma(double& d0, double& d1, double a, double b) {
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
+}
+
+__device__ __forceinline__ void col_bar_aux() { asm volatile("bar.sync 1, %0;" ::"n"(kColAux) : "memory"); }
+
+// canonical representative of (i, j) under transposition and the centro flip (i, j) -> (N-1-i, N-1-j)
+template <int N> __host__ __device__ constexpr int col_canon(int i, int j) {
+    int best = i * kColTab + j, c = j * kColTab + i;
+    if (c < best) best = c;
+    c = (N - 1 - i) * kColTab + (N - 1 - j); if (c < best) best = c;
+    c = (N - 1 - j) * kColTab + (N - 1 - i); if (c < best) best = c;
+    return best;
+}
+
+template <int P, int L> struct ColCfg {
+    static constexpr int N = P + 1;
+    static constexpr int NTM = (N * L + 31) / 32 * 32;               // main threads
+    static constexpr int NT = NTM + kColAux;                         // threads per CTA
+    static constexpr int PLANE = N * N * L;                          // doubles per ring plane and field
+    static constexpr int EPLANE = P * P * L;
+    static constexpr int VPLANE = P * P * 4;                         // staged potential of one plane
+    // a2 ring, b2 ring, E ring, X, potential stage (2 buffers of N planes)
+    static constexpr size_t SMEM = (size_t)(2 * N * PLANE + N * EPLANE + P * EPLANE + 2 * N * VPLANE) * sizeof(double);
+};
+
+// FAST: every node of the mesh is unconstrained (all directions periodic), nvec is a multiple of L/4 and the cells
+// are cubes (rho_y = rho_z = 1), so no load, store or RED needs a predicate and no rho multiply is issued.
+template <int P, int KS, bool FAST, int L>
+__global__ void __launch_bounds__(ColCfg<P, L>::NT, (P >= 4 && P <= 5) ? 2 : 1) column_kernel(const __grid_constant__ ColParams A) {
+    using Cfg = ColCfg<P, L>;
+    constexpr int N = Cfg::N, NTM = Cfg::NTM, VPC = L / 4;        // VPC vectors per CTA
+    constexpr int PLANE = Cfg::PLANE, EPLANE = Cfg::EPLANE, VPLANE = Cfg::VPLANE;
+    extern __shared__ double smem[];
+    double* R1 = smem;
+    double* R2 = R1 + N * PLANE;
+    double* E = R2 + N * PLANE;
+    double* X = E + N * EPLANE;
+    double* VS = X + P * EPLANE;
+
+#define AH(i, j) ((&A.Ah[0][0])[col_canon<N>(i, j)])
+#define UH(i) (((P & 1) && (i) > N - 1 - (i)) ? -A.uh[N - 1 - (i)] : A.uh[(i) < N - 1 - (i) ? (i) : N - 1 - (i)])
+#define BETA(i) (((i) == 0 || (i) == P) ? 0.5 : 1.0)
+
+    // ---- which (column, segment, vector chunk)
+    int r = blockIdx.x;
+    const int cg = r % A.chunk_group; r /= A.chunk_group;
+    const int cidx = r % A.ncols; r /= A.ncols;
+    const int seg = r % A.nseg; r /= A.nseg;
+    const int chunk = r * A.chunk_group + cg;
+    if (chunk >= A.nchunks) return;
+    const int col = A.col_order[cidx];
+    const int cx = col % A.ncx, cy = col / A.ncx;
+    const int cz0 = seg * A.seg_len;
+    const int S = min(A.seg_len, A.ncz - cz0);
+    const int tid = threadIdx.x;
+    const int plane_nodes = A.nfx * A.nfy;
+
+    // stage the nodal potential of planes [g0, g0 + np) of the segment into VS buffer `buf` (thread `at` of `nthr`)
+    auto stage_vb = [&](int buf, int g0, int np, int at, int nthr) {
+        for (int task = at; task < np * P * P; task += nthr) {
+            const int pl = task / (P * P), rem = task - pl * (P * P);
+            const int j = rem / P, i = rem - j * P;
+            const int gx = col_free_index(cx * P + i, A.ncx, P, A.bcx), gy = col_free_index(cy * P + j, A.ncy, P, A.bcy);
+            const int gz = col_free_index(cz0 * P + g0 + pl, A.ncz, P, A.bcz);
+            double2 v01 = make_double2(0.0, 0.0), v23 = v01;
+            if (FAST || (gx >= 0 && gy >= 0 && gz >= 0)) {
+                const double2* vp = reinterpret_cast<const double2*>(A.vb) + 2 * ((long long)gz * plane_nodes + gy * A.nfx + gx);
+                v01 = __ldg(vp); v23 = __ldg(vp + 1);
+            }
+            double2* o = reinterpret_cast<double2*>(VS + (buf * N + pl) * VPLANE + rem * 4);
+            o[0] = v01; o[1] = v23;
+        }
+    };
+
+    stage_vb(0, 0, N, tid, Cfg::NT);
+    __syncthreads();
+
+    if (tid >= NTM) {
+        // ============================================================== auxiliary warps
+        const int at = tid - NTM, aw = at >> 5, wl = at & 31;
+        const int kk = wl & 3, rw = wl >> 2;
+        for (int t = 0; t < S; ++t) {
+            for (int idx = at; idx < P * EPLANE / 2; idx += kColAux) reinterpret_cast<double2*>(X)[idx] = make_double2(0.0, 0.0);
+            col_bar_aux();
+            if (A.pair_ptr != nullptr) {
+                const int cell = cx + A.ncx * (cy + A.ncy * (cz0 + t));
+                const int pr0 = A.pair_ptr[cell], pr1 = A.pair_ptr[cell + 1];
+                for (int pr = pr0; pr < pr1; ++pr) {
+                    const int atom = A.pair_atom[pr];
+                    const int e0 = A.pair_beg[pr], e1 = A.pair_end[pr];
+                    const int npj = A.atom_npj[atom];
+                    const long long coff = A.atom_coff[atom];
+                    // B fragments: C~[2 chi + spin][vec] of this atom; element (k, n) = (chi, data lane)
+                    double b[KS][L / 8];
+#pragma unroll
+                    for (int nt = 0; nt < L / 8; ++nt) {
+                        const int dl = nt * 8 + rw, bspin = dl / (L / 2), bvec = chunk * VPC + ((dl % (L / 2)) >> 1);
+                        const double* cb = A.Ct + ((coff + bspin) * A.ldc + bvec) * 2 + (dl & 1);
+#pragma unroll
+                        for (int s = 0; s < KS; ++s) {
+                            const int chi = 4 * s + kk;
+                            const bool ok = chi < npj && (FAST || bvec < A.nvec);
+                            b[s][nt] = ok ? __ldg(cb + (long long)chi * A.ldc * 4) : 0.0;
+                        }
+                    }
+                    const int ntiles = (e1 - e0 + 7) >> 3;
+                    double a[KS]; int loc = 0; bool valid = false;
+                    auto load_tile = [&](int tile, double (&aa)[KS], int& lc, bool& vd) {
+                        const int erow = e0 + tile * 8 + rw;
+                        vd = tile < ntiles && erow < e1;
+                        const double* ap = A.ent_p + (long long)(vd ? erow : e0) * A.npjp + kk;
+#pragma unroll
+                        for (int s = 0; s < KS; ++s) aa[s] = vd ? __ldg(ap + 4 * s) : 0.0;
+                        lc = vd ? __ldg(A.ent_loc + erow) : 0;
+                    };
+                    load_tile(aw, a, loc, valid);
+                    for (int tile = aw; tile < ntiles; tile += 2) {
+                        double an[KS]; int locn; bool validn;
+                        load_tile(tile + 2, an, locn, validn);
+                        double c[L / 8][2];
+#pragma unroll
+                        for (int nt = 0; nt < L / 8; ++nt) { c[nt][0] = 0.0; c[nt][1] = 0.0; }
+#pragma unroll
+                        for (int s = 0; s < KS; ++s)
+#pragma unroll
+                            for (int nt = 0; nt < L / 8; ++nt) col_dmma(c[nt][0], c[nt][1], a[s], b[s][nt]);
+                        if (valid) {
+                            double2* ep = reinterpret_cast<double2*>(X + loc * L + 2 * kk);
+#pragma unroll
+                            for (int nt = 0; nt < L / 8; ++nt) { double2 v = ep[4 * nt]; v.x += c[nt][0]; v.y += c[nt][1]; ep[4 * nt] = v; }
+                        }
+#pragma unroll
+                        for (int s = 0; s < KS; ++s) a[s] = an[s];
+                        loc = locn; valid = validn;
+                    }
+                    col_bar_aux();      // the next pair may touch the same nodes from the other warp
+                }
+            }
+            if (t + 1 < S) stage_vb((t + 1) & 1, (t + 1) * P + 1, P, at, kColAux);
+            __syncthreads();     // X(t) complete, phase A(t) complete
+            __syncthreads();     // phase B(t) complete
+        }
+        return;
+    }
+
+    // ================================================================== main warps
+    const int lane = tid % L, q = tid / L;
+    const int spin = lane / (L / 2), ri = lane & 1;
+    const int vec = chunk * VPC + ((lane % (L / 2)) >> 1);
+    const bool lane_on = FAST || vec < A.nvec;
+    const bool q_on = q < N;
+
+    int xo[N], yo[N];                 // node offsets of the column's x / y indices (or -1 on a Dirichlet face)
+#pragma unroll
+    for (int i = 0; i < N; ++i) {
+        xo[i] = col_free_index(cx * P + i, A.ncx, P, A.bcx);
+        const int gy = col_free_index(cy * P + i, A.ncy, P, A.bcy);
+        yo[i] = gy < 0 ? -1 : gy * A.nfx;
+    }
+    const double* sp = A.src + ((long long)spin * (A.rs >> 2) + vec) * 2 + ri;
+    const int slot_out = ri ^ (A.rot & 1);
+    const unsigned sgn = (A.rot == 2 || (A.rot == 1 && ri == 1) || (A.rot == 3 && ri == 0)) ? 0x80000000u : 0u;
+    double* dp = A.dst + ((long long)spin * (A.rd >> 2) + vec) * 2 + slot_out;
+    const double sz = spin ? -1.0 : 1.0;
+    const double sy = (spin == ri) ? 1.0 : -1.0;
+    const double scax = A.sc * A.ax;
+
+    double u[N][N];
+    double carry[N];
+#pragma unroll
+    for (int i = 0; i < N; ++i) carry[i] = 0.0;
+
+    // plane of the segment handled by this thread in iteration t (segment-local plane index g), or -1
+    auto plane_of = [&](int t) -> int {
+        if (!q_on) return -1;
+        if (t == 0) return q;
+        const int rr = (q + t) % N;
+        return rr < P ? t * P + rr + 1 : -1;
+    };
+    auto load_plane = [&](int g) {
+        const int gz = g < 0 ? -1 : col_free_index(cz0 * P + g, A.ncz, P, A.bcz);
+        const bool pz = g >= 0 && lane_on && gz >= 0;
+        const int zn = (gz < 0 ? 0 : gz) * plane_nodes;
+#pragma unroll
+        for (int j = 0; j < N; ++j) {
+            const int yz = zn + (FAST ? yo[j] : max(yo[j], 0));
+#pragma unroll
+            for (int i = 0; i < N; ++i) {
+                const bool ok = FAST ? (g >= 0) : (pz && xo[i] >= 0 && yo[j] >= 0);
+                const int node = yz + (FAST ? xo[i] : max(xo[i], 0));
+                u[j][i] = ok ? __ldg(sp + (long long)node * A.rs) : 0.0;
+            }
+        }
+    };
+
+    load_plane(plane_of(0));
+
+    for (int t = 0; t < S; ++t) {
+        // ------------------------------------------------------------------ phase A
+        {
+            const int g = plane_of(t);
+            const bool act = g >= 0;
+            const int slot = act ? g % N : 0;
+            double* r1 = R1 + slot * PLANE + lane;
+            double* r2 = R2 + slot * PLANE + lane;
+            // nodal terms on the nodes this plane owns (the last plane of the segment belongs to the next segment)
+            {
+                const int gz = act ? col_free_index(cz0 * P + g, A.ncz, P, A.bcz) : -1;
+                const bool own_plane = act && g < S * P && gz >= 0;
+                double* ep = E + slot * EPLANE + lane;
+                const int pidx = t == 0 ? (act ? g : 0) : (act ? g - t * P - 1 : 0);
+                const double2* vs = reinterpret_cast<const double2*>(VS + ((t & 1) * N + pidx) * VPLANE);
+#pragma unroll
+                for (int j = 0; j < P; ++j)
+#pragma unroll
+                    for (int i = 0; i < P; ++i) {
+                        const double own = u[j][i];
+                        const double t1 = __shfl_xor_sync(0xffffffffu, own, L / 2);   // other spin, same re/im
+                        const double t2 = __shfl_xor_sync(0xffffffffu, t1, 1);        // other spin, other re/im
+                        const double2 v01 = vs[(j * P + i) * 2], v23 = vs[(j * P + i) * 2 + 1];
+                        const double e = fma(v01.x - A.shift + sz * v23.y, own, fma(v01.y, t1, sy * v23.x * t2));
+                        if (own_plane) ep[(j * P + i) * L] = e;
+                    }
+            }
+            // x-step bookkeeping: d[j] = uh . u[j][:]
+            double d[N];
+#pragma unroll
+            for (int j = 0; j < N; ++j) {
+                double s = 0.0;
+#pragma unroll
+                for (int i = 0; i < N; ++i) s = fma(UH(i), u[j][i], s);
+                d[j] = s;
+            }
+            // output column i: a1 = (Ah u)[:, i], b1 = (Bx u)[:, i]; then the y-step on the column
+#pragma unroll
+            for (int i = 0; i < N; ++i) {
+                double a1[N], b1[N], b1s[N];
+#pragma unroll
+                for (int j = 0; j < N; ++j) {
+                    double s = 0.0;
+#pragma unroll
+                    for (int ii = 0; ii < N; ++ii) s = fma(AH(i, ii), u[j][ii], s);
+                    a1[j] = s;
+                    b1[j] = fma(-UH(i), d[j], BETA(i) * u[j][i]);
+                    b1s[j] = FAST ? b1[j] : A.rho_y * b1[j];
+                }
+                double da = 0.0, db = 0.0;
+#pragma unroll
+                for (int j = 0; j < N; ++j) { da = fma(UH(j), a1[j], da); db = fma(UH(j), b1[j], db); }
+#pragma unroll
+                for (int j = 0; j < N; ++j) {
+                    double a2 = fma(-UH(j), da, BETA(j) * a1[j]);
+#pragma unroll
+                    for (int jj = 0; jj < N; ++jj) a2 = fma(AH(j, jj), b1s[jj], a2);
+                    double b2 = fma(-UH(j), db, BETA(j) * b1[j]);
+                    if (!FAST) b2 *= A.rho_z;
+                    if (act) { r1[(j * N + i) * L] = a2; r2[(j * N + i) * L] = b2; }
+                }
+            }
+        }
+        if (t + 1 < S) load_plane(plane_of(t + 1));      // in flight during phase B
+        __syncthreads();
+        // ------------------------------------------------------------------ phase B
+        if (q_on) {
+            const int j = q;
+            const int cz = cz0 + t;
+            const int s0 = (t * P) % N;                   // ring slot of local plane 0 of this cell
+            int so[N], zn[N];
+#pragma unroll
+            for (int k = 0; k < N; ++k) {
+                int sl = s0 + k; sl = sl >= N ? sl - N : sl;
+                so[k] = sl;
+                const int gz = col_free_index(cz * P + k, A.ncz, P, A.bcz);
+                zn[k] = gz < 0 ? -1 : gz * plane_nodes;
+            }
+            const double* r1 = R1 + j * N * L + lane;
+            const double* r2 = R2 + j * N * L + lane;
+            const double* ep = E + j * P * L + lane;
+            const double* xp = X + j * P * L + lane;
+#pragma unroll
+            for (int i = 0; i < N; ++i) {
+                double f1[N], f2[N];
+#pragma unroll
+                for (int k = 0; k < N; ++k) {
+                    f1[k] = r1[so[k] * PLANE + i * L];
+                    f2[k] = r2[so[k] * PLANE + i * L];
+                }
+                double d1 = 0.0;
+#pragma unroll
+                for (int k = 0; k < N; ++k) d1 = fma(UH(k), f1[k], d1);
+                double o[N];
+#pragma unroll
+                for (int k = 0; k < N; ++k) {
+                    double s = fma(-UH(k), d1, BETA(k) * f1[k]);
+#pragma unroll
+                    for (int k2 = 0; k2 < N; ++k2) s = fma(AH(k, k2), f2[k2], s);
+                    o[k] = s;
+                }
+                o[0] += carry[i];
+                carry[i] = o[P];
+                const bool xy_ok = FAST || (lane_on && xo[i] >= 0 && yo[j] >= 0);
+                const int xy = FAST ? xo[i] + yo[j] : max(xo[i], 0) + max(yo[j], 0);
+#pragma unroll
+                for (int k = 0; k < P; ++k) {
+                    double v;
+                    if (j < P && i < P) v = fma(scax, o[k], A.sc * (ep[so[k] * EPLANE + i * L] + xp[k * EPLANE + i * L]));
+                    else v = scax * o[k];
+                    if (FAST || (xy_ok && zn[k] >= 0)) atomicAdd(dp + (long long)(xy + zn[k]) * A.rd, col_flip(v, sgn));
+                }
+                if (t == S - 1 && (FAST || (xy_ok && zn[P] >= 0))) atomicAdd(dp + (long long)(xy + zn[P]) * A.rd, col_flip(scax * carry[i], sgn));
+            }
+        }
+        __syncthreads();
+    }
+#undef AH
+#undef UH
+#undef BETA
+}
+
+}  // namespace csf

@@ -1,0 +1,40 @@
+// csf_column_p.cu — instantiates the column kernel for one FE order (compile with -DCSF_P=<1..7>); one translation
+// unit per order so that the orders build in parallel.
+#include "csf_column.cuh"
+#include "csf_column_launch.h"
+
+#ifndef CSF_P
+#error "compile with -DCSF_P=<order>"
+#endif
+
+namespace csf {
+
+namespace {
+constexpr int kLanes = CSF_P <= 6 ? 16 : 8;      // order 7 does not fit shared memory with 4 vectors per CTA
+
+template <int KS, bool FAST>
+cudaError_t launch_t(const ColParams& cp, long long nblocks, cudaStream_t s) {
+    static bool configured = false;
+    auto kern = column_kernel<CSF_P, KS, FAST, kLanes>;
+    using Cfg = ColCfg<CSF_P, kLanes>;
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM);
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    kern<<<(unsigned)nblocks, Cfg::NT, Cfg::SMEM, s>>>(cp);
+    return cudaGetLastError();
+}
+}  // namespace
+
+#define CSF_CAT2(a, b) a##b
+#define CSF_CAT(a, b) CSF_CAT2(a, b)
+
+cudaError_t CSF_CAT(launch_column_p, CSF_P)(int ks, bool fast, const ColParams& cp, long long nblocks, cudaStream_t s) {
+    if (ks <= 5) return fast ? launch_t<5, true>(cp, nblocks, s) : launch_t<5, false>(cp, nblocks, s);
+    return fast ? launch_t<8, true>(cp, nblocks, s) : launch_t<8, false>(cp, nblocks, s);
+}
+
+ColInfo CSF_CAT(column_info_p, CSF_P)() { return ColInfo{kLanes, ColCfg<CSF_P, kLanes>::SMEM}; }
+
+}  // namespace csf

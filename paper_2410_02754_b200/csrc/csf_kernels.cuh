@@ -7,8 +7,8 @@
 //
 //   proj_gather_kernel   C^a  = P~^aT src|supp(a)                     (eq.84 inner sum, a5)
 //   delta_apply_kernel   C~^a = Delta^{gamma_a} C^a                   (eq.76, a6)
-//   cell_kernel          gather -> sum-factorised 1/2 K -> nodal 2x2 potential, shift and projector
-//                        expansion on the nodes the cell owns -> scaled scatter-add   (a1-a4, a7, a8)
+//   column_kernel        gather -> sum-factorised 1/2 K -> nodal 2x2 potential, shift and projector
+//                        expansion on the nodes the cell owns -> scaled scatter-add   (a1-a4, a7, a8; csf_column.cuh)
 //
 // Data layout: multivector element (node I, spin s, vector v) = complex128 at [(2I+s)*ld + v]. The operator
 // tables are real, so the real and imaginary parts are independent batch entries: a "lane" is one double of
@@ -21,210 +21,6 @@
 namespace csf {
 
 constexpr int kTabN = 8;
-
-struct CellParams {
-    // Loewdin-scaled 1-D operators (csf_tables.h). Ax, bxs, uxs carry the step scale sc.
-    double Ay[kTabN][kTabN], Az[kTabN][kTabN], Ax[kTabN][kTabN];
-    double by[kTabN], uy[kTabN], bz[kTabN], uz[kTabN], bxs[kTabN], ux[kTabN], uxs[kTabN];
-    const double* src; double* dst;
-    long long ld_src, ld_dst; int nvec;
-    int ncx, ncy, ncz, nfx, nfy, nfz, bcx, bcy, bcz;
-    const int* cell_order; int ncells;
-    const double* vb;        // [M][4] = V, Bx, By, Bz at the nodes
-    double shift;            // c of (Hhat - c)
-    double sc; int rot;      // gamma = sc * i^rot
-    // projector expansion (cell-major view of the entry list)
-    const int* pair_ptr;     // [ncells+1]
-    const int* pair_atom;    // [npairs]
-    const int* pair_off;     // [npairs][P+1] entry ranges per owned z-plane
-    const int* ent_loc;      // [nent] local index j*P+i inside the owned plane
-    const double* ent_p;     // [nent][npjp] S_I P_{I chi}
-    const long long* atom_coff;  // [natoms] row offset of atom a in C / C~ (rows 2 chi + s)
-    const int* atom_npj;     // [natoms]
-    const double* Ct;        // C~ [rows][ldc] complex128
-    long long ldc; int npjp;
-};
-
-__device__ __forceinline__ double flip_sign(double x, unsigned mask) {
-    return __hiloint2double(__double2hiint(x) ^ (int)mask, __double2loint(x));
-}
-
-// free (unconstrained) 1-D node index of full index f, or -1 on a Dirichlet face
-__device__ __forceinline__ int free_index(int f, int ncell, int p, int bc) {
-    const int nfull = ncell * p;
-    if (bc == 0) return f >= nfull ? f - nfull : f;
-    return (f == 0 || f == nfull) ? -1 : f - 1;
-}
-
-// ---------------------------------------------------------------------------------------------------
-// cell kernel: one CTA = one cell x (L/4) vectors x 2 spins. Thread (plane, lane).
-//   phase 1: plane = z index; the thread holds the x-y plane X[j][i] of its lane in registers,
-//            F1 = By X (rank-one form), F2 = Ay X (dense) -> shared memory;
-//            on owned nodes E = (V + B.sigma - c) x + sum_a P~ C~^a  -> shared memory.
-//   phase 2: plane = y index; per x-column the z-operators, then the x-operators row by row:
-//            out = Ax (Bz F1) + Bx (Bz F2 + Az F1) + sc E, scatter-added with RED.F64.
-// ---------------------------------------------------------------------------------------------------
-template <int P, int L, int NPJ>
-__global__ void __launch_bounds__((P + 1) * L) cell_kernel(const __grid_constant__ CellParams A) {
-    constexpr int N = P + 1;
-    extern __shared__ double smem[];
-    double* F1 = smem;
-    double* F2 = smem + N * N * N * L;
-    double* E = smem + 2 * N * N * N * L;
-
-    const int tid = threadIdx.x;
-    const int lane = tid % L;
-    const int plane = tid / L;
-    const unsigned wmask = __activemask();
-
-    const int nchunk_v = L / 4;
-    const int cidx = blockIdx.x % A.ncells;
-    const int chunk = blockIdx.x / A.ncells;
-    const int cell = A.cell_order[cidx];
-    const int cx = cell % A.ncx, cy = (cell / A.ncx) % A.ncy, cz = cell / (A.ncx * A.ncy);
-
-    const int spin = lane / (L / 2);
-    const int ri = lane & 1;
-    const int vec = chunk * nchunk_v + ((lane % (L / 2)) >> 1);
-    const bool lane_on = vec < A.nvec;
-
-    int gx[N], gy[N], gz[N];
-#pragma unroll
-    for (int i = 0; i < N; ++i) {
-        gx[i] = free_index(cx * P + i, A.ncx, P, A.bcx);
-        gy[i] = free_index(cy * P + i, A.ncy, P, A.bcy);
-        gz[i] = free_index(cz * P + i, A.ncz, P, A.bcz);
-    }
-    const long long rs = 4 * A.ld_src;                               // doubles per node (2 rows)
-    const long long lane_off = ((long long)spin * A.ld_src + vec) * 2 + ri;
-
-    // ------------------------------------------------------------------ phase 1
-    {
-        const int k = plane;
-        double x[N][N];
-        const double* sp = A.src + lane_off;
-#pragma unroll
-        for (int j = 0; j < N; ++j)
-#pragma unroll
-            for (int i = 0; i < N; ++i) {
-                const bool ok = lane_on && gx[i] >= 0 && gy[j] >= 0 && gz[k] >= 0;
-                const int node = gx[i] + A.nfx * (gy[j] + A.nfy * gz[k]);
-                x[j][i] = ok ? __ldg(sp + (long long)node * rs) : 0.0;
-            }
-        // y-operators, column by column
-#pragma unroll
-        for (int i = 0; i < N; ++i) {
-            double d = 0.0;
-#pragma unroll
-            for (int j = 0; j < N; ++j) d = fma(A.uy[j], x[j][i], d);
-#pragma unroll
-            for (int j = 0; j < N; ++j) {
-                double f1 = fma(-A.uy[j], d, A.by[j] * x[j][i]);
-                double f2 = 0.0;
-#pragma unroll
-                for (int jj = 0; jj < N; ++jj) f2 = fma(A.Ay[j][jj], x[jj][i], f2);
-                F1[((k * N + j) * N + i) * L + lane] = f1;
-                F2[((k * N + j) * N + i) * L + lane] = f2;
-            }
-        }
-        // nodal terms on the nodes this cell owns (local index < P in every direction)
-        const double sz = spin ? -1.0 : 1.0;
-        const double sy = (spin == ri) ? 1.0 : -1.0;
-#pragma unroll
-        for (int j = 0; j < P; ++j)
-#pragma unroll
-            for (int i = 0; i < P; ++i) {
-                const double own = x[j][i];
-                const double t1 = __shfl_xor_sync(wmask, own, L / 2);   // other spin, same re/im
-                const double t2 = __shfl_xor_sync(wmask, t1, 1);        // other spin, other re/im
-                if (k < P) {
-                    double e = 0.0;
-                    if (gx[i] >= 0 && gy[j] >= 0 && gz[k] >= 0) {
-                        const int node = gx[i] + A.nfx * (gy[j] + A.nfy * gz[k]);
-                        const double2 v01 = __ldg(reinterpret_cast<const double2*>(A.vb) + 2 * (long long)node);
-                        const double2 v23 = __ldg(reinterpret_cast<const double2*>(A.vb) + 2 * (long long)node + 1);
-                        e = fma(v01.x - A.shift + sz * v23.y, own, fma(v01.y, t1, sy * v23.x * t2));
-                    }
-                    E[((k * P + j) * P + i) * L + lane] = e;
-                }
-            }
-        // projector expansion  E += sum_a P~^a C~^a  on owned nodes of this z-plane
-        if (k < P && A.pair_ptr != nullptr) {
-            const int pr0 = A.pair_ptr[cell], pr1 = A.pair_ptr[cell + 1];
-            for (int pr = pr0; pr < pr1; ++pr) {
-                const int e0 = A.pair_off[pr * (P + 1) + k], e1 = A.pair_off[pr * (P + 1) + k + 1];
-                if (e0 == e1) continue;
-                const int atom = A.pair_atom[pr];
-                const double* cb = A.Ct + ((A.atom_coff[atom] + spin) * A.ldc + vec) * 2 + ri;
-                if (NPJ > 0) {
-                    double ct[NPJ > 0 ? NPJ : 1];
-#pragma unroll
-                    for (int c = 0; c < NPJ; ++c) ct[c] = lane_on ? __ldg(cb + (long long)c * 4 * A.ldc) : 0.0;
-                    for (int e = e0; e < e1; ++e) {
-                        const double2* pp = reinterpret_cast<const double2*>(A.ent_p + (long long)e * A.npjp);
-                        double acc = 0.0;
-#pragma unroll
-                        for (int c = 0; c < NPJ / 2; ++c) { const double2 pv = __ldg(pp + c); acc = fma(pv.x, ct[2 * c], acc); acc = fma(pv.y, ct[2 * c + 1], acc); }
-                        E[(k * P * P + A.ent_loc[e]) * L + lane] += acc;
-                    }
-                } else {
-                    const int npj = A.atom_npj[atom];
-                    for (int e = e0; e < e1; ++e) {
-                        const double* pp = A.ent_p + (long long)e * A.npjp;
-                        double acc = 0.0;
-                        for (int c = 0; c < npj; ++c) acc = fma(__ldg(pp + c), lane_on ? __ldg(cb + (long long)c * 4 * A.ldc) : 0.0, acc);
-                        E[(k * P * P + A.ent_loc[e]) * L + lane] += acc;
-                    }
-                }
-            }
-        }
-    }
-    __syncthreads();
-    // ------------------------------------------------------------------ phase 2
-    {
-        const int j = plane;
-        double a[N][N], g[N][N];     // [k][i]
-#pragma unroll
-        for (int i = 0; i < N; ++i) {
-            double f1[N], f2[N];
-#pragma unroll
-            for (int k = 0; k < N; ++k) { f1[k] = F1[((k * N + j) * N + i) * L + lane]; f2[k] = F2[((k * N + j) * N + i) * L + lane]; }
-            double d1 = 0.0, d2 = 0.0;
-#pragma unroll
-            for (int k = 0; k < N; ++k) { d1 = fma(A.uz[k], f1[k], d1); d2 = fma(A.uz[k], f2[k], d2); }
-#pragma unroll
-            for (int k = 0; k < N; ++k) {
-                a[k][i] = fma(-A.uz[k], d1, A.bz[k] * f1[k]);
-                double t = fma(-A.uz[k], d2, A.bz[k] * f2[k]);
-#pragma unroll
-                for (int kk = 0; kk < N; ++kk) t = fma(A.Az[k][kk], f1[kk], t);
-                g[k][i] = t;
-            }
-        }
-        // multiplication by i^rot: swap re/im slot and flip signs (exact)
-        const int slot = ri ^ (A.rot & 1);
-        const unsigned sgn = (A.rot == 2 || (A.rot == 1 && ri == 1) || (A.rot == 3 && ri == 0)) ? 0x80000000u : 0u;
-        double* dp = A.dst + ((long long)spin * A.ld_dst + vec) * 2 + slot;
-        const long long rd = 4 * A.ld_dst;
-#pragma unroll
-        for (int k = 0; k < N; ++k) {
-            double dg = 0.0;
-#pragma unroll
-            for (int i = 0; i < N; ++i) dg = fma(A.ux[i], g[k][i], dg);
-#pragma unroll
-            for (int i = 0; i < N; ++i) {
-                double o = fma(-A.uxs[i], dg, A.bxs[i] * g[k][i]);
-#pragma unroll
-                for (int ii = 0; ii < N; ++ii) o = fma(A.Ax[i][ii], a[k][ii], o);
-                if (k < P && j < P && i < P) o = fma(A.sc, E[((k * P + j) * P + i) * L + lane], o);
-                if (lane_on && gx[i] >= 0 && gy[j] >= 0 && gz[k] >= 0) {
-                    const int node = gx[i] + A.nfx * (gy[j] + A.nfy * gz[k]);
-                    atomicAdd(dp + (long long)node * rd, flip_sign(o, sgn));
-                }
-            }
-        }
-    }
-}
 
 // ---------------------------------------------------------------------------------------------------
 // proj_gather_kernel: C[atom][2 chi + s][v] += sum_{I in block's node range} P~_{I chi} src[(2I+s)][v].

@@ -33,7 +33,7 @@ def test_apply_H_all_orders(order):
     assert rel_fro(gpu_apply_H(gpu, X), ref.apply_H(X)) < TOL
 
 
-@pytest.mark.parametrize("variant", [1, 2, 3])
+@pytest.mark.parametrize("variant", [0, 1])
 @pytest.mark.parametrize("nvec,ld", [(16, 16), (13, 13), (5, 9), (1, 1), (33, 40)])
 def test_apply_H_cfg0_variants_and_ragged(variant, nvec, ld):
     ref, gpu, s = setup_pair(synth.CONFIGS[0])
