@@ -41,7 +41,7 @@ struct csf_ctx {
     Gll1D gll; Dir1D dir[3];
     bool have_pot = false;
     DevBuf d_cell_order, d_col_order, d_vb;
-    DevBuf d_pair_beg, d_pair_end, d_ent_locf;
+    DevBuf d_sub_ptr, d_sub_desc, d_ent_locf;
     int seg_len = 8, chunk_group = 4;
     // projectors
     int natoms = 0, npj_uniform = 0, npjp = 0; long long crows = 0;
@@ -117,11 +117,11 @@ int enqueue_step(csf_ctx* c, const double* src, long long ld, double* dst, long 
         gp.ent_node = c->d_ent_node.as<int>(); gp.ent_p = c->d_ent_p.as<double>(); gp.npjp = c->npjp;
         gp.atom_coff = c->d_atom_coff.as<long long>(); gp.atom_npj = c->d_atom_npj.as<int>();
         gp.C = dC; gp.ldc = ldc;
-        dim3 gg(c->n_gather_blocks, (nvec + 7) / 8);
+        dim3 gg(c->n_gather_blocks, (nvec + 31) / 32);
         {
             ProfScope ps(c, CSF_KIND_PGATHER);
-            if (c->npj_uniform == 18) proj_gather_kernel<18><<<gg, 128, 0, c->stream>>>(gp);
-            else proj_gather_kernel<0><<<gg, 128, 0, c->stream>>>(gp);
+            if (c->npjp <= 24) proj_gather_kernel<3><<<gg, 256, 0, c->stream>>>(gp);
+            else proj_gather_kernel<4><<<gg, 256, 0, c->stream>>>(gp);
         }
         CSF_CUDA(c, cudaGetLastError());
         DeltaParams dp{};
@@ -155,10 +155,8 @@ int enqueue_step(csf_ctx* c, const double* src, long long ld, double* dst, long 
         q.nchunks = (nvec + vpc - 1) / vpc; q.chunk_group = std::min(c->chunk_group, q.nchunks);
         q.vb = c->d_vb.as<double>(); q.shift = shift; q.sc = sc; q.rot = rot & 3;
         if (c->natoms > 0) {
-            q.pair_ptr = c->d_pair_ptr.as<int>(); q.pair_atom = c->d_pair_atom.as<int>();
-            q.pair_beg = c->d_pair_beg.as<int>(); q.pair_end = c->d_pair_end.as<int>();
+            q.sub_ptr = c->d_sub_ptr.as<int>(); q.sub_desc = c->d_sub_desc.as<int4>();
             q.ent_loc = c->d_ent_locf.as<int>(); q.ent_p = c->d_ent_p.as<double>();
-            q.atom_coff = c->d_atom_coff.as<long long>(); q.atom_npj = c->d_atom_npj.as<int>();
             q.Ct = dCt; q.ldc = ldc; q.npjp = c->npjp;
         }
         const long long ngroups = (q.nchunks + q.chunk_group - 1) / q.chunk_group;
@@ -389,17 +387,32 @@ int csf_set_projectors(csf_ctx* c, int natoms, const int64_t* node_ptr, const in
     for (const Pair& pr : pairs) pair_ptr[pr.cell + 1]++;
     for (int e = 0; e < c->E; ++e) pair_ptr[e + 1] += pair_ptr[e];
     std::vector<int> fill(pair_ptr.begin(), pair_ptr.end() - 1), pair_atom(pairs.size()), pair_off(pairs.size() * (p + 1));
-    std::vector<int> pair_beg(pairs.size()), pair_end(pairs.size());
     for (const Pair& pr : pairs) {
         int s = fill[pr.cell]++; pair_atom[s] = pr.atom;
         for (int k = 0; k <= p; ++k) pair_off[(size_t)s * (p + 1) + k] = pr.off[k];
-        pair_beg[s] = pr.off[0]; pair_end[s] = pr.off[p];
     }
+    // sub-pairs for the column kernel: every (cell, atom) pair split at the owned-node index XSPLIT = ceil(p^3 / 2)
+    // (entries of a pair are sorted by that index), grouped by (cell, half)
+    const int xsplit = (p * p * p + 1) / 2;
+    struct Sub { int key; int4 d; };
+    std::vector<Sub> subs; subs.reserve(2 * pairs.size());
+    if (crows >= (1LL << 31)) return fail(c, CSF_EUNSUPPORTED, "too many projector rows");
+    for (const Pair& pr : pairs) {
+        const int e0 = pr.off[0], e1 = pr.off[p];
+        int em = e0; while (em < e1 && ent_locf[em] < xsplit) ++em;
+        const int coff = (int)atom_coff[pr.atom], npj = nproj[pr.atom];
+        if (em > e0) subs.push_back({pr.cell * 2, make_int4(coff, npj, e0, em)});
+        if (e1 > em) subs.push_back({pr.cell * 2 + 1, make_int4(coff, npj, em, e1)});
+    }
+    std::stable_sort(subs.begin(), subs.end(), [](const Sub& x, const Sub& y) { return x.key < y.key; });
+    std::vector<int> sub_ptr(2 * (size_t)c->E + 1, 0); std::vector<int4> sub_desc(subs.size());
+    for (size_t q = 0; q < subs.size(); ++q) { sub_ptr[subs[q].key + 1]++; sub_desc[q] = subs[q].d; }
+    for (size_t q = 0; q < 2 * (size_t)c->E; ++q) sub_ptr[q + 1] += sub_ptr[q];
     std::vector<double2> dl((size_t)delta_ptr[ntypes]);
     for (size_t i = 0; i < dl.size(); ++i) dl[i] = make_double2(delta[i].re, delta[i].im);
     std::vector<long long> dptr(delta_ptr, delta_ptr + ntypes + 1);
     CSF_CUDA(c, c->d_pair_ptr.upload(pair_ptr)); CSF_CUDA(c, c->d_pair_atom.upload(pair_atom)); CSF_CUDA(c, c->d_pair_off.upload(pair_off));
-    CSF_CUDA(c, c->d_pair_beg.upload(pair_beg)); CSF_CUDA(c, c->d_pair_end.upload(pair_end)); CSF_CUDA(c, c->d_ent_locf.upload(ent_locf));
+    CSF_CUDA(c, c->d_sub_ptr.upload(sub_ptr)); CSF_CUDA(c, c->d_sub_desc.upload(sub_desc)); CSF_CUDA(c, c->d_ent_locf.upload(ent_locf));
     CSF_CUDA(c, c->d_ent_loc.upload(ent_loc)); CSF_CUDA(c, c->d_ent_node.upload(ent_node)); CSF_CUDA(c, c->d_ent_p.upload(ent_p));
     CSF_CUDA(c, c->d_atom_coff.upload(atom_coff)); CSF_CUDA(c, c->d_atom_npj.upload(atom_npj)); CSF_CUDA(c, c->d_atom_type.upload(atom_ty));
     CSF_CUDA(c, c->d_delta.upload(dl)); CSF_CUDA(c, c->d_delta_ptr.upload(dptr));

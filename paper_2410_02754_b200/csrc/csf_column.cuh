@@ -52,14 +52,10 @@ struct ColParams {
     const double* vb;                    // [M][4] = V, Bx, By, Bz at the nodes
     double shift, sc; int rot;           // gamma = sc * i^rot, c = shift
     // projector expansion: (cell, atom) pairs, entries sorted by local owned index
-    const int* pair_ptr;                 // [ncells+1]
-    const int* pair_atom;                // [npairs]
-    const int* pair_beg;                 // [npairs] entry range of the pair
-    const int* pair_end;
+    const int* sub_ptr;                  // [2 ncells + 1] sub-pairs (cell, atom, half of the owned-node range)
+    const int4* sub_desc;                // [nsub] {first row of the atom in C~, n_pj, entry begin, entry end}
     const int* ent_loc;                  // [nent] local owned index (lz*p + ly)*p + lx
     const double* ent_p;                 // [nent][npjp] S_I P_{I chi}, zero padded
-    const long long* atom_coff;          // [natoms] first row of atom a in C / C~ (row = 2 chi + spin)
-    const int* atom_npj;                 // [natoms]
     const double* Ct;                    // C~ [rows][ldc] complex128
     long long ldc; int npjp;
 };
@@ -152,68 +148,86 @@ __global__ void __launch_bounds__(ColCfg<P, L>::NT, (P >= 4 && P <= 5) ? 2 : 1) 
     stage_vb(0, 0, N, tid, Cfg::NT);
     __syncthreads();
 
-    if (tid >= NTM) {
+    // warp-uniform role (broadcast from lane 0 so that the compiler knows the branch does not split a warp)
+    const int warp_id = __shfl_sync(0xffffffffu, tid >> 5, 0);
+    if (warp_id >= NTM / 32) {
         // ============================================================== auxiliary warps
-        const int at = tid - NTM, aw = at >> 5, wl = at & 31;
+        // Warp aw owns the owned-node range [aw * XSPLIT, (aw + 1) * XSPLIT) of X, so the two warps never touch the
+        // same row and need no barrier between them. Its sub-pairs (cell, atom, range) come from the host.
+        const int aw = warp_id - NTM / 32, wl = tid & 31;
         const int kk = wl & 3, rw = wl >> 2;
+        constexpr int XSPLIT = (P * P * P + 1) / 2, TMAX = (XSPLIT + 7) / 8, TCH = TMAX < 8 ? TMAX : 8;
+        const int xr0 = aw * XSPLIT, xr1 = min(P * P * P, xr0 + XSPLIT);
+        const double* cbase[L / 8]; bool bon[L / 8];
+#pragma unroll
+        for (int nt = 0; nt < L / 8; ++nt) {
+            const int dl = nt * 8 + rw, bspin = dl / (L / 2), bvec = chunk * VPC + ((dl % (L / 2)) >> 1);
+            cbase[nt] = A.Ct + ((long long)bspin * A.ldc + bvec) * 2 + (dl & 1);
+            bon[nt] = FAST || bvec < A.nvec;
+        }
+        auto load_b = [&](const int4& ds, double (&bb)[KS][L / 8]) {
+#pragma unroll
+            for (int nt = 0; nt < L / 8; ++nt)
+#pragma unroll
+                for (int s = 0; s < KS; ++s) {
+                    const int chi = 4 * s + kk;
+                    bb[s][nt] = (chi < ds.y && bon[nt]) ? __ldg(cbase[nt] + ((long long)ds.x + 2 * chi) * A.ldc * 2) : 0.0;
+                }
+        };
         for (int t = 0; t < S; ++t) {
-            for (int idx = at; idx < P * EPLANE / 2; idx += kColAux) reinterpret_cast<double2*>(X)[idx] = make_double2(0.0, 0.0);
-            col_bar_aux();
-            if (A.pair_ptr != nullptr) {
+            for (int idx = xr0 * (L / 2) + wl; idx < xr1 * (L / 2); idx += 32) reinterpret_cast<double2*>(X)[idx] = make_double2(0.0, 0.0);
+            __syncwarp();
+            if (A.sub_ptr != nullptr) {
                 const int cell = cx + A.ncx * (cy + A.ncy * (cz0 + t));
-                const int pr0 = A.pair_ptr[cell], pr1 = A.pair_ptr[cell + 1];
-                for (int pr = pr0; pr < pr1; ++pr) {
-                    const int atom = A.pair_atom[pr];
-                    const int e0 = A.pair_beg[pr], e1 = A.pair_end[pr];
-                    const int npj = A.atom_npj[atom];
-                    const long long coff = A.atom_coff[atom];
-                    // B fragments: C~[2 chi + spin][vec] of this atom; element (k, n) = (chi, data lane)
-                    double b[KS][L / 8];
+                const int sp0 = A.sub_ptr[cell * 2 + aw], sp1 = A.sub_ptr[cell * 2 + aw + 1];
+                int4 ds = make_int4(0, 0, 0, 0);       // {first row of the atom in C~, n_pj, entry begin, entry end}
+                double b[KS][L / 8];
+                if (sp0 < sp1) { ds = __ldg(A.sub_desc + sp0); load_b(ds, b); }
+                for (int sp = sp0; sp < sp1; ++sp) {
+                    // A fragments of up to TCH tiles at once (one exposed round trip), next sub-pair's B meanwhile
+                    const int e0 = ds.z, e1 = ds.w;
+                    int4 dn = ds; double bn[KS][L / 8];
+                    if (sp + 1 < sp1) { dn = __ldg(A.sub_desc + sp + 1); load_b(dn, bn); }
+                    for (int eb = e0; eb < e1; eb += 8 * TCH) {
+                        double a[TCH][KS]; int loc[TCH];
 #pragma unroll
-                    for (int nt = 0; nt < L / 8; ++nt) {
-                        const int dl = nt * 8 + rw, bspin = dl / (L / 2), bvec = chunk * VPC + ((dl % (L / 2)) >> 1);
-                        const double* cb = A.Ct + ((coff + bspin) * A.ldc + bvec) * 2 + (dl & 1);
+                        for (int tl = 0; tl < TCH; ++tl) {
+                            const int erow = eb + tl * 8 + rw;
+                            const bool vd = erow < e1;
+                            const double* ap = A.ent_p + (long long)(vd ? erow : e0) * A.npjp + kk;
 #pragma unroll
-                        for (int s = 0; s < KS; ++s) {
-                            const int chi = 4 * s + kk;
-                            const bool ok = chi < npj && (FAST || bvec < A.nvec);
-                            b[s][nt] = ok ? __ldg(cb + (long long)chi * A.ldc * 4) : 0.0;
+                            for (int s = 0; s < KS; ++s) a[tl][s] = vd ? __ldg(ap + 4 * s) : 0.0;
+                            loc[tl] = vd ? __ldg(A.ent_loc + erow) : -1;
+                        }
+#pragma unroll
+                        for (int tl = 0; tl < TCH; ++tl) {
+                            if (eb + tl * 8 < e1) {
+                                double c[L / 8][2];
+#pragma unroll
+                                for (int nt = 0; nt < L / 8; ++nt) { c[nt][0] = 0.0; c[nt][1] = 0.0; }
+#pragma unroll
+                                for (int s = 0; s < KS; ++s)
+#pragma unroll
+                                    for (int nt = 0; nt < L / 8; ++nt) col_dmma(c[nt][0], c[nt][1], a[tl][s], b[s][nt]);
+                                if (loc[tl] >= 0) {
+                                    double2* ep = reinterpret_cast<double2*>(X + loc[tl] * L + 2 * kk);
+#pragma unroll
+                                    for (int nt = 0; nt < L / 8; ++nt) { double2 v = ep[4 * nt]; v.x += c[nt][0]; v.y += c[nt][1]; ep[4 * nt] = v; }
+                                }
+                            }
                         }
                     }
-                    const int ntiles = (e1 - e0 + 7) >> 3;
-                    double a[KS]; int loc = 0; bool valid = false;
-                    auto load_tile = [&](int tile, double (&aa)[KS], int& lc, bool& vd) {
-                        const int erow = e0 + tile * 8 + rw;
-                        vd = tile < ntiles && erow < e1;
-                        const double* ap = A.ent_p + (long long)(vd ? erow : e0) * A.npjp + kk;
-#pragma unroll
-                        for (int s = 0; s < KS; ++s) aa[s] = vd ? __ldg(ap + 4 * s) : 0.0;
-                        lc = vd ? __ldg(A.ent_loc + erow) : 0;
-                    };
-                    load_tile(aw, a, loc, valid);
-                    for (int tile = aw; tile < ntiles; tile += 2) {
-                        double an[KS]; int locn; bool validn;
-                        load_tile(tile + 2, an, locn, validn);
-                        double c[L / 8][2];
-#pragma unroll
-                        for (int nt = 0; nt < L / 8; ++nt) { c[nt][0] = 0.0; c[nt][1] = 0.0; }
+                    __syncwarp();          // the next sub-pair of this warp may touch the same rows from other lanes
+                    if (sp + 1 < sp1) {
+                        ds = dn;
 #pragma unroll
                         for (int s = 0; s < KS; ++s)
 #pragma unroll
-                            for (int nt = 0; nt < L / 8; ++nt) col_dmma(c[nt][0], c[nt][1], a[s], b[s][nt]);
-                        if (valid) {
-                            double2* ep = reinterpret_cast<double2*>(X + loc * L + 2 * kk);
-#pragma unroll
-                            for (int nt = 0; nt < L / 8; ++nt) { double2 v = ep[4 * nt]; v.x += c[nt][0]; v.y += c[nt][1]; ep[4 * nt] = v; }
-                        }
-#pragma unroll
-                        for (int s = 0; s < KS; ++s) a[s] = an[s];
-                        loc = locn; valid = validn;
+                            for (int nt = 0; nt < L / 8; ++nt) b[s][nt] = bn[s][nt];
                     }
-                    col_bar_aux();      // the next pair may touch the same nodes from the other warp
                 }
             }
-            if (t + 1 < S) stage_vb((t + 1) & 1, (t + 1) * P + 1, P, at, kColAux);
+            if (t + 1 < S) stage_vb((t + 1) & 1, (t + 1) * P + 1, P, tid - NTM, kColAux);
             __syncthreads();     // X(t) complete, phase A(t) complete
             __syncthreads();     // phase B(t) complete
         }
@@ -255,7 +269,7 @@ __global__ void __launch_bounds__(ColCfg<P, L>::NT, (P >= 4 && P <= 5) ? 2 : 1) 
         return rr < P ? t * P + rr + 1 : -1;
     };
     auto load_plane = [&](int g) {
-        const int gz = g < 0 ? -1 : col_free_index(cz0 * P + g, A.ncz, P, A.bcz);
+        const int gz = g < 0 ? (FAST ? 0 : -1) : col_free_index(cz0 * P + g, A.ncz, P, A.bcz);
         const bool pz = g >= 0 && lane_on && gz >= 0;
         const int zn = (gz < 0 ? 0 : gz) * plane_nodes;
 #pragma unroll
@@ -263,9 +277,9 @@ __global__ void __launch_bounds__(ColCfg<P, L>::NT, (P >= 4 && P <= 5) ? 2 : 1) 
             const int yz = zn + (FAST ? yo[j] : max(yo[j], 0));
 #pragma unroll
             for (int i = 0; i < N; ++i) {
-                const bool ok = FAST ? (g >= 0) : (pz && xo[i] >= 0 && yo[j] >= 0);
                 const int node = yz + (FAST ? xo[i] : max(xo[i], 0));
-                u[j][i] = ok ? __ldg(sp + (long long)node * A.rs) : 0.0;
+                if (FAST) u[j][i] = __ldg(sp + (long long)node * A.rs);       // idle threads read plane 0 and drop it
+                else u[j][i] = (pz && xo[i] >= 0 && yo[j] >= 0) ? __ldg(sp + (long long)node * A.rs) : 0.0;
             }
         }
     };

@@ -23,9 +23,11 @@ namespace csf {
 constexpr int kTabN = 8;
 
 // ---------------------------------------------------------------------------------------------------
-// proj_gather_kernel: C[atom][2 chi + s][v] += sum_{I in block's node range} P~_{I chi} src[(2I+s)][v].
-// grid.x = gather blocks (atom, node range), grid.y = vector chunks of 8; 4 warps split the nodes,
-// shared-memory reduce, one RED per (chi, lane).
+// proj_gather_kernel (a5): C[atom][2 chi + s][v] += sum_{I in the block's entry range} P~_{I chi} src[(2I+s)][v]
+// as FP64 tensor-core tiles (mma.sync m8n8k4): A = P~^T (8 projectors x 4 support rows), B = src (4 rows x 8 real
+// lanes = 4 vectors), D (8 projectors x 4 complex vectors) accumulated over the entry range and RED-added into C.
+// grid.x = gather blocks (atom, <= 256 entries), grid.y = chunks of 32 vectors; the 8 warps of a CTA are
+// (spin, 8 vectors) and read the same P~ rows (L1), every src element is read exactly once per H apply.
 // ---------------------------------------------------------------------------------------------------
 struct GatherParams {
     const double* src; long long ld; int nvec;
@@ -35,46 +37,63 @@ struct GatherParams {
     double* C; long long ldc;
 };
 
-template <int NPJ>
-__global__ void __launch_bounds__(128) proj_gather_kernel(const __grid_constant__ GatherParams A) {
-    constexpr int NA = NPJ > 0 ? NPJ : 32;
-    __shared__ double red[3][NA][32];
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int spin = lane >> 4, ri = lane & 1;
-    const int vec = blockIdx.y * 8 + ((lane & 15) >> 1);
-    const bool lane_on = vec < A.nvec;
+__device__ __forceinline__ void gather_dmma(double& d0, double& d1, double a, double b) {
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
+}
+
+template <int MT>      // projector tiles of 8 (npjp <= 8 MT)
+__global__ void __launch_bounds__(256) proj_gather_kernel(const __grid_constant__ GatherParams A) {
+    const int wl = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int kk = wl & 3, rw = wl >> 2;
+    const int spin = warp & 1;
+    const int v0 = blockIdx.y * 32 + (warp >> 1) * 8;
+    if (v0 >= A.nvec) return;
     const int atom = A.gb_atom[blockIdx.x];
     const int e0 = A.gb_beg[blockIdx.x], e1 = A.gb_end[blockIdx.x];
-    const int npj = NPJ > 0 ? NPJ : A.atom_npj[atom];
-    const double* sp = A.src + ((long long)spin * A.ld + vec) * 2 + ri;
-    const long long rs = 4 * A.ld;
-    double acc[NA];
+    const int npj = A.atom_npj[atom];
+    double acc[MT][2][2];
 #pragma unroll
-    for (int c = 0; c < NA; ++c) acc[c] = 0.0;
-    for (int e = e0 + warp; e < e1; e += 4) {
-        const double xv = lane_on ? __ldg(sp + (long long)A.ent_node[e] * rs) : 0.0;
-        if (NPJ > 0) {
-            const double2* pp = reinterpret_cast<const double2*>(A.ent_p + (long long)e * A.npjp);
+    for (int m = 0; m < MT; ++m)
 #pragma unroll
-            for (int c = 0; c < NPJ / 2; ++c) { const double2 pv = __ldg(pp + c); acc[2 * c] = fma(pv.x, xv, acc[2 * c]); acc[2 * c + 1] = fma(pv.y, xv, acc[2 * c + 1]); }
-        } else {
-            const double* pp = A.ent_p + (long long)e * A.npjp;
+        for (int nt = 0; nt < 2; ++nt) { acc[m][nt][0] = 0.0; acc[m][nt][1] = 0.0; }
+    const int bv[2] = { v0 + (rw >> 1), v0 + 4 + (rw >> 1) };
+    const double* sb = A.src + ((long long)spin * A.ld) * 2 + (rw & 1);
+    auto load_step = [&](int e, double (&a)[MT], double (&b)[2]) {
+        const int er = e + kk;
+        const bool ok = er < e1;
+        const int node = __ldg(A.ent_node + (ok ? er : e0));
+        const double* ap = A.ent_p + (long long)(ok ? er : e0) * A.npjp + rw;
 #pragma unroll
-            for (int c = 0; c < NA; ++c) if (c < npj) acc[c] = fma(__ldg(pp + c), xv, acc[c]);
-        }
+        for (int m = 0; m < MT; ++m) a[m] = (ok && m * 8 + rw < A.npjp) ? __ldg(ap + m * 8) : 0.0;
+        const double* xp = sb + (long long)node * A.ld * 4;
+#pragma unroll
+        for (int nt = 0; nt < 2; ++nt) b[nt] = (ok && bv[nt] < A.nvec) ? __ldg(xp + (long long)bv[nt] * 2) : 0.0;
+    };
+    for (int e = e0; e < e1; e += 8) {
+        double a0[MT], b0[2], a1[MT], b1[2];
+        load_step(e, a0, b0);
+        load_step(e + 4, a1, b1);
+#pragma unroll
+        for (int m = 0; m < MT; ++m)
+#pragma unroll
+            for (int nt = 0; nt < 2; ++nt) gather_dmma(acc[m][nt][0], acc[m][nt][1], a0[m], b0[nt]);
+#pragma unroll
+        for (int m = 0; m < MT; ++m)
+#pragma unroll
+            for (int nt = 0; nt < 2; ++nt) gather_dmma(acc[m][nt][0], acc[m][nt][1], a1[m], b1[nt]);
     }
-    if (warp > 0) {
+    const long long coff = A.atom_coff[atom];
 #pragma unroll
-        for (int c = 0; c < NA; ++c) red[warp - 1][c][lane] = acc[c];
-    }
-    __syncthreads();
-    if (warp == 0 && lane_on) {
-        double* cp = A.C + ((A.atom_coff[atom] + spin) * A.ldc + vec) * 2 + ri;
+    for (int m = 0; m < MT; ++m) {
+        const int chi = m * 8 + rw;
+        if (chi < npj) {
 #pragma unroll
-        for (int c = 0; c < NA; ++c) {
-            if (c < npj) {
-                const double s = acc[c] + red[0][c][lane] + red[1][c][lane] + red[2][c][lane];
-                atomicAdd(cp + (long long)c * 4 * A.ldc, s);
+            for (int nt = 0; nt < 2; ++nt) {
+                const int v = v0 + nt * 4 + kk;
+                if (v < A.nvec) {
+                    double* cp = A.C + ((coff + 2 * chi + spin) * A.ldc + v) * 2;
+                    atomicAdd(cp, acc[m][nt][0]); atomicAdd(cp + 1, acc[m][nt][1]);
+                }
             }
         }
     }
