@@ -74,7 +74,10 @@ __device__ __forceinline__ void col_dmma(double& d0, double& d1, double a, doubl
     asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
 }
 
-__device__ __forceinline__ void col_bar_aux() { asm volatile("bar.sync 1, %0;" ::"n"(kColAux) : "memory"); }
+// named barriers: 1 = main threads only; 2 + b = "X buffer b is full" (expansion warps arrive, main threads wait);
+// 4 + b = "X buffer b is free" (main threads arrive, expansion warps wait)
+__device__ __forceinline__ void col_bar_sync(int id, int count) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(count) : "memory"); }
+__device__ __forceinline__ void col_bar_arrive(int id, int count) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(count) : "memory"); }
 
 // canonical representative of (i, j) under transposition and the centro flip (i, j) -> (N-1-i, N-1-j)
 template <int N> __host__ __device__ constexpr int col_canon(int i, int j) {
@@ -92,8 +95,8 @@ template <int P, int L> struct ColCfg {
     static constexpr int PLANE = N * N * L;                          // doubles per ring plane and field
     static constexpr int EPLANE = P * P * L;
     static constexpr int VPLANE = P * P * 4;                         // staged potential of one plane
-    // a2 ring, b2 ring, E ring, X, potential stage (2 buffers of N planes)
-    static constexpr size_t SMEM = (size_t)(2 * N * PLANE + N * EPLANE + P * EPLANE + 2 * N * VPLANE) * sizeof(double);
+    // a2 ring, b2 ring, E ring, X (2 buffers), potential stage (N planes)
+    static constexpr size_t SMEM = (size_t)(2 * N * PLANE + N * EPLANE + 2 * P * EPLANE + N * VPLANE) * sizeof(double);
 };
 
 // FAST: every node of the mesh is unconstrained (all directions periodic), nvec is a multiple of L/4 and the cells
@@ -107,8 +110,8 @@ __global__ void __launch_bounds__(ColCfg<P, L>::NT, (P >= 4 && P <= 5) ? 2 : 1) 
     double* R1 = smem;
     double* R2 = R1 + N * PLANE;
     double* E = R2 + N * PLANE;
-    double* X = E + N * EPLANE;
-    double* VS = X + P * EPLANE;
+    double* Xb = E + N * EPLANE;
+    double* VS = Xb + 2 * P * EPLANE;
 
 #define AH(i, j) ((&A.Ah[0][0])[col_canon<N>(i, j)])
 #define UH(i) (((P & 1) && (i) > N - 1 - (i)) ? -A.uh[N - 1 - (i)] : A.uh[(i) < N - 1 - (i) ? (i) : N - 1 - (i)])
@@ -128,24 +131,23 @@ __global__ void __launch_bounds__(ColCfg<P, L>::NT, (P >= 4 && P <= 5) ? 2 : 1) 
     const int tid = threadIdx.x;
     const int plane_nodes = A.nfx * A.nfy;
 
-    // stage the nodal potential of planes [g0, g0 + np) of the segment into VS buffer `buf` (thread `at` of `nthr`)
-    auto stage_vb = [&](int buf, int g0, int np, int at, int nthr) {
-        for (int task = at; task < np * P * P; task += nthr) {
-            const int pl = task / (P * P), rem = task - pl * (P * P);
-            const int j = rem / P, i = rem - j * P;
-            const int gx = col_free_index(cx * P + i, A.ncx, P, A.bcx), gy = col_free_index(cy * P + j, A.ncy, P, A.bcy);
-            const int gz = col_free_index(cz0 * P + g0 + pl, A.ncz, P, A.bcz);
-            double2 v01 = make_double2(0.0, 0.0), v23 = v01;
-            if (FAST || (gx >= 0 && gy >= 0 && gz >= 0)) {
-                const double2* vp = reinterpret_cast<const double2*>(A.vb) + 2 * ((long long)gz * plane_nodes + gy * A.nfx + gx);
-                v01 = __ldg(vp); v23 = __ldg(vp + 1);
-            }
-            double2* o = reinterpret_cast<double2*>(VS + (buf * N + pl) * VPLANE + rem * 4);
-            o[0] = v01; o[1] = v23;
+    // nodal potential (V, Bx, By, Bz) of owned node `task` of the segment planes starting at g0 -> two double2
+    auto load_vb = [&](int g0, int task, double2& v01, double2& v23) {
+        const int pl = task / (P * P), rem = task - pl * (P * P);
+        const int j = rem / P, i = rem - j * P;
+        const int gx = col_free_index(cx * P + i, A.ncx, P, A.bcx), gy = col_free_index(cy * P + j, A.ncy, P, A.bcy);
+        const int gz = col_free_index(cz0 * P + g0 + pl, A.ncz, P, A.bcz);
+        v01 = make_double2(0.0, 0.0); v23 = v01;
+        if (FAST || (gx >= 0 && gy >= 0 && gz >= 0)) {
+            const double2* vp = reinterpret_cast<const double2*>(A.vb) + 2 * ((long long)gz * plane_nodes + gy * A.nfx + gx);
+            v01 = __ldg(vp); v23 = __ldg(vp + 1);
         }
     };
-
-    stage_vb(0, 0, N, tid, Cfg::NT);
+    for (int task = tid; task < N * P * P; task += Cfg::NT) {
+        double2 v01, v23; load_vb(0, task, v01, v23);
+        double2* o = reinterpret_cast<double2*>(VS + task * 4);
+        o[0] = v01; o[1] = v23;
+    }
     __syncthreads();
 
     // warp-uniform role (broadcast from lane 0 so that the compiler knows the branch does not split a warp)
@@ -175,6 +177,8 @@ __global__ void __launch_bounds__(ColCfg<P, L>::NT, (P >= 4 && P <= 5) ? 2 : 1) 
                 }
         };
         for (int t = 0; t < S; ++t) {
+            double* X = Xb + (t & 1) * P * EPLANE;
+            if (t >= 2) col_bar_sync(4 + (t & 1), Cfg::NT);      // phase B(t - 2) has consumed this buffer
             for (int idx = xr0 * (L / 2) + wl; idx < xr1 * (L / 2); idx += 32) reinterpret_cast<double2*>(X)[idx] = make_double2(0.0, 0.0);
             __syncwarp();
             if (A.sub_ptr != nullptr) {
@@ -227,9 +231,8 @@ __global__ void __launch_bounds__(ColCfg<P, L>::NT, (P >= 4 && P <= 5) ? 2 : 1) 
                     }
                 }
             }
-            if (t + 1 < S) stage_vb((t + 1) & 1, (t + 1) * P + 1, P, tid - NTM, kColAux);
-            __syncthreads();     // X(t) complete, phase A(t) complete
-            __syncthreads();     // phase B(t) complete
+            __threadfence_block();
+            col_bar_arrive(2 + (t & 1), Cfg::NT);                // X(t) is complete
         }
         return;
     }
@@ -300,7 +303,7 @@ __global__ void __launch_bounds__(ColCfg<P, L>::NT, (P >= 4 && P <= 5) ? 2 : 1) 
                 const bool own_plane = act && g < S * P && gz >= 0;
                 double* ep = E + slot * EPLANE + lane;
                 const int pidx = t == 0 ? (act ? g : 0) : (act ? g - t * P - 1 : 0);
-                const double2* vs = reinterpret_cast<const double2*>(VS + ((t & 1) * N + pidx) * VPLANE);
+                const double2* vs = reinterpret_cast<const double2*>(VS + pidx * VPLANE);
 #pragma unroll
                 for (int j = 0; j < P; ++j)
 #pragma unroll
@@ -349,8 +352,17 @@ __global__ void __launch_bounds__(ColCfg<P, L>::NT, (P >= 4 && P <= 5) ? 2 : 1) 
                 }
             }
         }
-        if (t + 1 < S) load_plane(plane_of(t + 1));      // in flight during phase B
-        __syncthreads();
+        // in flight during phase B: the next planes and their nodal potential
+        constexpr int VT = (P * P * P + NTM - 1) / NTM;
+        double2 nv01[VT], nv23[VT];
+        if (t + 1 < S) {
+            load_plane(plane_of(t + 1));
+#pragma unroll
+            for (int v = 0; v < VT; ++v) if (tid + v * NTM < P * P * P) load_vb((t + 1) * P + 1, tid + v * NTM, nv01[v], nv23[v]);
+        }
+        col_bar_sync(1, NTM);                                 // ring, E written; VS no longer read
+        col_bar_sync(2 + (t & 1), Cfg::NT);                   // X(t) complete
+        const double* X = Xb + (t & 1) * P * EPLANE;
         // ------------------------------------------------------------------ phase B
         if (q_on) {
             const int j = q;
@@ -401,7 +413,16 @@ __global__ void __launch_bounds__(ColCfg<P, L>::NT, (P >= 4 && P <= 5) ? 2 : 1) 
                 if (t == S - 1 && (FAST || (xy_ok && zn[P] >= 0))) atomicAdd(dp + (long long)(xy + zn[P]) * A.rd, col_flip(scax * carry[i], sgn));
             }
         }
-        __syncthreads();
+        if (t + 1 < S) {
+#pragma unroll
+            for (int v = 0; v < VT; ++v)
+                if (tid + v * NTM < P * P * P) {
+                    double2* o = reinterpret_cast<double2*>(VS + (tid + v * NTM) * 4);
+                    o[0] = nv01[v]; o[1] = nv23[v];
+                }
+        }
+        if (t + 2 < S) col_bar_arrive(4 + (t & 1), Cfg::NT);  // X buffer t & 1 is free
+        col_bar_sync(1, NTM);                                 // ring free, VS visible
     }
 #undef AH
 #undef UH
