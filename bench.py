@@ -273,8 +273,15 @@ def main_ours(args):
     if cell_n > 0:
         t_cell = cell_ms / cell_n * 1e-3
         ach = f_cell * rows * nvec / t_cell / 1e12
-        roof = {"kernel": "cell_kernel (a1-a4, a7, a8)", "bound": "alu", "achieved": ach, "peak": peak_alu, "unit": "TFLOP/s", "frac": ach / peak_alu,
-                "peak_source": "148 SMs x 64 FP64 FMA/clk x 2 x %.0f MHz (DESIGN.md)" % sm_max, "traffic": None,
+        traffic = None
+        try:
+            with open(os.path.join(ROOT, "profiles", "r1_traffic.json")) as f:
+                traffic = float(json.load(f)["dram_bytes_per_unit"]) * rows * nvec    # ncu --set full capture, scaled to this launch
+        except (OSError, KeyError, ValueError):
+            pass
+        roof = {"kernel": "column_kernel (a1-a4, a7, a8)", "bound": "alu", "achieved": ach, "peak": peak_alu, "unit": "TFLOP/s", "frac": ach / peak_alu,
+                "peak_source": "148 SMs x 64 FP64 FMA/clk x 2 x %.0f MHz (DESIGN.md)" % sm_max, "traffic": traffic,
+                "algorithmic_bytes": 48.0 * rows * nvec,
                 "flops_per_unit": f_cell, "avg_launch_ms": t_cell * 1e3, "launches": cell_n,
                 "share_of_step": cell_ms / ms_local,
                 "hbm_achieved_gbs": 48.0 * rows * nvec / t_cell / 1e9, "hbm_peak_gbs": hbm, "hbm_frac": 48.0 * rows * nvec / t_cell / 1e9 / hbm,
