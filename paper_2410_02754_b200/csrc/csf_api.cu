@@ -5,6 +5,8 @@
 #include "csf_column_launch.h"
 #include "csf_tables.h"
 
+#include <cuda.h>
+
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
@@ -105,6 +107,29 @@ ColInfo column_info(int p) {
     }
 }
 
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
+                                  const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+// cuTensorMapEncodeTiled through the runtime's driver entry point (no link-time dependency on libcuda)
+EncodeTiledFn encode_tiled_fn() {
+    static EncodeTiledFn fn = nullptr;
+    if (!fn) {
+        void* p = nullptr; cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess && q == cudaDriverEntryPointSuccess)
+            fn = reinterpret_cast<EncodeTiledFn>(p);
+    }
+    return fn;
+}
+
+// FP64 tensor map of rank `rank`: dims / box in elements (innermost first), strides in bytes for dims 1..rank-1
+bool encode_map(CUtensorMap* tm, const void* base, int rank, const cuuint64_t* dims, const cuuint64_t* strides, const cuuint32_t* box) {
+    EncodeTiledFn fn = encode_tiled_fn();
+    if (!fn) return false;
+    cuuint32_t es[5] = {1, 1, 1, 1, 1};
+    return fn(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, (cuuint32_t)rank, const_cast<void*>(base), dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+              CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
 // one step: dst += sc * i^rot * (Hhat - shift) src
 int enqueue_step(csf_ctx* c, const double* src, long long ld, double* dst, long long ld_dst, int nvec, double sc, int rot, double shift,
                  double* dC, double* dCt) {
@@ -147,6 +172,18 @@ int enqueue_step(csf_ctx* c, const double* src, long long ld, double* dst, long 
         }
         q.ax = 2.0 / hx2; q.rho_y = hx2 / (c->h[1] * c->h[1]); q.rho_z = hx2 / (c->h[2] * c->h[2]);
         q.src = src; q.dst = dst; q.rs = (int)(4 * ld); q.rd = (int)(4 * ld_dst); q.nvec = nvec;
+        {
+            const cuuint64_t nfx = c->nfree[0], nfy = c->nfree[1], nfz = c->nfree[2], p = c->p;
+            const cuuint64_t sd[4] = {(cuuint64_t)2 * nvec, 2 * nfx, nfy, nfz};
+            const cuuint64_t ss[3] = {(cuuint64_t)ld * 16, 2 * nfx * (cuuint64_t)ld * 16, nfy * 2 * nfx * (cuuint64_t)ld * 16};
+            const cuuint32_t sb[4] = {(cuuint32_t)(ci.lanes / 2), (cuuint32_t)(2 * p), (cuuint32_t)p, (cuuint32_t)p};
+            const cuuint64_t vd[3] = {4 * nfx, nfy, nfz};
+            const cuuint64_t vs[2] = {nfx * 32, nfy * nfx * 32};
+            const cuuint32_t vbx[3] = {(cuuint32_t)(4 * p), (cuuint32_t)p, (cuuint32_t)p};
+            if (((uintptr_t)src & 15) != 0) return fail(c, CSF_EINVAL, "block pointer must be 16-byte aligned");
+            if (!encode_map(&q.tm_src, src, 4, sd, ss, sb) || !encode_map(&q.tm_vb, c->d_vb.p, 3, vd, vs, vbx))
+                return fail(c, CSF_ECUDA, "cuTensorMapEncodeTiled failed");
+        }
         q.ncx = c->ncell[0]; q.ncy = c->ncell[1]; q.ncz = c->ncell[2];
         q.nfx = c->nfree[0]; q.nfy = c->nfree[1]; q.nfz = c->nfree[2];
         q.bcx = c->bc[0]; q.bcy = c->bc[1]; q.bcz = c->bc[2];

@@ -30,6 +30,7 @@
 // x 8 lanes x 4 projectors each; the tensor pipe works while the FP64 pipe does phase A), and they stage the nodal
 // potential of the next cell into shared memory.
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <cstdint>
 
@@ -39,6 +40,10 @@ constexpr int kColTab = 8;
 constexpr int kColAux = 64;      // auxiliary threads (2 warps)
 
 struct ColParams {
+    // TMA descriptors (cuTensorMapEncodeTiled): src viewed as [nfz][nfy][2 nfx rows][2 nvec doubles], box = the owned
+    // nodes of one cell x L/2 doubles per spin row; vb viewed as [nfz][nfy][4 nfx doubles], box = one cell's owned nodes
+    alignas(64) CUtensorMap tm_src;
+    alignas(64) CUtensorMap tm_vb;
     double Ah[kColTab][kColTab];         // h-independent Loewdin-scaled 1-D stiffness (times 1/2), see above
     double uh[kColTab];                  // rank-one part of the 1-D mass
     double ax, rho_y, rho_z;             // 2/h_x^2, h_x^2/h_y^2, h_x^2/h_z^2
@@ -94,24 +99,27 @@ template <int P, int L> struct ColCfg {
     static constexpr int NT = NTM + kColAux;                         // threads per CTA
     static constexpr int PLANE = N * N * L;                          // doubles per ring plane and field
     static constexpr int EPLANE = P * P * L;
-    static constexpr int VPLANE = P * P * 4;                         // staged potential of one plane
-    // a2 ring, b2 ring, E ring, X (2 buffers), potential stage (N planes)
-    static constexpr size_t SMEM = (size_t)(2 * N * PLANE + N * EPLANE + 2 * P * EPLANE + N * VPLANE) * sizeof(double);
+    static constexpr int VCELL = P * P * P * 4;                      // V, Bx, By, Bz of the owned nodes of one cell
+    // a2 ring, b2 ring, X (nodal + nonlocal terms on the owned nodes of the current cell), staged potential, mbarrier
+    static constexpr size_t XOFF = ((size_t)2 * N * PLANE * sizeof(double) + 127) / 128 * 128;
+    static constexpr size_t VOFF = (XOFF + (size_t)P * EPLANE * sizeof(double) + 127) / 128 * 128;
+    static constexpr size_t MOFF = (VOFF + (size_t)VCELL * sizeof(double) + 15) / 16 * 16;
+    static constexpr size_t SMEM = MOFF + 16;
 };
 
 // FAST: every node of the mesh is unconstrained (all directions periodic), nvec is a multiple of L/4 and the cells
 // are cubes (rho_y = rho_z = 1), so no load, store or RED needs a predicate and no rho multiply is issued.
 template <int P, int KS, bool FAST, int L>
-__global__ void __launch_bounds__(ColCfg<P, L>::NT, (P >= 4 && P <= 5) ? 2 : 1) column_kernel(const __grid_constant__ ColParams A) {
+__global__ void __launch_bounds__(ColCfg<P, L>::NT, (P >= 4 && P <= 5) ? 3 : 1) column_kernel(const __grid_constant__ ColParams A) {
     using Cfg = ColCfg<P, L>;
     constexpr int N = Cfg::N, NTM = Cfg::NTM, VPC = L / 4;        // VPC vectors per CTA
-    constexpr int PLANE = Cfg::PLANE, EPLANE = Cfg::EPLANE, VPLANE = Cfg::VPLANE;
-    extern __shared__ double smem[];
+    constexpr int PLANE = Cfg::PLANE, EPLANE = Cfg::EPLANE;
+    extern __shared__ __align__(128) double smem[];
     double* R1 = smem;
     double* R2 = R1 + N * PLANE;
-    double* E = R2 + N * PLANE;
-    double* Xb = E + N * EPLANE;
-    double* VS = Xb + 2 * P * EPLANE;
+    double* X = reinterpret_cast<double*>(reinterpret_cast<char*>(smem) + Cfg::XOFF);
+    double* VS = reinterpret_cast<double*>(reinterpret_cast<char*>(smem) + Cfg::VOFF);
+    const unsigned mbar = (unsigned)__cvta_generic_to_shared(reinterpret_cast<char*>(smem) + Cfg::MOFF);
 
 #define AH(i, j) ((&A.Ah[0][0])[col_canon<N>(i, j)])
 #define UH(i) (((P & 1) && (i) > N - 1 - (i)) ? -A.uh[N - 1 - (i)] : A.uh[(i) < N - 1 - (i) ? (i) : N - 1 - (i)])
@@ -131,22 +139,9 @@ __global__ void __launch_bounds__(ColCfg<P, L>::NT, (P >= 4 && P <= 5) ? 2 : 1) 
     const int tid = threadIdx.x;
     const int plane_nodes = A.nfx * A.nfy;
 
-    // nodal potential (V, Bx, By, Bz) of owned node `task` of the segment planes starting at g0 -> two double2
-    auto load_vb = [&](int g0, int task, double2& v01, double2& v23) {
-        const int pl = task / (P * P), rem = task - pl * (P * P);
-        const int j = rem / P, i = rem - j * P;
-        const int gx = col_free_index(cx * P + i, A.ncx, P, A.bcx), gy = col_free_index(cy * P + j, A.ncy, P, A.bcy);
-        const int gz = col_free_index(cz0 * P + g0 + pl, A.ncz, P, A.bcz);
-        v01 = make_double2(0.0, 0.0); v23 = v01;
-        if (FAST || (gx >= 0 && gy >= 0 && gz >= 0)) {
-            const double2* vp = reinterpret_cast<const double2*>(A.vb) + 2 * ((long long)gz * plane_nodes + gy * A.nfx + gx);
-            v01 = __ldg(vp); v23 = __ldg(vp + 1);
-        }
-    };
-    for (int task = tid; task < N * P * P; task += Cfg::NT) {
-        double2 v01, v23; load_vb(0, task, v01, v23);
-        double2* o = reinterpret_cast<double2*>(VS + task * 4);
-        o[0] = v01; o[1] = v23;
+    if (tid == 0) {
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(mbar));
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
 
@@ -177,9 +172,38 @@ __global__ void __launch_bounds__(ColCfg<P, L>::NT, (P >= 4 && P <= 5) ? 2 : 1) 
                 }
         };
         for (int t = 0; t < S; ++t) {
-            double* X = Xb + (t & 1) * P * EPLANE;
-            if (t >= 2) col_bar_sync(4 + (t & 1), Cfg::NT);      // phase B(t - 2) has consumed this buffer
-            for (int idx = xr0 * (L / 2) + wl; idx < xr1 * (L / 2); idx += 32) reinterpret_cast<double2*>(X)[idx] = make_double2(0.0, 0.0);
+            if (t >= 1) col_bar_sync(3, Cfg::NT);                // phase B(t - 1) has consumed X
+            // TMA: the owned nodes of cell t (src rows of both spins, this CTA's vectors) land in X, their nodal
+            // potential in VS; nodes outside the mesh (Dirichlet faces) and vectors >= nvec are zero-filled
+            if (aw == 0 && wl == 0) {
+                const int bx0 = cx * P - (A.bcx == 0 ? 0 : 1), by0 = cy * P - (A.bcy == 0 ? 0 : 1), bz0 = (cz0 + t) * P - (A.bcz == 0 ? 0 : 1);
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mbar), "r"((unsigned)((P * EPLANE + Cfg::VCELL) * sizeof(double))) : "memory");
+                asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];"
+                             ::"r"((unsigned)__cvta_generic_to_shared(X)), "l"(&A.tm_src), "r"(chunk * VPC * 2), "r"(bx0 * 2), "r"(by0), "r"(bz0), "r"(mbar) : "memory");
+                asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+                             ::"r"((unsigned)__cvta_generic_to_shared(VS)), "l"(&A.tm_vb), "r"(bx0 * 4), "r"(by0), "r"(bz0), "r"(mbar) : "memory");
+            }
+            {
+                unsigned done = 0;
+                while (!done)
+                    asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }" : "=r"(done) : "r"(mbar), "r"((unsigned)(t & 1)) : "memory");
+            }
+            // X = (V + B.sigma - c) X in place on this warp's rows: thread = (node, vector), both spins and re/im in
+            // registers, so the 2x2 spin block needs no exchange between threads
+            for (int task = wl; task < (xr1 - xr0) * VPC; task += 32) {
+                const int loc = xr0 + task / VPC, vl = task % VPC;
+                double2* xu = reinterpret_cast<double2*>(X + loc * L) + vl;
+                const double2 uu = xu[0], ud = xu[L / 4];
+                const double2 v01 = reinterpret_cast<const double2*>(VS)[2 * loc], v23 = reinterpret_cast<const double2*>(VS)[2 * loc + 1];
+                const double vv = v01.x - A.shift, bx = v01.y, by = v23.x, bz = v23.y;
+                double2 ou, od;
+                ou.x = fma(vv + bz, uu.x, fma(bx, ud.x, by * ud.y));
+                ou.y = fma(vv + bz, uu.y, fma(bx, ud.y, -by * ud.x));
+                od.x = fma(vv - bz, ud.x, fma(bx, uu.x, -by * uu.y));
+                od.y = fma(vv - bz, ud.y, fma(bx, uu.y, by * uu.x));
+                xu[0] = ou; xu[L / 4] = od;
+            }
             __syncwarp();
             if (A.sub_ptr != nullptr) {
                 const int cell = cx + A.ncx * (cy + A.ncy * (cz0 + t));
@@ -232,7 +256,7 @@ __global__ void __launch_bounds__(ColCfg<P, L>::NT, (P >= 4 && P <= 5) ? 2 : 1) 
                 }
             }
             __threadfence_block();
-            col_bar_arrive(2 + (t & 1), Cfg::NT);                // X(t) is complete
+            col_bar_arrive(2, Cfg::NT);                          // X(t) is complete
         }
         return;
     }
@@ -255,8 +279,6 @@ __global__ void __launch_bounds__(ColCfg<P, L>::NT, (P >= 4 && P <= 5) ? 2 : 1) 
     const int slot_out = ri ^ (A.rot & 1);
     const unsigned sgn = (A.rot == 2 || (A.rot == 1 && ri == 1) || (A.rot == 3 && ri == 0)) ? 0x80000000u : 0u;
     double* dp = A.dst + ((long long)spin * (A.rd >> 2) + vec) * 2 + slot_out;
-    const double sz = spin ? -1.0 : 1.0;
-    const double sy = (spin == ri) ? 1.0 : -1.0;
     const double scax = A.sc * A.ax;
 
     double u[N][N];
@@ -297,25 +319,6 @@ __global__ void __launch_bounds__(ColCfg<P, L>::NT, (P >= 4 && P <= 5) ? 2 : 1) 
             const int slot = act ? g % N : 0;
             double* r1 = R1 + slot * PLANE + lane;
             double* r2 = R2 + slot * PLANE + lane;
-            // nodal terms on the nodes this plane owns (the last plane of the segment belongs to the next segment)
-            {
-                const int gz = act ? col_free_index(cz0 * P + g, A.ncz, P, A.bcz) : -1;
-                const bool own_plane = act && g < S * P && gz >= 0;
-                double* ep = E + slot * EPLANE + lane;
-                const int pidx = t == 0 ? (act ? g : 0) : (act ? g - t * P - 1 : 0);
-                const double2* vs = reinterpret_cast<const double2*>(VS + pidx * VPLANE);
-#pragma unroll
-                for (int j = 0; j < P; ++j)
-#pragma unroll
-                    for (int i = 0; i < P; ++i) {
-                        const double own = u[j][i];
-                        const double t1 = __shfl_xor_sync(0xffffffffu, own, L / 2);   // other spin, same re/im
-                        const double t2 = __shfl_xor_sync(0xffffffffu, t1, 1);        // other spin, other re/im
-                        const double2 v01 = vs[(j * P + i) * 2], v23 = vs[(j * P + i) * 2 + 1];
-                        const double e = fma(v01.x - A.shift + sz * v23.y, own, fma(v01.y, t1, sy * v23.x * t2));
-                        if (own_plane) ep[(j * P + i) * L] = e;
-                    }
-            }
             // x-step bookkeeping: d[j] = uh . u[j][:]
             double d[N];
 #pragma unroll
@@ -352,17 +355,9 @@ __global__ void __launch_bounds__(ColCfg<P, L>::NT, (P >= 4 && P <= 5) ? 2 : 1) 
                 }
             }
         }
-        // in flight during phase B: the next planes and their nodal potential
-        constexpr int VT = (P * P * P + NTM - 1) / NTM;
-        double2 nv01[VT], nv23[VT];
-        if (t + 1 < S) {
-            load_plane(plane_of(t + 1));
-#pragma unroll
-            for (int v = 0; v < VT; ++v) if (tid + v * NTM < P * P * P) load_vb((t + 1) * P + 1, tid + v * NTM, nv01[v], nv23[v]);
-        }
-        col_bar_sync(1, NTM);                                 // ring, E written; VS no longer read
-        col_bar_sync(2 + (t & 1), Cfg::NT);                   // X(t) complete
-        const double* X = Xb + (t & 1) * P * EPLANE;
+        if (t + 1 < S) load_plane(plane_of(t + 1));          // in flight during phase B
+        col_bar_sync(1, NTM);                                 // ring written
+        col_bar_sync(2, Cfg::NT);                             // X(t) complete
         // ------------------------------------------------------------------ phase B
         if (q_on) {
             const int j = q;
@@ -378,7 +373,6 @@ __global__ void __launch_bounds__(ColCfg<P, L>::NT, (P >= 4 && P <= 5) ? 2 : 1) 
             }
             const double* r1 = R1 + j * N * L + lane;
             const double* r2 = R2 + j * N * L + lane;
-            const double* ep = E + j * P * L + lane;
             const double* xp = X + j * P * L + lane;
 #pragma unroll
             for (int i = 0; i < N; ++i) {
@@ -406,23 +400,15 @@ __global__ void __launch_bounds__(ColCfg<P, L>::NT, (P >= 4 && P <= 5) ? 2 : 1) 
 #pragma unroll
                 for (int k = 0; k < P; ++k) {
                     double v;
-                    if (j < P && i < P) v = fma(scax, o[k], A.sc * (ep[so[k] * EPLANE + i * L] + xp[k * EPLANE + i * L]));
+                    if (j < P && i < P) v = fma(scax, o[k], A.sc * xp[k * EPLANE + i * L]);
                     else v = scax * o[k];
                     if (FAST || (xy_ok && zn[k] >= 0)) atomicAdd(dp + (long long)(xy + zn[k]) * A.rd, col_flip(v, sgn));
                 }
                 if (t == S - 1 && (FAST || (xy_ok && zn[P] >= 0))) atomicAdd(dp + (long long)(xy + zn[P]) * A.rd, col_flip(scax * carry[i], sgn));
             }
         }
-        if (t + 1 < S) {
-#pragma unroll
-            for (int v = 0; v < VT; ++v)
-                if (tid + v * NTM < P * P * P) {
-                    double2* o = reinterpret_cast<double2*>(VS + (tid + v * NTM) * 4);
-                    o[0] = nv01[v]; o[1] = nv23[v];
-                }
-        }
-        if (t + 2 < S) col_bar_arrive(4 + (t & 1), Cfg::NT);  // X buffer t & 1 is free
-        col_bar_sync(1, NTM);                                 // ring free, VS visible
+        if (t + 1 < S) col_bar_arrive(3, Cfg::NT);            // X is free
+        col_bar_sync(1, NTM);                                 // ring free
     }
 #undef AH
 #undef UH
