@@ -110,7 +110,7 @@ template <int P, int L> struct ColCfg {
 // FAST: every node of the mesh is unconstrained (all directions periodic), nvec is a multiple of L/4 and the cells
 // are cubes (rho_y = rho_z = 1), so no load, store or RED needs a predicate and no rho multiply is issued.
 template <int P, int KS, bool FAST, int L>
-__global__ void __launch_bounds__(ColCfg<P, L>::NT, (P >= 4 && P <= 5) ? 3 : 1) column_kernel(const __grid_constant__ ColParams A) {
+__global__ void __launch_bounds__(ColCfg<P, L>::NT) __maxnreg__((P >= 4 && P <= 5) ? 136 : 255) column_kernel(const __grid_constant__ ColParams A) {
     using Cfg = ColCfg<P, L>;
     constexpr int N = Cfg::N, NTM = Cfg::NTM, VPC = L / 4;        // VPC vectors per CTA
     constexpr int PLANE = Cfg::PLANE, EPLANE = Cfg::EPLANE;
@@ -153,7 +153,7 @@ __global__ void __launch_bounds__(ColCfg<P, L>::NT, (P >= 4 && P <= 5) ? 3 : 1) 
         // same row and need no barrier between them. Its sub-pairs (cell, atom, range) come from the host.
         const int aw = warp_id - NTM / 32, wl = tid & 31;
         const int kk = wl & 3, rw = wl >> 2;
-        constexpr int XSPLIT = (P * P * P + 1) / 2, TMAX = (XSPLIT + 7) / 8, TCH = TMAX < 8 ? TMAX : 8;
+        constexpr int XSPLIT = (P * P * P + 1) / 2, TMAX = (XSPLIT + 7) / 8, TCH = TMAX < 5 ? TMAX : 5;
         const int xr0 = aw * XSPLIT, xr1 = min(P * P * P, xr0 + XSPLIT);
         const double* cbase[L / 8]; bool bon[L / 8];
 #pragma unroll
@@ -268,13 +268,21 @@ __global__ void __launch_bounds__(ColCfg<P, L>::NT, (P >= 4 && P <= 5) ? 3 : 1) 
     const bool lane_on = FAST || vec < A.nvec;
     const bool q_on = q < N;
 
-    int xo[N], yo[N];                 // node offsets of the column's x / y indices (or -1 on a Dirichlet face)
+    // node offsets of the column's x / y indices (or -1 on a Dirichlet face). On a periodic mesh only the last index
+    // of the last cell wraps, so the FAST kernel keeps two numbers per direction instead of the arrays.
+    int xo_[FAST ? 1 : N], yo_[FAST ? 1 : N];
+    const int x0f = cx * P, xPf = (cx == A.ncx - 1) ? 0 : cx * P + P;
+    const int y0f = cy * P * A.nfx, yPf = (cy == A.ncy - 1) ? 0 : (cy * P + P) * A.nfx;
+    if (!FAST) {
 #pragma unroll
-    for (int i = 0; i < N; ++i) {
-        xo[i] = col_free_index(cx * P + i, A.ncx, P, A.bcx);
-        const int gy = col_free_index(cy * P + i, A.ncy, P, A.bcy);
-        yo[i] = gy < 0 ? -1 : gy * A.nfx;
+        for (int i = 0; i < N; ++i) {
+            xo_[i] = col_free_index(cx * P + i, A.ncx, P, A.bcx);
+            const int gy = col_free_index(cy * P + i, A.ncy, P, A.bcy);
+            yo_[i] = gy < 0 ? -1 : gy * A.nfx;
+        }
     }
+#define XO(i) (FAST ? ((i) < P ? x0f + (i) : xPf) : xo_[FAST ? 0 : (i)])
+#define YO(j) (FAST ? ((j) < P ? y0f + (j) * A.nfx : yPf) : yo_[FAST ? 0 : (j)])
     const double* sp = A.src + ((long long)spin * (A.rs >> 2) + vec) * 2 + ri;
     const int slot_out = ri ^ (A.rot & 1);
     const unsigned sgn = (A.rot == 2 || (A.rot == 1 && ri == 1) || (A.rot == 3 && ri == 0)) ? 0x80000000u : 0u;
@@ -299,12 +307,12 @@ __global__ void __launch_bounds__(ColCfg<P, L>::NT, (P >= 4 && P <= 5) ? 3 : 1) 
         const int zn = (gz < 0 ? 0 : gz) * plane_nodes;
 #pragma unroll
         for (int j = 0; j < N; ++j) {
-            const int yz = zn + (FAST ? yo[j] : max(yo[j], 0));
+            const int yz = zn + (FAST ? YO(j) : max(YO(j), 0));
 #pragma unroll
             for (int i = 0; i < N; ++i) {
-                const int node = yz + (FAST ? xo[i] : max(xo[i], 0));
+                const int node = yz + (FAST ? XO(i) : max(XO(i), 0));
                 if (FAST) u[j][i] = __ldg(sp + (long long)node * A.rs);       // idle threads read plane 0 and drop it
-                else u[j][i] = (pz && xo[i] >= 0 && yo[j] >= 0) ? __ldg(sp + (long long)node * A.rs) : 0.0;
+                else u[j][i] = (pz && XO(i) >= 0 && YO(j) >= 0) ? __ldg(sp + (long long)node * A.rs) : 0.0;
             }
         }
     };
@@ -395,8 +403,8 @@ __global__ void __launch_bounds__(ColCfg<P, L>::NT, (P >= 4 && P <= 5) ? 3 : 1) 
                 }
                 o[0] += carry[i];
                 carry[i] = o[P];
-                const bool xy_ok = FAST || (lane_on && xo[i] >= 0 && yo[j] >= 0);
-                const int xy = FAST ? xo[i] + yo[j] : max(xo[i], 0) + max(yo[j], 0);
+                const bool xy_ok = FAST || (lane_on && XO(i) >= 0 && YO(j) >= 0);
+                const int xy = FAST ? XO(i) + YO(j) : max(XO(i), 0) + max(YO(j), 0);
 #pragma unroll
                 for (int k = 0; k < P; ++k) {
                     double v;
@@ -411,6 +419,8 @@ __global__ void __launch_bounds__(ColCfg<P, L>::NT, (P >= 4 && P <= 5) ? 3 : 1) 
         col_bar_sync(1, NTM);                                 // ring free
     }
 #undef AH
+#undef XO
+#undef YO
 #undef UH
 #undef BETA
 }
