@@ -10,6 +10,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <numeric>
 #include <string>
@@ -43,8 +44,8 @@ struct csf_ctx {
     Gll1D gll; Dir1D dir[3];
     bool have_pot = false;
     DevBuf d_cell_order, d_col_order, d_vb;
-    DevBuf d_sub_ptr, d_sub_desc, d_ent_locf;
-    int seg_len = 8, chunk_group = 4;
+    DevBuf d_sub_ptr, d_sub_desc, d_ent_locf, d_a_pack;
+    int seg_len = 16, chunk_group = 16;
     // projectors
     int natoms = 0, npj_uniform = 0, npjp = 0; long long crows = 0;
     DevBuf d_pair_ptr, d_pair_atom, d_pair_off, d_ent_loc, d_ent_node, d_ent_p, d_atom_coff, d_atom_npj, d_atom_type,
@@ -130,6 +131,8 @@ bool encode_map(CUtensorMap* tm, const void* base, int rank, const cuuint64_t* d
               CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
+size_t ctp_bytes(const csf_ctx* c, int nvec);
+
 // one step: dst += sc * i^rot * (Hhat - shift) src
 int enqueue_step(csf_ctx* c, const double* src, long long ld, double* dst, long long ld_dst, int nvec, double sc, int rot, double shift,
                  double* dC, double* dCt) {
@@ -150,7 +153,10 @@ int enqueue_step(csf_ctx* c, const double* src, long long ld, double* dst, long 
         }
         CSF_CUDA(c, cudaGetLastError());
         DeltaParams dp{};
-        dp.C = reinterpret_cast<const double2*>(dC); dp.Ct = reinterpret_cast<double2*>(dCt); dp.ldc = ldc; dp.nvec = nvec;
+        const int lanes = column_info(c->p).lanes, nchunks = (nvec + lanes / 4 - 1) / (lanes / 4);
+        CSF_CUDA(c, cudaMemsetAsync(dCt, 0, ctp_bytes(c, nvec), c->stream));
+        dp.C = reinterpret_cast<const double2*>(dC); dp.Ct = dCt; dp.ldc = ldc; dp.nvec = nvec;
+        dp.lanes = lanes; dp.ks = c->npjp / 4; dp.nchunks = nchunks;
         dp.atom_coff = c->d_atom_coff.as<long long>(); dp.atom_npj = c->d_atom_npj.as<int>(); dp.atom_type = c->d_atom_type.as<int>();
         dp.delta = c->d_delta.as<double2>(); dp.delta_ptr = c->d_delta_ptr.as<long long>();
         dim3 dg(c->natoms, (nvec + 31) / 32);
@@ -194,7 +200,7 @@ int enqueue_step(csf_ctx* c, const double* src, long long ld, double* dst, long 
         if (c->natoms > 0) {
             q.sub_ptr = c->d_sub_ptr.as<int>(); q.sub_desc = c->d_sub_desc.as<int4>();
             q.ent_loc = c->d_ent_locf.as<int>(); q.ent_p = c->d_ent_p.as<double>();
-            q.Ct = dCt; q.ldc = ldc; q.npjp = c->npjp;
+            q.Ct = dCt; q.npjp = c->npjp; q.a_pack = c->d_a_pack.as<double>();
         }
         const long long ngroups = (q.nchunks + q.chunk_group - 1) / q.chunk_group;
         const long long nblocks = (long long)q.chunk_group * q.ncols * q.nseg * ngroups;
@@ -211,6 +217,11 @@ int enqueue_step(csf_ctx* c, const double* src, long long ld, double* dst, long 
 }
 
 size_t block_bytes(const csf_ctx* c, int nvec) { return (size_t)2 * c->M * nvec * sizeof(double2); }
+// C~ in fragment order: [atom][chunk][KS][L/8][32] doubles
+size_t ctp_bytes(const csf_ctx* c, int nvec) {
+    const int lanes = column_info(c->p).lanes, nchunks = (nvec + lanes / 4 - 1) / (lanes / 4);
+    return ((size_t)c->natoms * nchunks * (c->npjp / 4) * (lanes / 8) * 32 * sizeof(double) + 255) / 256 * 256;
+}
 size_t coef_bytes(const csf_ctx* c, int nvec) { return ((size_t)c->crows * nvec * sizeof(double2) + 255) / 256 * 256; }
 
 int enqueue_zero(csf_ctx* c, double* dst, long long ld, int nvec) {
@@ -273,6 +284,9 @@ int csf_create(csf_ctx** out, const int ncell[3], const double box[3], int order
     ce = cudaGetDeviceProperties(&prop, device);
     if (ce != cudaSuccess) { delete c; return cuda_fail(nullptr, ce, "cudaGetDeviceProperties"); }
     c->sm_count = prop.multiProcessorCount; c->smem_optin = prop.sharedMemPerBlockOptin;
+    // tuning hooks for sweeps (defaults are the measured best on B200): cells per z-segment, vector chunks per group
+    if (const char* e = std::getenv("CSF_SEG_LEN")) { int v = std::atoi(e); if (v >= 1) c->seg_len = v; }
+    if (const char* e = std::getenv("CSF_CHUNK_GROUP")) { int v = std::atoi(e); if (v >= 1) c->chunk_group = v; }
     // traversal order of the cells: 8x8x8 bricks, x fastest inside, so that the faces shared between
     // neighbouring cells are combined in L2 before they are evicted
     std::vector<int> order_v; order_v.reserve(E);
@@ -437,19 +451,32 @@ int csf_set_projectors(csf_ctx* c, int natoms, const int64_t* node_ptr, const in
     for (const Pair& pr : pairs) {
         const int e0 = pr.off[0], e1 = pr.off[p];
         int em = e0; while (em < e1 && ent_locf[em] < xsplit) ++em;
-        const int coff = (int)atom_coff[pr.atom], npj = nproj[pr.atom];
-        if (em > e0) subs.push_back({pr.cell * 2, make_int4(coff, npj, e0, em)});
-        if (e1 > em) subs.push_back({pr.cell * 2 + 1, make_int4(coff, npj, em, e1)});
+        if (em > e0) subs.push_back({pr.cell * 2, make_int4(pr.atom, 0, e0, em)});
+        if (e1 > em) subs.push_back({pr.cell * 2 + 1, make_int4(pr.atom, 0, em, e1)});
     }
     std::stable_sort(subs.begin(), subs.end(), [](const Sub& x, const Sub& y) { return x.key < y.key; });
     std::vector<int> sub_ptr(2 * (size_t)c->E + 1, 0); std::vector<int4> sub_desc(subs.size());
-    for (size_t q = 0; q < subs.size(); ++q) { sub_ptr[subs[q].key + 1]++; sub_desc[q] = subs[q].d; }
+    long long ntiles = 0;
+    for (size_t q = 0; q < subs.size(); ++q) {
+        sub_ptr[subs[q].key + 1]++;
+        subs[q].d.y = (int)ntiles; ntiles += (subs[q].d.w - subs[q].d.z + 7) / 8;
+        sub_desc[q] = subs[q].d;
+    }
+    if (ntiles >= (1LL << 31)) return fail(c, CSF_EUNSUPPORTED, "too many projector tiles");
     for (size_t q = 0; q < 2 * (size_t)c->E; ++q) sub_ptr[q + 1] += sub_ptr[q];
+    // P~ of every tile (8 rows of a sub-pair) in the order of the DMMA A fragment: [tile][k-step][lane = row*4 + k]
+    const int ks = npjp / 4;
+    std::vector<double> a_pack((size_t)ntiles * ks * 32, 0.0);
+    for (const Sub& sb : subs)
+        for (int e = sb.d.z; e < sb.d.w; ++e) {
+            const size_t tile = (size_t)sb.d.y + (e - sb.d.z) / 8; const int row = (e - sb.d.z) % 8;
+            for (int x = 0; x < npjp; ++x) a_pack[(tile * ks + x / 4) * 32 + row * 4 + x % 4] = ent_p[(size_t)e * npjp + x];
+        }
     std::vector<double2> dl((size_t)delta_ptr[ntypes]);
     for (size_t i = 0; i < dl.size(); ++i) dl[i] = make_double2(delta[i].re, delta[i].im);
     std::vector<long long> dptr(delta_ptr, delta_ptr + ntypes + 1);
     CSF_CUDA(c, c->d_pair_ptr.upload(pair_ptr)); CSF_CUDA(c, c->d_pair_atom.upload(pair_atom)); CSF_CUDA(c, c->d_pair_off.upload(pair_off));
-    CSF_CUDA(c, c->d_sub_ptr.upload(sub_ptr)); CSF_CUDA(c, c->d_sub_desc.upload(sub_desc)); CSF_CUDA(c, c->d_ent_locf.upload(ent_locf));
+    CSF_CUDA(c, c->d_sub_ptr.upload(sub_ptr)); CSF_CUDA(c, c->d_sub_desc.upload(sub_desc)); CSF_CUDA(c, c->d_a_pack.upload(a_pack)); CSF_CUDA(c, c->d_ent_locf.upload(ent_locf));
     CSF_CUDA(c, c->d_ent_loc.upload(ent_loc)); CSF_CUDA(c, c->d_ent_node.upload(ent_node)); CSF_CUDA(c, c->d_ent_p.upload(ent_p));
     CSF_CUDA(c, c->d_atom_coff.upload(atom_coff)); CSF_CUDA(c, c->d_atom_npj.upload(atom_npj)); CSF_CUDA(c, c->d_atom_type.upload(atom_ty));
     CSF_CUDA(c, c->d_delta.upload(dl)); CSF_CUDA(c, c->d_delta_ptr.upload(dptr));
@@ -462,13 +489,13 @@ int csf_set_projectors(csf_ctx* c, int natoms, const int64_t* node_ptr, const in
 int csf_workspace_bytes(const csf_ctx* c, int nvec, int mode, size_t* bytes) {
     if (!c || !bytes || nvec < 0) return CSF_EINVAL;
     if (mode != CSF_FP64) return CSF_EUNSUPPORTED;
-    *bytes = block_bytes(c, nvec) + 2 * coef_bytes(c, nvec) + 256;
+    *bytes = block_bytes(c, nvec) + coef_bytes(c, nvec) + ctp_bytes(c, nvec) + 256;
     return CSF_OK;
 }
 
 int csf_apply_H(csf_ctx* c, const csf_c128* dX, csf_c128* dY, int64_t ld, int nvec, void* d_work, size_t work_bytes) {
     if (!c) return CSF_EINVAL;
-    const size_t need = c->natoms > 0 ? 2 * coef_bytes(c, std::max(nvec, 0)) : 0;
+    const size_t need = c->natoms > 0 ? coef_bytes(c, std::max(nvec, 0)) + ctp_bytes(c, std::max(nvec, 0)) : 0;
     int rc = check_block_args(c, dX, dY, ld, nvec, d_work, work_bytes, need);
     if (rc != CSF_OK || nvec == 0) return rc;
     CSF_CUDA(c, cudaSetDevice(c->device));

@@ -58,11 +58,12 @@ struct ColParams {
     double shift, sc; int rot;           // gamma = sc * i^rot, c = shift
     // projector expansion: (cell, atom) pairs, entries sorted by local owned index
     const int* sub_ptr;                  // [2 ncells + 1] sub-pairs (cell, atom, half of the owned-node range)
-    const int4* sub_desc;                // [nsub] {first row of the atom in C~, n_pj, entry begin, entry end}
+    const int4* sub_desc;                // [nsub] {atom, first tile in a_pack, entry begin, entry end}
+    const double* a_pack;                // [ntiles][KS][32] P~ in DMMA A-fragment order (lane = row*4 + k), zero padded
     const int* ent_loc;                  // [nent] local owned index (lz*p + ly)*p + lx
     const double* ent_p;                 // [nent][npjp] S_I P_{I chi}, zero padded
-    const double* Ct;                    // C~ [rows][ldc] complex128
-    long long ldc; int npjp;
+    const double* Ct;                    // C~ in B-fragment order: [atom][chunk][KS][L/8][32] (DeltaParams)
+    int npjp;
 };
 
 __device__ __forceinline__ double col_flip(double x, unsigned mask) {
@@ -155,21 +156,12 @@ __global__ void __launch_bounds__(ColCfg<P, L>::NT) __maxnreg__((P >= 4 && P <= 
         const int kk = wl & 3, rw = wl >> 2;
         constexpr int XSPLIT = (P * P * P + 1) / 2, TMAX = (XSPLIT + 7) / 8, TCH = TMAX < 5 ? TMAX : 5;
         const int xr0 = aw * XSPLIT, xr1 = min(P * P * P, xr0 + XSPLIT);
-        const double* cbase[L / 8]; bool bon[L / 8];
-#pragma unroll
-        for (int nt = 0; nt < L / 8; ++nt) {
-            const int dl = nt * 8 + rw, bspin = dl / (L / 2), bvec = chunk * VPC + ((dl % (L / 2)) >> 1);
-            cbase[nt] = A.Ct + ((long long)bspin * A.ldc + bvec) * 2 + (dl & 1);
-            bon[nt] = FAST || bvec < A.nvec;
-        }
         auto load_b = [&](const int4& ds, double (&bb)[KS][L / 8]) {
+            const double* cb = A.Ct + ((long long)ds.x * A.nchunks + chunk) * (KS * (L / 8) * 32) + wl;
 #pragma unroll
-            for (int nt = 0; nt < L / 8; ++nt)
+            for (int s = 0; s < KS; ++s)
 #pragma unroll
-                for (int s = 0; s < KS; ++s) {
-                    const int chi = 4 * s + kk;
-                    bb[s][nt] = (chi < ds.y && bon[nt]) ? __ldg(cbase[nt] + ((long long)ds.x + 2 * chi) * A.ldc * 2) : 0.0;
-                }
+                for (int nt = 0; nt < L / 8; ++nt) bb[s][nt] = __ldg(cb + (s * (L / 8) + nt) * 32);
         };
         for (int t = 0; t < S; ++t) {
             if (t >= 1) col_bar_sync(3, Cfg::NT);                // phase B(t - 1) has consumed X
@@ -221,10 +213,10 @@ __global__ void __launch_bounds__(ColCfg<P, L>::NT) __maxnreg__((P >= 4 && P <= 
 #pragma unroll
                         for (int tl = 0; tl < TCH; ++tl) {
                             const int erow = eb + tl * 8 + rw;
-                            const bool vd = erow < e1;
-                            const double* ap = A.ent_p + (long long)(vd ? erow : e0) * A.npjp + kk;
+                            const bool vd = erow < e1, tv = eb + tl * 8 < e1;
+                            const double* ap = A.a_pack + ((long long)(ds.y + ((eb - e0) >> 3) + (tv ? tl : 0)) * KS) * 32 + wl;
 #pragma unroll
-                            for (int s = 0; s < KS; ++s) a[tl][s] = vd ? __ldg(ap + 4 * s) : 0.0;
+                            for (int s = 0; s < KS; ++s) a[tl][s] = tv ? __ldg(ap + s * 32) : 0.0;
                             loc[tl] = vd ? __ldg(A.ent_loc + erow) : -1;
                         }
 #pragma unroll

@@ -104,7 +104,11 @@ __global__ void __launch_bounds__(256) proj_gather_kernel(const __grid_constant_
 // grid = (atoms, vector chunks of 32); thread = (row group, vector).
 // ---------------------------------------------------------------------------------------------------
 struct DeltaParams {
-    const double2* C; double2* Ct; long long ldc; int nvec;
+    // Ct is written in the fragment order the column kernel's DMMA B operand wants: for (atom, chunk of VPC vectors)
+    // a block [KS][L/8][32] doubles, element (s, nt, lane = rw*4 + kk) = C~[2 (4s + kk) + spin][vector].{re, im} with the
+    // real lane nt*8 + rw = spin*(L/2) + 2*(vector % VPC) + ri; rows chi >= n_pj stay zero (the buffer is cleared).
+    const double2* C; double* Ct; long long ldc; int nvec;
+    int lanes, ks, nchunks;
     const long long* atom_coff; const int* atom_npj; const int* atom_type;
     const double2* delta; const long long* delta_ptr;
 };
@@ -124,7 +128,10 @@ __global__ void __launch_bounds__(256) delta_apply_kernel(const __grid_constant_
             sr = fma(d.x, c.x, sr); sr = fma(-d.y, c.y, sr);
             si = fma(d.x, c.y, si); si = fma(d.y, c.x, si);
         }
-        A.Ct[(base + r) * A.ldc + v] = make_double2(sr, si);
+        const int chi = r >> 1, spin = r & 1, vpc = A.lanes / 4;
+        const int dl = spin * (A.lanes / 2) + (v % vpc) * 2;
+        double* o = A.Ct + ((((long long)atom * A.nchunks + v / vpc) * A.ks + (chi >> 2)) * (A.lanes / 8) + (dl >> 3)) * 32 + (dl & 7) * 4 + (chi & 3);
+        o[0] = sr; o[4] = si;
     }
 }
 
