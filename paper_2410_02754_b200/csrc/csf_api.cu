@@ -49,7 +49,7 @@ struct csf_ctx {
     // projectors
     int natoms = 0, npj_uniform = 0, npjp = 0; long long crows = 0;
     DevBuf d_pair_ptr, d_pair_atom, d_pair_off, d_ent_loc, d_ent_node, d_ent_p, d_atom_coff, d_atom_npj, d_atom_type,
-        d_delta, d_delta_ptr, d_gb_atom, d_gb_beg, d_gb_end;
+        d_delta, d_delta_ptr, d_gb_atom, d_gb_beg, d_gb_end, d_gb_k0, d_g_pack;
     int n_gather_blocks = 0;
     int variant = 0;
     long long launches = 0;
@@ -142,10 +142,10 @@ int enqueue_step(csf_ctx* c, const double* src, long long ld, double* dst, long 
         GatherParams gp{};
         gp.src = src; gp.ld = ld; gp.nvec = nvec;
         gp.gb_atom = c->d_gb_atom.as<int>(); gp.gb_beg = c->d_gb_beg.as<int>(); gp.gb_end = c->d_gb_end.as<int>();
-        gp.ent_node = c->d_ent_node.as<int>(); gp.ent_p = c->d_ent_p.as<double>(); gp.npjp = c->npjp;
+        gp.ent_node = c->d_ent_node.as<int>(); gp.g_pack = c->d_g_pack.as<double>(); gp.gb_k0 = c->d_gb_k0.as<int>();
         gp.atom_coff = c->d_atom_coff.as<long long>(); gp.atom_npj = c->d_atom_npj.as<int>();
         gp.C = dC; gp.ldc = ldc;
-        dim3 gg(c->n_gather_blocks, (nvec + 31) / 32);
+        dim3 gg(c->n_gather_blocks, (nvec + 16 * kGatherNT - 1) / (16 * kGatherNT));
         {
             ProfScope ps(c, CSF_KIND_PGATHER);
             if (c->npjp <= 24) proj_gather_kernel<3><<<gg, 256, 0, c->stream>>>(gp);
@@ -433,6 +433,20 @@ int csf_set_projectors(csf_ctx* c, int natoms, const int64_t* node_ptr, const in
         for (long long b = t0; b < t1; b += 256) { gb_atom.push_back(a); gb_beg.push_back((int)b); gb_end.push_back((int)std::min(b + 256, t1)); }
         pv_off += (t1 - t0) * nproj[a];
     }
+    // P~^T of every k-step (4 entries, aligned to the atom's first entry) in DMMA A-fragment order for the gather kernel:
+    // [k-step][m-tile][lane = (chi % 8) * 4 + entry % 4]
+    const int mt = npjp <= 24 ? 3 : 4;
+    std::vector<int> gb_k0(gb_atom.size());
+    std::vector<long long> atom_k0(natoms + 1, 0);
+    for (int a = 0; a < natoms; ++a) atom_k0[a + 1] = atom_k0[a] + (node_ptr[a + 1] - node_ptr[a] + 3) / 4;
+    if (atom_k0[natoms] >= (1LL << 31)) return fail(c, CSF_EUNSUPPORTED, "too many projector entries");
+    for (size_t b = 0; b < gb_atom.size(); ++b) gb_k0[b] = (int)(atom_k0[gb_atom[b]] + (gb_beg[b] - node_ptr[gb_atom[b]]) / 4);
+    std::vector<double> g_pack((size_t)atom_k0[natoms] * mt * 32, 0.0);
+    for (int a = 0; a < natoms; ++a)
+        for (long long e = node_ptr[a]; e < node_ptr[a + 1]; ++e) {
+            const size_t kstep = (size_t)atom_k0[a] + (e - node_ptr[a]) / 4; const int kq = (int)((e - node_ptr[a]) % 4);
+            for (int x = 0; x < nproj[a]; ++x) g_pack[(kstep * mt + x / 8) * 32 + (x % 8) * 4 + kq] = ent_p[(size_t)e * npjp + x];
+        }
     // cell-major pair lists
     std::vector<int> pair_ptr(c->E + 1, 0);
     for (const Pair& pr : pairs) pair_ptr[pr.cell + 1]++;
@@ -480,7 +494,7 @@ int csf_set_projectors(csf_ctx* c, int natoms, const int64_t* node_ptr, const in
     CSF_CUDA(c, c->d_ent_loc.upload(ent_loc)); CSF_CUDA(c, c->d_ent_node.upload(ent_node)); CSF_CUDA(c, c->d_ent_p.upload(ent_p));
     CSF_CUDA(c, c->d_atom_coff.upload(atom_coff)); CSF_CUDA(c, c->d_atom_npj.upload(atom_npj)); CSF_CUDA(c, c->d_atom_type.upload(atom_ty));
     CSF_CUDA(c, c->d_delta.upload(dl)); CSF_CUDA(c, c->d_delta_ptr.upload(dptr));
-    CSF_CUDA(c, c->d_gb_atom.upload(gb_atom)); CSF_CUDA(c, c->d_gb_beg.upload(gb_beg)); CSF_CUDA(c, c->d_gb_end.upload(gb_end));
+    CSF_CUDA(c, c->d_gb_k0.upload(gb_k0)); CSF_CUDA(c, c->d_g_pack.upload(g_pack)); CSF_CUDA(c, c->d_gb_atom.upload(gb_atom)); CSF_CUDA(c, c->d_gb_beg.upload(gb_beg)); CSF_CUDA(c, c->d_gb_end.upload(gb_end));
     c->natoms = natoms; c->crows = crows; c->npjp = npjp; c->npj_uniform = uniform ? nproj[0] : 0;
     c->n_gather_blocks = (int)gb_atom.size();
     return CSF_OK;

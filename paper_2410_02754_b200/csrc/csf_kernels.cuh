@@ -32,7 +32,8 @@ constexpr int kTabN = 8;
 struct GatherParams {
     const double* src; long long ld; int nvec;
     const int* gb_atom; const int* gb_beg; const int* gb_end;   // gather blocks over the entry list
-    const int* ent_node; const double* ent_p; int npjp;
+    const int* gb_k0;                                            // first k-step (4 entries) of the block in g_pack
+    const int* ent_node; const double* g_pack;                   // P~^T in A-fragment order [k-step][MT][32]
     const long long* atom_coff; const int* atom_npj;
     double* C; long long ldc;
 };
@@ -41,46 +42,56 @@ __device__ __forceinline__ void gather_dmma(double& d0, double& d1, double a, do
     asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
 }
 
+constexpr int kGatherNT = 4;     // n-tiles (of 4 vectors) per warp
+
 template <int MT>      // projector tiles of 8 (npjp <= 8 MT)
 __global__ void __launch_bounds__(256) proj_gather_kernel(const __grid_constant__ GatherParams A) {
     const int wl = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int kk = wl & 3, rw = wl >> 2;
     const int spin = warp & 1;
-    const int v0 = blockIdx.y * 32 + (warp >> 1) * 8;
+    const int v0 = blockIdx.y * (16 * kGatherNT) + (warp >> 1) * (4 * kGatherNT);
     if (v0 >= A.nvec) return;
     const int atom = A.gb_atom[blockIdx.x];
     const int e0 = A.gb_beg[blockIdx.x], e1 = A.gb_end[blockIdx.x];
     const int npj = A.atom_npj[atom];
-    double acc[MT][2][2];
+    double acc[MT][kGatherNT][2];
 #pragma unroll
     for (int m = 0; m < MT; ++m)
 #pragma unroll
-        for (int nt = 0; nt < 2; ++nt) { acc[m][nt][0] = 0.0; acc[m][nt][1] = 0.0; }
-    const int bv[2] = { v0 + (rw >> 1), v0 + 4 + (rw >> 1) };
-    const double* sb = A.src + ((long long)spin * A.ld) * 2 + (rw & 1);
-    auto load_step = [&](int e, double (&a)[MT], double (&b)[2]) {
+        for (int nt = 0; nt < kGatherNT; ++nt) { acc[m][nt][0] = 0.0; acc[m][nt][1] = 0.0; }
+    const double* sb = A.src + ((long long)spin * A.ld + v0 + (rw >> 1)) * 2 + (rw & 1);
+    const double* gp = A.g_pack + (long long)A.gb_k0[blockIdx.x] * (MT * 32) + wl;
+    auto load_step = [&](int e, int ks, double (&a)[MT], double (&b)[kGatherNT]) {
         const int er = e + kk;
         const bool ok = er < e1;
         const int node = __ldg(A.ent_node + (ok ? er : e0));
-        const double* ap = A.ent_p + (long long)(ok ? er : e0) * A.npjp + rw;
 #pragma unroll
-        for (int m = 0; m < MT; ++m) a[m] = (ok && m * 8 + rw < A.npjp) ? __ldg(ap + m * 8) : 0.0;
+        for (int m = 0; m < MT; ++m) a[m] = (e < e1) ? __ldg(gp + ((long long)ks * MT + m) * 32) : 0.0;
         const double* xp = sb + (long long)node * A.ld * 4;
 #pragma unroll
-        for (int nt = 0; nt < 2; ++nt) b[nt] = (ok && bv[nt] < A.nvec) ? __ldg(xp + (long long)bv[nt] * 2) : 0.0;
+        for (int nt = 0; nt < kGatherNT; ++nt) b[nt] = (ok && v0 + nt * 4 + (rw >> 1) < A.nvec) ? __ldg(xp + nt * 8) : 0.0;
     };
-    for (int e = e0; e < e1; e += 8) {
-        double a0[MT], b0[2], a1[MT], b1[2];
-        load_step(e, a0, b0);
-        load_step(e + 4, a1, b1);
+    // two k-steps are multiplied while the next two are in flight
+    double a0[MT], b0[kGatherNT], a1[MT], b1[kGatherNT];
+    load_step(e0, 0, a0, b0);
+    load_step(e0 + 4, 1, a1, b1);
+    int ks = 0;
+    for (int e = e0; e < e1; e += 8, ks += 2) {
+        double a2[MT], b2[kGatherNT], a3[MT], b3[kGatherNT];
+        load_step(e + 8, ks + 2, a2, b2);
+        load_step(e + 12, ks + 3, a3, b3);
 #pragma unroll
         for (int m = 0; m < MT; ++m)
 #pragma unroll
-            for (int nt = 0; nt < 2; ++nt) gather_dmma(acc[m][nt][0], acc[m][nt][1], a0[m], b0[nt]);
+            for (int nt = 0; nt < kGatherNT; ++nt) gather_dmma(acc[m][nt][0], acc[m][nt][1], a0[m], b0[nt]);
 #pragma unroll
         for (int m = 0; m < MT; ++m)
 #pragma unroll
-            for (int nt = 0; nt < 2; ++nt) gather_dmma(acc[m][nt][0], acc[m][nt][1], a1[m], b1[nt]);
+            for (int nt = 0; nt < kGatherNT; ++nt) gather_dmma(acc[m][nt][0], acc[m][nt][1], a1[m], b1[nt]);
+#pragma unroll
+        for (int m = 0; m < MT; ++m) { a0[m] = a2[m]; a1[m] = a3[m]; }
+#pragma unroll
+        for (int nt = 0; nt < kGatherNT; ++nt) { b0[nt] = b2[nt]; b1[nt] = b3[nt]; }
     }
     const long long coff = A.atom_coff[atom];
 #pragma unroll
@@ -88,7 +99,7 @@ __global__ void __launch_bounds__(256) proj_gather_kernel(const __grid_constant_
         const int chi = m * 8 + rw;
         if (chi < npj) {
 #pragma unroll
-            for (int nt = 0; nt < 2; ++nt) {
+            for (int nt = 0; nt < kGatherNT; ++nt) {
                 const int v = v0 + nt * 4 + kk;
                 if (v < A.nvec) {
                     double* cp = A.C + ((coff + 2 * chi + spin) * A.ldc + v) * 2;
