@@ -115,11 +115,12 @@ class ClockSampler:
         return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "power_w_max": float(max(pw)), "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def build_system(cfg, ctx):
+def build_system(cfg, ctx, with_projectors=True):
     """Seeded synthetic operator inputs for `cfg` on node coordinates / masses exported by `ctx` (either side)."""
-    sysm = synth.make_system(cfg, ctx.node_coords(), ctx.mass_diag())
+    sysm = synth.make_system(cfg, ctx.node_coords(), ctx.mass_diag(), with_projectors=with_projectors)
     ctx.set_potential(sysm.veff, sysm.bxyz)
-    ctx.set_projectors(sysm.node_ptr, sysm.node_idx, sysm.nproj, sysm.pvals, sysm.atom_type, sysm.delta, sysm.delta_ptr)
+    if with_projectors:
+        ctx.set_projectors(sysm.node_ptr, sysm.node_idx, sysm.nproj, sysm.pvals, sysm.atom_type, sysm.delta, sysm.delta_ptr)
     return sysm
 
 
@@ -200,7 +201,7 @@ def main_ours(args):
     if args.variant:
         ctx.set_variant(args.variant)
     t_setup = time.perf_counter()
-    sysm = build_system(cfg, ctx)
+    sysm = build_system(cfg, ctx, with_projectors=not args.no_projectors)
     M = ctx.M; rows = 2 * M
     wb = ctx.workspace_bytes(nvec)
     work = torch.empty(max(wb, 16), dtype=torch.uint8, device="cuda")
@@ -356,6 +357,7 @@ def main():
     ap.add_argument("--variant", type=int, default=0)
     ap.add_argument("--host-chunk", type=int, default=64)
     ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--no-projectors", action="store_true", help="local part only (diagnostic, not a bench value)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-profile", action="store_true")

@@ -3,7 +3,7 @@
 //
 // Paper steps fused here: a1 extraction X^(e) = R^(e) X with the M_D^{-1/2} scaling folded into the
 // 1-D operators, a2 cell-level product with the sum-factorised 1/2 K^(e), a3 nodal 2x2 spin potential, a7 projector
-// expansion P^a C~^a (FP64 tensor-core tiles, mma.sync m8n8k4 = DMMA), a4 assembly (RED.F64 scatter-add),
+// expansion P^a C~^a (FP64 tensor-core tiles, mma.sync m8n8k4 = DMMA; inputs staged by TMA), a4 assembly (RED.F64),
 // a8 recurrence update (accumulate form, csf_kernels.cuh).
 //
 // Why a column and not a cell: the L2 <-> SM fabric of B200 is barely faster than HBM, so the (n/p)^3 re-read /
@@ -22,13 +22,18 @@
 // Warp roles. Main threads = (q, lane): L lanes = (spin, vector, re/im) are independent real streams of the same
 // operator (the tables are real); q indexes a plane.
 //   phase A  thread holds the x-y plane u[j][i] of one new z-plane in registers:
-//              a2 = By Ah u + rho_y Ah Bx u,  b2 = rho_z By Bx u  -> ring;
-//              E = (V + B.sigma - c) u on the nodes the plane owns -> E ring (spin partner by shuffle)
-//   phase B  thread j takes the z-lines (j, i): out = ax (Bz a2 + Ah b2) (+ E + X on owned nodes, + carry on k = 0),
+//              a2 = By Ah u + rho_y Ah Bx u,  b2 = rho_z By Bx u  -> ring
+//   phase B  thread j takes the z-lines (j, i): out = ax (Bz a2 + Ah b2) (+ X on owned nodes, + carry on k = 0),
 //              RED.F64 into dst for k < p, out[p] becomes the carry.
-// Two auxiliary warps run beside phase A: X = sum_a P~^a C~^a per (cell, atom) pair as DMMA tiles (8 support rows
-// x 8 lanes x 4 projectors each; the tensor pipe works while the FP64 pipe does phase A), and they stage the nodal
-// potential of the next cell into shared memory.
+// Two auxiliary warps build X, the nodal and nonlocal terms on the owned nodes of the cell, beside phase A:
+//   - one thread issues two TMA loads (cp.async.bulk.tensor + mbarrier): the src rows of the owned nodes (both spins,
+//     this CTA's vectors) land in X, their V, Bx, By, Bz in a small stage; Dirichlet faces and vectors >= nvec are
+//     zero-filled by the out-of-bounds rule;
+//   - X = (V + B.sigma - c) X in place, thread = (node, vector) with both spins in registers;
+//   - X += sum_a P~^a C~^a per (cell, atom) sub-pair as DMMA tiles (8 support rows x 8 lanes x 4 projectors); both
+//     operands are stored in fragment order, so each fragment is one coalesced 256-byte load. Each warp owns one half
+//     of the rows. The tensor pipe works while the FP64 pipe does phase A.
+// Main and auxiliary warps meet at two named barriers ("X full" / "X free", bar.arrive + bar.sync).
 #pragma once
 #include <cuda.h>
 #include <cuda_runtime.h>
@@ -80,8 +85,8 @@ __device__ __forceinline__ void col_dmma(double& d0, double& d1, double a, doubl
     asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
 }
 
-// named barriers: 1 = main threads only; 2 + b = "X buffer b is full" (expansion warps arrive, main threads wait);
-// 4 + b = "X buffer b is free" (main threads arrive, expansion warps wait)
+// named barriers: 1 = main threads only; 2 = "X is full" (expansion warps arrive, main threads wait);
+// 3 = "X is free" (main threads arrive, expansion warps wait)
 __device__ __forceinline__ void col_bar_sync(int id, int count) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(count) : "memory"); }
 __device__ __forceinline__ void col_bar_arrive(int id, int count) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(count) : "memory"); }
 
