@@ -458,18 +458,21 @@ int csf_set_projectors(csf_ctx* c, int natoms, const int64_t* node_ptr, const in
     }
     // sub-pairs for the column kernel: every (cell, atom) pair split at the owned-node index XSPLIT = ceil(p^3 / 2)
     // (entries of a pair are sorted by that index), grouped by (cell, half)
-    const int xsplit = (p * p * p + 1) / 2;
+    const int nq = kColAuxWarps, xsplit = (p * p * p + nq - 1) / nq;
     struct Sub { int key; int4 d; };
-    std::vector<Sub> subs; subs.reserve(2 * pairs.size());
+    std::vector<Sub> subs; subs.reserve(nq * pairs.size());
     if (crows >= (1LL << 31)) return fail(c, CSF_EUNSUPPORTED, "too many projector rows");
     for (const Pair& pr : pairs) {
-        const int e0 = pr.off[0], e1 = pr.off[p];
-        int em = e0; while (em < e1 && ent_locf[em] < xsplit) ++em;
-        if (em > e0) subs.push_back({pr.cell * 2, make_int4(pr.atom, 0, e0, em)});
-        if (e1 > em) subs.push_back({pr.cell * 2 + 1, make_int4(pr.atom, 0, em, e1)});
+        const int e1 = pr.off[p];
+        int e = pr.off[0];
+        for (int r = 0; r < nq; ++r) {
+            int em = e; while (em < e1 && ent_locf[em] < (r + 1) * xsplit) ++em;
+            if (em > e) subs.push_back({pr.cell * nq + r, make_int4(pr.atom, 0, e, em)});
+            e = em;
+        }
     }
     std::stable_sort(subs.begin(), subs.end(), [](const Sub& x, const Sub& y) { return x.key < y.key; });
-    std::vector<int> sub_ptr(2 * (size_t)c->E + 1, 0); std::vector<int4> sub_desc(subs.size());
+    std::vector<int> sub_ptr(nq * (size_t)c->E + 1, 0); std::vector<int4> sub_desc(subs.size());
     long long ntiles = 0;
     for (size_t q = 0; q < subs.size(); ++q) {
         sub_ptr[subs[q].key + 1]++;
@@ -477,7 +480,7 @@ int csf_set_projectors(csf_ctx* c, int natoms, const int64_t* node_ptr, const in
         sub_desc[q] = subs[q].d;
     }
     if (ntiles >= (1LL << 31)) return fail(c, CSF_EUNSUPPORTED, "too many projector tiles");
-    for (size_t q = 0; q < 2 * (size_t)c->E; ++q) sub_ptr[q + 1] += sub_ptr[q];
+    for (size_t q = 0; q < nq * (size_t)c->E; ++q) sub_ptr[q + 1] += sub_ptr[q];
     // P~ of every tile (8 rows of a sub-pair) in the order of the DMMA A fragment: [tile][k-step][lane = row*4 + k]
     const int ks = npjp / 4;
     std::vector<double> a_pack((size_t)ntiles * ks * 32, 0.0);

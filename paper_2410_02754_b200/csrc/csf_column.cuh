@@ -42,7 +42,11 @@
 namespace csf {
 
 constexpr int kColTab = 8;
-constexpr int kColAux = 64;      // auxiliary threads (2 warps)
+#ifndef CSF_AUX_WARPS
+#define CSF_AUX_WARPS 2
+#endif
+constexpr int kColAuxWarps = CSF_AUX_WARPS;   // expansion warps per CTA; each owns an equal share of the owned-node rows of X
+constexpr int kColAux = 32 * kColAuxWarps;
 
 struct ColParams {
     // TMA descriptors (cuTensorMapEncodeTiled): src viewed as [nfz][nfy][2 nfx rows][2 nvec doubles], box = the owned
@@ -85,8 +89,8 @@ __device__ __forceinline__ void col_dmma(double& d0, double& d1, double a, doubl
     asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
 }
 
-// named barriers: 1 = main threads only; 2 = "X is full" (expansion warps arrive, main threads wait);
-// 3 = "X is free" (main threads arrive, expansion warps wait)
+// named barriers: 1 = main threads only; 2 + b = "X buffer b is full" (expansion warps arrive, main threads wait);
+// 4 + b = "X buffer b is free" (main threads arrive, expansion warps wait)
 __device__ __forceinline__ void col_bar_sync(int id, int count) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(count) : "memory"); }
 __device__ __forceinline__ void col_bar_arrive(int id, int count) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(count) : "memory"); }
 
@@ -108,24 +112,26 @@ template <int P, int L> struct ColCfg {
     static constexpr int VCELL = P * P * P * 4;                      // V, Bx, By, Bz of the owned nodes of one cell
     // a2 ring, b2 ring, X (nodal + nonlocal terms on the owned nodes of the current cell), staged potential, mbarrier
     static constexpr size_t XOFF = ((size_t)2 * N * PLANE * sizeof(double) + 127) / 128 * 128;
-    static constexpr size_t VOFF = (XOFF + (size_t)P * EPLANE * sizeof(double) + 127) / 128 * 128;
-    static constexpr size_t MOFF = (VOFF + (size_t)VCELL * sizeof(double) + 15) / 16 * 16;
-    static constexpr size_t SMEM = MOFF + 16;
+    static constexpr size_t XBYTES = ((size_t)P * EPLANE * sizeof(double) + 127) / 128 * 128;     // one X buffer
+    static constexpr size_t VBYTES = ((size_t)VCELL * sizeof(double) + 127) / 128 * 128;          // one potential stage
+    static constexpr size_t VOFF = XOFF + 2 * XBYTES;          // X and the stage are double-buffered (cell t uses t & 1)
+    static constexpr size_t MOFF = VOFF + 2 * VBYTES;
+    static constexpr size_t SMEM = MOFF + 32;
 };
 
 // FAST: every node of the mesh is unconstrained (all directions periodic), nvec is a multiple of L/4 and the cells
 // are cubes (rho_y = rho_z = 1), so no load, store or RED needs a predicate and no rho multiply is issued.
 template <int P, int KS, bool FAST, int L>
-__global__ void __launch_bounds__(ColCfg<P, L>::NT) __maxnreg__((P >= 4 && P <= 5) ? 136 : 255) column_kernel(const __grid_constant__ ColParams A) {
+__global__ void __launch_bounds__(ColCfg<P, L>::NT) __maxnreg__((P >= 4 && P <= 5) ? (kColAuxWarps == 2 ? 136 : 144) : 255) column_kernel(const __grid_constant__ ColParams A) {
     using Cfg = ColCfg<P, L>;
     constexpr int N = Cfg::N, NTM = Cfg::NTM, VPC = L / 4;        // VPC vectors per CTA
     constexpr int PLANE = Cfg::PLANE, EPLANE = Cfg::EPLANE;
     extern __shared__ __align__(128) double smem[];
     double* R1 = smem;
     double* R2 = R1 + N * PLANE;
-    double* X = reinterpret_cast<double*>(reinterpret_cast<char*>(smem) + Cfg::XOFF);
-    double* VS = reinterpret_cast<double*>(reinterpret_cast<char*>(smem) + Cfg::VOFF);
-    const unsigned mbar = (unsigned)__cvta_generic_to_shared(reinterpret_cast<char*>(smem) + Cfg::MOFF);
+    char* const xbase = reinterpret_cast<char*>(smem) + Cfg::XOFF;
+    char* const vbase = reinterpret_cast<char*>(smem) + Cfg::VOFF;
+    const unsigned mbar0 = (unsigned)__cvta_generic_to_shared(reinterpret_cast<char*>(smem) + Cfg::MOFF);
 
 #define AH(i, j) ((&A.Ah[0][0])[col_canon<N>(i, j)])
 #define UH(i) (((P & 1) && (i) > N - 1 - (i)) ? -A.uh[N - 1 - (i)] : A.uh[(i) < N - 1 - (i) ? (i) : N - 1 - (i)])
@@ -146,7 +152,8 @@ __global__ void __launch_bounds__(ColCfg<P, L>::NT) __maxnreg__((P >= 4 && P <= 
     const int plane_nodes = A.nfx * A.nfy;
 
     if (tid == 0) {
-        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(mbar));
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(mbar0));
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(mbar0 + 8));
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
@@ -159,7 +166,7 @@ __global__ void __launch_bounds__(ColCfg<P, L>::NT) __maxnreg__((P >= 4 && P <= 
         // same row and need no barrier between them. Its sub-pairs (cell, atom, range) come from the host.
         const int aw = warp_id - NTM / 32, wl = tid & 31;
         const int kk = wl & 3, rw = wl >> 2;
-        constexpr int XSPLIT = (P * P * P + 1) / 2, TMAX = (XSPLIT + 7) / 8, TCH = TMAX < 5 ? TMAX : 5;
+        constexpr int XSPLIT = (P * P * P + kColAuxWarps - 1) / kColAuxWarps, TMAX = (XSPLIT + 7) / 8, TCH = TMAX < 5 ? TMAX : 5;
         const int xr0 = aw * XSPLIT, xr1 = min(P * P * P, xr0 + XSPLIT);
         auto load_b = [&](const int4& ds, double (&bb)[KS][L / 8]) {
             const double* cb = A.Ct + ((long long)ds.x * A.nchunks + chunk) * (KS * (L / 8) * 32) + wl;
@@ -169,7 +176,10 @@ __global__ void __launch_bounds__(ColCfg<P, L>::NT) __maxnreg__((P >= 4 && P <= 
                 for (int nt = 0; nt < L / 8; ++nt) bb[s][nt] = __ldg(cb + (s * (L / 8) + nt) * 32);
         };
         for (int t = 0; t < S; ++t) {
-            if (t >= 1) col_bar_sync(3, Cfg::NT);                // phase B(t - 1) has consumed X
+            double* X = reinterpret_cast<double*>(xbase + (t & 1) * Cfg::XBYTES);
+            double* VS = reinterpret_cast<double*>(vbase + (t & 1) * Cfg::VBYTES);
+            const unsigned mbar = mbar0 + 8 * (t & 1);
+            if (t >= 2) col_bar_sync(4 + (t & 1), Cfg::NT);      // phase B(t - 2) has consumed this X buffer
             // TMA: the owned nodes of cell t (src rows of both spins, this CTA's vectors) land in X, their nodal
             // potential in VS; nodes outside the mesh (Dirichlet faces) and vectors >= nvec are zero-filled
             if (aw == 0 && wl == 0) {
@@ -184,7 +194,7 @@ __global__ void __launch_bounds__(ColCfg<P, L>::NT) __maxnreg__((P >= 4 && P <= 
             {
                 unsigned done = 0;
                 while (!done)
-                    asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }" : "=r"(done) : "r"(mbar), "r"((unsigned)(t & 1)) : "memory");
+                    asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }" : "=r"(done) : "r"(mbar), "r"((unsigned)((t >> 1) & 1)) : "memory");
             }
             // X = (V + B.sigma - c) X in place on this warp's rows: thread = (node, vector), both spins and re/im in
             // registers, so the 2x2 spin block needs no exchange between threads
@@ -204,7 +214,7 @@ __global__ void __launch_bounds__(ColCfg<P, L>::NT) __maxnreg__((P >= 4 && P <= 
             __syncwarp();
             if (A.sub_ptr != nullptr) {
                 const int cell = cx + A.ncx * (cy + A.ncy * (cz0 + t));
-                const int sp0 = A.sub_ptr[cell * 2 + aw], sp1 = A.sub_ptr[cell * 2 + aw + 1];
+                const int sp0 = A.sub_ptr[cell * kColAuxWarps + aw], sp1 = A.sub_ptr[cell * kColAuxWarps + aw + 1];
                 int4 ds = make_int4(0, 0, 0, 0);       // {first row of the atom in C~, n_pj, entry begin, entry end}
                 double b[KS][L / 8];
                 if (sp0 < sp1) { ds = __ldg(A.sub_desc + sp0); load_b(ds, b); }
@@ -253,7 +263,7 @@ __global__ void __launch_bounds__(ColCfg<P, L>::NT) __maxnreg__((P >= 4 && P <= 
                 }
             }
             __threadfence_block();
-            col_bar_arrive(2, Cfg::NT);                          // X(t) is complete
+            col_bar_arrive(2 + (t & 1), Cfg::NT);                // X(t) is complete
         }
         return;
     }
@@ -362,7 +372,8 @@ __global__ void __launch_bounds__(ColCfg<P, L>::NT) __maxnreg__((P >= 4 && P <= 
         }
         if (t + 1 < S) load_plane(plane_of(t + 1));          // in flight during phase B
         col_bar_sync(1, NTM);                                 // ring written
-        col_bar_sync(2, Cfg::NT);                             // X(t) complete
+        col_bar_sync(2 + (t & 1), Cfg::NT);                   // X(t) complete
+        const double* X = reinterpret_cast<const double*>(xbase + (t & 1) * Cfg::XBYTES);
         // ------------------------------------------------------------------ phase B
         if (q_on) {
             const int j = q;
@@ -412,7 +423,7 @@ __global__ void __launch_bounds__(ColCfg<P, L>::NT) __maxnreg__((P >= 4 && P <= 
                 if (t == S - 1 && (FAST || (xy_ok && zn[P] >= 0))) atomicAdd(dp + (long long)(xy + zn[P]) * A.rd, col_flip(scax * carry[i], sgn));
             }
         }
-        if (t + 1 < S) col_bar_arrive(3, Cfg::NT);            // X is free
+        if (t + 2 < S) col_bar_arrive(4 + (t & 1), Cfg::NT);  // this X buffer is free
         col_bar_sync(1, NTM);                                 // ring free
     }
 #undef AH
