@@ -160,11 +160,13 @@ __global__ void __launch_bounds__(ColCfg<P, L>::NT) __maxnreg__((P >= 4 && P <= 
 
     // warp-uniform role (broadcast from lane 0 so that the compiler knows the branch does not split a warp)
     const int warp_id = __shfl_sync(0xffffffffu, tid >> 5, 0);
-    if (warp_id >= NTM / 32) {
+    // the expansion warps take the LOW warp ids: the scheduler favours high warp ids, and the main warps carry the
+    // FP64 work, while the expansion warps mostly wait
+    if (warp_id < kColAuxWarps) {
         // ============================================================== auxiliary warps
         // Warp aw owns the owned-node range [aw * XSPLIT, (aw + 1) * XSPLIT) of X, so the two warps never touch the
         // same row and need no barrier between them. Its sub-pairs (cell, atom, range) come from the host.
-        const int aw = warp_id - NTM / 32, wl = tid & 31;
+        const int aw = warp_id, wl = tid & 31;
         const int kk = wl & 3, rw = wl >> 2;
         constexpr int XSPLIT = (P * P * P + kColAuxWarps - 1) / kColAuxWarps, TMAX = (XSPLIT + 7) / 8, TCH = TMAX < 5 ? TMAX : 5;
         const int xr0 = aw * XSPLIT, xr1 = min(P * P * P, xr0 + XSPLIT);
@@ -269,7 +271,8 @@ __global__ void __launch_bounds__(ColCfg<P, L>::NT) __maxnreg__((P >= 4 && P <= 
     }
 
     // ================================================================== main warps
-    const int lane = tid % L, q = tid / L;
+    const int mtid = tid - kColAux;
+    const int lane = mtid % L, q = mtid / L;
     const int spin = lane / (L / 2), ri = lane & 1;
     const int vec = chunk * VPC + ((lane % (L / 2)) >> 1);
     const bool lane_on = FAST || vec < A.nvec;
