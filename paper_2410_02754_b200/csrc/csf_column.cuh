@@ -181,6 +181,15 @@ __global__ void __launch_bounds__(ColCfg<P, L>::NT) __maxnreg__((P >= 4 && P <= 
             double* X = reinterpret_cast<double*>(xbase + (t & 1) * Cfg::XBYTES);
             double* VS = reinterpret_cast<double*>(vbase + (t & 1) * Cfg::VBYTES);
             const unsigned mbar = mbar0 + 8 * (t & 1);
+            // the first sub-pair's descriptor and C~ fragments do not depend on X: fetch them before any waiting
+            int sp0 = 0, sp1 = 0;
+            int4 ds = make_int4(0, 0, 0, 0);           // {atom, first tile in a_pack, entry begin, entry end}
+            double b[KS][L / 8];
+            if (A.sub_ptr != nullptr) {
+                const int cell = cx + A.ncx * (cy + A.ncy * (cz0 + t));
+                sp0 = A.sub_ptr[cell * kColAuxWarps + aw]; sp1 = A.sub_ptr[cell * kColAuxWarps + aw + 1];
+                if (sp0 < sp1) { ds = __ldg(A.sub_desc + sp0); load_b(ds, b); }
+            }
             if (t >= 2) col_bar_sync(4 + (t & 1), Cfg::NT);      // phase B(t - 2) has consumed this X buffer
             // TMA: the owned nodes of cell t (src rows of both spins, this CTA's vectors) land in X, their nodal
             // potential in VS; nodes outside the mesh (Dirichlet faces) and vectors >= nvec are zero-filled
@@ -214,12 +223,7 @@ __global__ void __launch_bounds__(ColCfg<P, L>::NT) __maxnreg__((P >= 4 && P <= 
                 xu[0] = ou; xu[L / 4] = od;
             }
             __syncwarp();
-            if (A.sub_ptr != nullptr) {
-                const int cell = cx + A.ncx * (cy + A.ncy * (cz0 + t));
-                const int sp0 = A.sub_ptr[cell * kColAuxWarps + aw], sp1 = A.sub_ptr[cell * kColAuxWarps + aw + 1];
-                int4 ds = make_int4(0, 0, 0, 0);       // {first row of the atom in C~, n_pj, entry begin, entry end}
-                double b[KS][L / 8];
-                if (sp0 < sp1) { ds = __ldg(A.sub_desc + sp0); load_b(ds, b); }
+            {
                 for (int sp = sp0; sp < sp1; ++sp) {
                     // A fragments of up to TCH tiles at once (one exposed round trip), next sub-pair's B meanwhile
                     const int e0 = ds.z, e1 = ds.w;
