@@ -159,3 +159,23 @@ def test_error_codes():
         g.filter(X, Y, 4, 4, 2, 0.0, 1.0, 0, w[:64])
     assert ei.value.code == binding.CSF_EINVAL
     g.filter(X, Y, 4, 0, 2, 0.0, 1.0, 0, w)     # nvec = 0 is a no-op
+
+
+@pytest.mark.parametrize("chunk,nvec,ld", [(8, 20, 24), (64, 16, 16), (5, 5, 5), (4, 9, 9)])
+def test_filter_host_pipeline_matches_oracle(chunk, nvec, ld, cfg0_oracle):
+    """The end-to-end entry point: host buffers staged in column chunks (H2D / filter / D2H on three streams)."""
+    import torch
+    ref, a, b = (cfg0_oracle[k] for k in ("ctx", "a", "b"))
+    _, gpu, s = setup_pair(synth.CONFIGS[0])
+    gpu.set_host_chunk(chunk)
+    X = synth.random_block(s.rng, 2 * ref.M, nvec)
+    hX = torch.zeros((2 * ref.M, ld), dtype=torch.complex128).pin_memory(); hX[:, :nvec] = torch.from_numpy(X)
+    hY = torch.full((2 * ref.M, ld), 7.0 + 3.0j, dtype=torch.complex128).pin_memory()
+    gpu.filter_host(hX, hY, ld, nvec, 8, a, b)
+    out = hY.numpy()
+    assert rel_fro(out[:, :nvec], ref.filter(X, 8, a, b)) < TOL
+    if ld > nvec:
+        assert np.all(out[:, nvec:] == 7.0 + 3.0j), "padding columns were touched"
+    Yn = np.zeros((2 * ref.M, ld), dtype=np.complex128)      # pageable NumPy buffers work too
+    gpu.filter_host(np.ascontiguousarray(hX.numpy()), Yn, ld, nvec, 8, a, b)
+    assert rel_fro(Yn[:, :nvec], out[:, :nvec]) < 1e-13
