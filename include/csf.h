@@ -112,7 +112,8 @@ int csf_apply_H(csf_ctx* ctx, const csf_c128* dX, csf_c128* dY, int64_t ld, int 
 
 /* Y = T_degree((Hhat - c)/e) X with c = (a+b)/2, e = (b-a)/2 (eq.70). degree = 0 copies X to Y.
  * Same pointer rules as csf_apply_H; X is not modified. mode: CSF_FP64, or CSF_FP32_INTERMEDIATE (complex128
- * in and out, fp32 recurrence buffers and cell arithmetic in between; CSF_EUNSUPPORTED until built).
+ * in and out; both recurrence buffers complex64 and the cell-level arithmetic FP32 in between, projector coefficients
+ * kept in FP64; agrees with the FP64 result to about 1e-5 relative).
  * Errors: CSF_EINVAL also for degree < 0 or a >= b. Enqueues only. */
 int csf_filter(csf_ctx* ctx, const csf_c128* dX, csf_c128* dY, int64_t ld, int nvec,
                int degree, double a, double b, int mode, void* d_work, size_t work_bytes);

@@ -88,15 +88,15 @@ struct ProfScope {
     ~ProfScope() { if (e1) { cudaEventRecord(e1, c->stream); c->prof_ev[kind].push_back({e0, e1}); } }
 };
 
-cudaError_t launch_column(int p, int ks, bool fast, const ColParams& cp, long long nblocks, cudaStream_t s) {
+cudaError_t launch_column(int p, int ks, bool fast, bool f32, const ColParams& cp, long long nblocks, cudaStream_t s) {
     switch (p) {
-        case 1: return launch_column_p1(ks, fast, cp, nblocks, s);
-        case 2: return launch_column_p2(ks, fast, cp, nblocks, s);
-        case 3: return launch_column_p3(ks, fast, cp, nblocks, s);
-        case 4: return launch_column_p4(ks, fast, cp, nblocks, s);
-        case 5: return launch_column_p5(ks, fast, cp, nblocks, s);
-        case 6: return launch_column_p6(ks, fast, cp, nblocks, s);
-        case 7: return launch_column_p7(ks, fast, cp, nblocks, s);
+        case 1: return launch_column_p1(ks, fast, f32, cp, nblocks, s);
+        case 2: return launch_column_p2(ks, fast, f32, cp, nblocks, s);
+        case 3: return launch_column_p3(ks, fast, f32, cp, nblocks, s);
+        case 4: return launch_column_p4(ks, fast, f32, cp, nblocks, s);
+        case 5: return launch_column_p5(ks, fast, f32, cp, nblocks, s);
+        case 6: return launch_column_p6(ks, fast, f32, cp, nblocks, s);
+        case 7: return launch_column_p7(ks, fast, f32, cp, nblocks, s);
     }
     return cudaErrorInvalidValue;
 }
@@ -123,19 +123,21 @@ EncodeTiledFn encode_tiled_fn() {
 }
 
 // FP64 tensor map of rank `rank`: dims / box in elements (innermost first), strides in bytes for dims 1..rank-1
-bool encode_map(CUtensorMap* tm, const void* base, int rank, const cuuint64_t* dims, const cuuint64_t* strides, const cuuint32_t* box) {
+bool encode_map(CUtensorMap* tm, const void* base, int rank, const cuuint64_t* dims, const cuuint64_t* strides, const cuuint32_t* box, bool f32 = false) {
     EncodeTiledFn fn = encode_tiled_fn();
     if (!fn) return false;
     cuuint32_t es[5] = {1, 1, 1, 1, 1};
-    return fn(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, (cuuint32_t)rank, const_cast<void*>(base), dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+    return fn(tm, f32 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT64, (cuuint32_t)rank, const_cast<void*>(base), dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
               CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
 size_t ctp_bytes(const csf_ctx* c, int nvec);
+size_t f32_block_bytes(const csf_ctx* c, int nvec);
 
 // one step: dst += sc * i^rot * (Hhat - shift) src
-int enqueue_step(csf_ctx* c, const double* src, long long ld, double* dst, long long ld_dst, int nvec, double sc, int rot, double shift,
-                 double* dC, double* dCt) {
+// src, dst: complex128 blocks, or complex64 blocks when f32 (CSF_FP32_INTERMEDIATE)
+int enqueue_step(csf_ctx* c, const void* src, long long ld, void* dst, long long ld_dst, int nvec, double sc, int rot, double shift,
+                 double* dC, double* dCt, bool f32 = false) {
     const long long ldc = nvec;
     if (c->natoms > 0) {
         CSF_CUDA(c, cudaMemsetAsync(dC, 0, (size_t)c->crows * ldc * sizeof(double2), c->stream));
@@ -148,8 +150,8 @@ int enqueue_step(csf_ctx* c, const double* src, long long ld, double* dst, long 
         dim3 gg(c->n_gather_blocks, (nvec + 16 * kGatherNT - 1) / (16 * kGatherNT));
         {
             ProfScope ps(c, CSF_KIND_PGATHER);
-            if (c->npjp <= 24) proj_gather_kernel<3><<<gg, 256, 0, c->stream>>>(gp);
-            else proj_gather_kernel<4><<<gg, 256, 0, c->stream>>>(gp);
+            if (c->npjp <= 24) { if (f32) proj_gather_kernel<3, float><<<gg, 256, 0, c->stream>>>(gp); else proj_gather_kernel<3, double><<<gg, 256, 0, c->stream>>>(gp); }
+            else { if (f32) proj_gather_kernel<4, float><<<gg, 256, 0, c->stream>>>(gp); else proj_gather_kernel<4, double><<<gg, 256, 0, c->stream>>>(gp); }
         }
         CSF_CUDA(c, cudaGetLastError());
         DeltaParams dp{};
@@ -173,21 +175,23 @@ int enqueue_step(csf_ctx* c, const double* src, long long ld, double* dst, long 
         const int n = c->n;
         const double hx2 = c->h[0] * c->h[0];
         for (int i = 0; i < n; ++i) {
-            for (int j = 0; j < n; ++j) q.Ah[i][j] = c->dir[0].A[i][j] * (0.5 * hx2);
-            q.uh[i] = c->dir[0].u[i];
+            for (int j = 0; j < n; ++j) { q.Ah[i][j] = c->dir[0].A[i][j] * (0.5 * hx2); q.Ahf[i][j] = (float)q.Ah[i][j]; }
+            q.uh[i] = c->dir[0].u[i]; q.uhf[i] = (float)q.uh[i];
         }
         q.ax = 2.0 / hx2; q.rho_y = hx2 / (c->h[1] * c->h[1]); q.rho_z = hx2 / (c->h[2] * c->h[2]);
         q.src = src; q.dst = dst; q.rs = (int)(4 * ld); q.rd = (int)(4 * ld_dst); q.nvec = nvec;
         {
             const cuuint64_t nfx = c->nfree[0], nfy = c->nfree[1], nfz = c->nfree[2], p = c->p;
             const cuuint64_t sd[4] = {(cuuint64_t)2 * nvec, 2 * nfx, nfy, nfz};
-            const cuuint64_t ss[3] = {(cuuint64_t)ld * 16, 2 * nfx * (cuuint64_t)ld * 16, nfy * 2 * nfx * (cuuint64_t)ld * 16};
+            const cuuint64_t rb = (cuuint64_t)ld * (f32 ? 8 : 16);        // bytes per spinor row
+            if (rb % 16 != 0) return fail(c, CSF_EINVAL, "leading dimension of a complex64 block must be even");
+            const cuuint64_t ss[3] = {rb, 2 * nfx * rb, nfy * 2 * nfx * rb};
             const cuuint32_t sb[4] = {(cuuint32_t)(ci.lanes / 2), (cuuint32_t)(2 * p), (cuuint32_t)p, (cuuint32_t)p};
             const cuuint64_t vd[3] = {4 * nfx, nfy, nfz};
             const cuuint64_t vs[2] = {nfx * 32, nfy * nfx * 32};
             const cuuint32_t vbx[3] = {(cuuint32_t)(4 * p), (cuuint32_t)p, (cuuint32_t)p};
             if (((uintptr_t)src & 15) != 0) return fail(c, CSF_EINVAL, "block pointer must be 16-byte aligned");
-            if (!encode_map(&q.tm_src, src, 4, sd, ss, sb) || !encode_map(&q.tm_vb, c->d_vb.p, 3, vd, vs, vbx))
+            if (!encode_map(&q.tm_src, src, 4, sd, ss, sb, f32) || !encode_map(&q.tm_vb, c->d_vb.p, 3, vd, vs, vbx))
                 return fail(c, CSF_ECUDA, "cuTensorMapEncodeTiled failed");
         }
         q.ncx = c->ncell[0]; q.ncy = c->ncell[1]; q.ncz = c->ncell[2];
@@ -209,13 +213,14 @@ int enqueue_step(csf_ctx* c, const double* src, long long ld, double* dst, long 
             ProfScope ps(c, CSF_KIND_CELL);
             const bool fast = c->bc[0] == CSF_BC_PERIODIC && c->bc[1] == CSF_BC_PERIODIC && c->bc[2] == CSF_BC_PERIODIC && nvec % vpc == 0 &&
                               q.rho_y == 1.0 && q.rho_z == 1.0 && c->variant != 1;
-            CSF_CUDA(c, launch_column(c->p, c->natoms > 0 ? c->npjp / 4 : 5, fast, q, nblocks, c->stream));
+            CSF_CUDA(c, launch_column(c->p, c->natoms > 0 ? c->npjp / 4 : 5, fast, f32, q, nblocks, c->stream));
         }
         c->launches += 1;
         return CSF_OK;
     }
 }
 
+size_t f32_block_bytes(const csf_ctx* c, int nvec) { return ((size_t)2 * c->M * ((nvec + 1) & ~1) * sizeof(float2) + 255) / 256 * 256; }
 size_t block_bytes(const csf_ctx* c, int nvec) { return (size_t)2 * c->M * nvec * sizeof(double2); }
 // C~ in fragment order: [atom][chunk][KS][L/8][32] doubles
 size_t ctp_bytes(const csf_ctx* c, int nvec) {
@@ -505,6 +510,11 @@ int csf_set_projectors(csf_ctx* c, int natoms, const int64_t* node_ptr, const in
 
 int csf_workspace_bytes(const csf_ctx* c, int nvec, int mode, size_t* bytes) {
     if (!c || !bytes || nvec < 0) return CSF_EINVAL;
+    if (mode == CSF_FP32_INTERMEDIATE) {
+        // two complex64 blocks with an even leading dimension (16-byte rows for TMA) = the bytes of one complex128 block
+        *bytes = f32_block_bytes(c, nvec) * 2 + coef_bytes(c, nvec) + ctp_bytes(c, nvec) + 256;
+        return CSF_OK;
+    }
     if (mode != CSF_FP64) return CSF_EUNSUPPORTED;
     *bytes = block_bytes(c, nvec) + coef_bytes(c, nvec) + ctp_bytes(c, nvec) + 256;
     return CSF_OK;
@@ -526,8 +536,7 @@ int csf_apply_H(csf_ctx* c, const csf_c128* dX, csf_c128* dY, int64_t ld, int nv
 int csf_filter(csf_ctx* c, const csf_c128* dX, csf_c128* dY, int64_t ld, int nvec, int degree, double a, double b, int mode,
                void* d_work, size_t work_bytes) {
     if (!c) return CSF_EINVAL;
-    if (mode == CSF_FP32_INTERMEDIATE) return fail(c, CSF_EUNSUPPORTED, "CSF_FP32_INTERMEDIATE is not built yet");
-    if (mode != CSF_FP64) return fail(c, CSF_EINVAL, "unknown mode");
+    if (mode != CSF_FP64 && mode != CSF_FP32_INTERMEDIATE) return fail(c, CSF_EINVAL, "unknown mode");
     if (degree < 0) return fail(c, CSF_EINVAL, "degree < 0");
     if (!(a < b)) return fail(c, CSF_EINVAL, "need a < b");
     size_t need = 0;
@@ -545,6 +554,27 @@ int csf_filter(csf_ctx* c, const csf_c128* dX, csf_c128* dY, int64_t ld, int nve
         return CSF_OK;
     }
     char* w = static_cast<char*>(d_work);
+    if (mode == CSF_FP32_INTERMEDIATE) {
+        // The same recurrence with both block buffers in complex64 and FP32 cell arithmetic; X is narrowed on the way in
+        // (W_0 = i^m X), W_m is widened into Y. Projector coefficients C, C~ stay in FP64.
+        const long long ldw = (nvec + 1) & ~1;
+        float2* f0 = reinterpret_cast<float2*>(w);
+        float2* f1 = reinterpret_cast<float2*>(w + f32_block_bytes(c, nvec));
+        double* fC = reinterpret_cast<double*>(w + 2 * f32_block_bytes(c, nvec));
+        double* fCt = reinterpret_cast<double*>(w + 2 * f32_block_bytes(c, nvec) + coef_bytes(c, nvec));
+        { ProfScope ps(c, CSF_KIND_AUX); rot_narrow_kernel<<<c->sm_count * 8, 256, 0, c->stream>>>(X, ld, f0, ldw, rows, nvec, degree & 3); }
+        CSF_CUDA(c, cudaGetLastError()); c->launches += 1;
+        CSF_CUDA(c, cudaMemsetAsync(f1, 0, (size_t)rows * ldw * sizeof(float2), c->stream));
+        // W_1 = (-i/e)(Hhat - c) W_0, then W_{k+1} = W_{k-1} + (-2i/e)(Hhat - c) W_k
+        for (int k = 0; k < degree; ++k) {
+            const bool odd = (k & 1);
+            rc = enqueue_step(c, odd ? f1 : f0, ldw, odd ? f0 : f1, ldw, nvec, (k == 0 ? 1.0 : 2.0) / ee, 3, cc, fC, fCt, true);
+            if (rc != CSF_OK) return rc;
+        }
+        { ProfScope ps(c, CSF_KIND_AUX); widen_kernel<<<c->sm_count * 8, 256, 0, c->stream>>>((degree & 1) ? f1 : f0, ldw, reinterpret_cast<double2*>(Y), ld, rows, nvec); }
+        CSF_CUDA(c, cudaGetLastError()); c->launches += 1;
+        return CSF_OK;
+    }
     double* Wk = reinterpret_cast<double*>(w);                              // the second block buffer, [2M][nvec]
     double* dC = reinterpret_cast<double*>(w + block_bytes(c, nvec));
     double* dCt = reinterpret_cast<double*>(w + block_bytes(c, nvec) + coef_bytes(c, nvec));

@@ -55,9 +55,11 @@ struct ColParams {
     alignas(64) CUtensorMap tm_vb;
     double Ah[kColTab][kColTab];         // h-independent Loewdin-scaled 1-D stiffness (times 1/2), see above
     double uh[kColTab];                  // rank-one part of the 1-D mass
+    float Ahf[kColTab][kColTab];         // the same tables rounded to FP32 (CSF_FP32_INTERMEDIATE)
+    float uhf[kColTab];
     double ax, rho_y, rho_z;             // 2/h_x^2, h_x^2/h_y^2, h_x^2/h_z^2
-    const double* src; double* dst;
-    int rs, rd;                          // doubles per node in src / dst (4 * ld)
+    const void* src; void* dst;          // real type T = double (complex128 blocks) or float (complex64 blocks)
+    int rs, rd;                          // reals per node in src / dst (4 * ld)
     int nvec;
     int ncx, ncy, ncz, nfx, nfy, nfz, bcx, bcy, bcz;
     const int* col_order; int ncols;     // traversal order of the (cx, cy) columns (8x8 tiles)
@@ -78,6 +80,11 @@ struct ColParams {
 __device__ __forceinline__ double col_flip(double x, unsigned mask) {
     return __hiloint2double(__double2hiint(x) ^ (int)mask, __double2loint(x));
 }
+__device__ __forceinline__ float col_flip(float x, unsigned mask) { return __int_as_float(__float_as_int(x) ^ (int)mask); }
+
+template <typename T> struct ColVec2;
+template <> struct ColVec2<double> { using type = double2; };
+template <> struct ColVec2<float> { using type = float2; };
 
 __device__ __forceinline__ int col_free_index(int f, int ncell, int p, int bc) {
     const int nfull = ncell * p;
@@ -103,16 +110,16 @@ template <int N> __host__ __device__ constexpr int col_canon(int i, int j) {
     return best;
 }
 
-template <int P, int L> struct ColCfg {
+template <typename T, int P, int L> struct ColCfg {
     static constexpr int N = P + 1;
     static constexpr int NTM = (N * L + 31) / 32 * 32;               // main threads
     static constexpr int NT = NTM + kColAux;                         // threads per CTA
-    static constexpr int PLANE = N * N * L;                          // doubles per ring plane and field
+    static constexpr int PLANE = N * N * L;                          // reals per ring plane and field
     static constexpr int EPLANE = P * P * L;
     static constexpr int VCELL = P * P * P * 4;                      // V, Bx, By, Bz of the owned nodes of one cell
     // a2 ring, b2 ring, X (nodal + nonlocal terms on the owned nodes of the current cell), staged potential, mbarrier
-    static constexpr size_t XOFF = ((size_t)2 * N * PLANE * sizeof(double) + 127) / 128 * 128;
-    static constexpr size_t XBYTES = ((size_t)P * EPLANE * sizeof(double) + 127) / 128 * 128;     // one X buffer
+    static constexpr size_t XOFF = ((size_t)2 * N * PLANE * sizeof(T) + 127) / 128 * 128;
+    static constexpr size_t XBYTES = ((size_t)P * EPLANE * sizeof(T) + 127) / 128 * 128;          // one X buffer
     static constexpr size_t VBYTES = ((size_t)VCELL * sizeof(double) + 127) / 128 * 128;          // one potential stage
     static constexpr size_t VOFF = XOFF + 2 * XBYTES;          // X and the stage are double-buffered (cell t uses t & 1)
     static constexpr size_t MOFF = VOFF + 2 * VBYTES;
@@ -121,21 +128,25 @@ template <int P, int L> struct ColCfg {
 
 // FAST: every node of the mesh is unconstrained (all directions periodic), nvec is a multiple of L/4 and the cells
 // are cubes (rho_y = rho_z = 1), so no load, store or RED needs a predicate and no rho multiply is issued.
-template <int P, int KS, bool FAST, int L>
-__global__ void __launch_bounds__(ColCfg<P, L>::NT) __maxnreg__((P >= 4 && P <= 5) ? (kColAuxWarps == 2 ? 136 : 144) : 255) column_kernel(const __grid_constant__ ColParams A) {
-    using Cfg = ColCfg<P, L>;
+template <typename T, int P, int KS, bool FAST, int L>
+__global__ void __launch_bounds__(ColCfg<T, P, L>::NT) __maxnreg__((P >= 4 && P <= 5) ? (kColAuxWarps == 2 ? 136 : 144) : 255) column_kernel(const __grid_constant__ ColParams A) {
+    using Cfg = ColCfg<T, P, L>;
+    using T2 = typename ColVec2<T>::type;
     constexpr int N = Cfg::N, NTM = Cfg::NTM, VPC = L / 4;        // VPC vectors per CTA
     constexpr int PLANE = Cfg::PLANE, EPLANE = Cfg::EPLANE;
-    extern __shared__ __align__(128) double smem[];
-    double* R1 = smem;
-    double* R2 = R1 + N * PLANE;
+    extern __shared__ __align__(128) unsigned char smem[];
+    T* R1 = reinterpret_cast<T*>(smem);
+    T* R2 = R1 + N * PLANE;
     char* const xbase = reinterpret_cast<char*>(smem) + Cfg::XOFF;
     char* const vbase = reinterpret_cast<char*>(smem) + Cfg::VOFF;
     const unsigned mbar0 = (unsigned)__cvta_generic_to_shared(reinterpret_cast<char*>(smem) + Cfg::MOFF);
 
-#define AH(i, j) ((&A.Ah[0][0])[col_canon<N>(i, j)])
-#define UH(i) (((P & 1) && (i) > N - 1 - (i)) ? -A.uh[N - 1 - (i)] : A.uh[(i) < N - 1 - (i) ? (i) : N - 1 - (i)])
-#define BETA(i) (((i) == 0 || (i) == P) ? 0.5 : 1.0)
+    constexpr bool F32 = sizeof(T) == 4;
+#define TAB_A(k) (F32 ? (T)(&A.Ahf[0][0])[k] : (T)(&A.Ah[0][0])[k])
+#define TAB_U(k) (F32 ? (T)A.uhf[k] : (T)A.uh[k])
+#define AH(i, j) TAB_A(col_canon<N>(i, j))
+#define UH(i) (((P & 1) && (i) > N - 1 - (i)) ? -TAB_U(N - 1 - (i)) : TAB_U((i) < N - 1 - (i) ? (i) : N - 1 - (i)))
+#define BETA(i) (((i) == 0 || (i) == P) ? (T)0.5 : (T)1.0)
 
     // ---- which (column, segment, vector chunk)
     int r = blockIdx.x;
@@ -178,7 +189,7 @@ __global__ void __launch_bounds__(ColCfg<P, L>::NT) __maxnreg__((P >= 4 && P <= 
                 for (int nt = 0; nt < L / 8; ++nt) bb[s][nt] = __ldg(cb + (s * (L / 8) + nt) * 32);
         };
         for (int t = 0; t < S; ++t) {
-            double* X = reinterpret_cast<double*>(xbase + (t & 1) * Cfg::XBYTES);
+            T* X = reinterpret_cast<T*>(xbase + (t & 1) * Cfg::XBYTES);
             double* VS = reinterpret_cast<double*>(vbase + (t & 1) * Cfg::VBYTES);
             const unsigned mbar = mbar0 + 8 * (t & 1);
             // the first sub-pair's descriptor and C~ fragments do not depend on X: fetch them before any waiting
@@ -196,7 +207,7 @@ __global__ void __launch_bounds__(ColCfg<P, L>::NT) __maxnreg__((P >= 4 && P <= 
             if (aw == 0 && wl == 0) {
                 const int bx0 = cx * P - (A.bcx == 0 ? 0 : 1), by0 = cy * P - (A.bcy == 0 ? 0 : 1), bz0 = (cz0 + t) * P - (A.bcz == 0 ? 0 : 1);
                 asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-                asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mbar), "r"((unsigned)((P * EPLANE + Cfg::VCELL) * sizeof(double))) : "memory");
+                asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mbar), "r"((unsigned)(P * EPLANE * sizeof(T) + Cfg::VCELL * sizeof(double))) : "memory");
                 asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];"
                              ::"r"((unsigned)__cvta_generic_to_shared(X)), "l"(&A.tm_src), "r"(chunk * VPC * 2), "r"(bx0 * 2), "r"(by0), "r"(bz0), "r"(mbar) : "memory");
                 asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
@@ -211,11 +222,11 @@ __global__ void __launch_bounds__(ColCfg<P, L>::NT) __maxnreg__((P >= 4 && P <= 
             // registers, so the 2x2 spin block needs no exchange between threads
             for (int task = wl; task < (xr1 - xr0) * VPC; task += 32) {
                 const int loc = xr0 + task / VPC, vl = task % VPC;
-                double2* xu = reinterpret_cast<double2*>(X + loc * L) + vl;
-                const double2 uu = xu[0], ud = xu[L / 4];
+                T2* xu = reinterpret_cast<T2*>(X + loc * L) + vl;
+                const T2 uu = xu[0], ud = xu[L / 4];
                 const double2 v01 = reinterpret_cast<const double2*>(VS)[2 * loc], v23 = reinterpret_cast<const double2*>(VS)[2 * loc + 1];
-                const double vv = v01.x - A.shift, bx = v01.y, by = v23.x, bz = v23.y;
-                double2 ou, od;
+                const T vv = (T)(v01.x - A.shift), bx = (T)v01.y, by = (T)v23.x, bz = (T)v23.y;
+                T2 ou, od;
                 ou.x = fma(vv + bz, uu.x, fma(bx, ud.x, by * ud.y));
                 ou.y = fma(vv + bz, uu.y, fma(bx, ud.y, -by * ud.x));
                 od.x = fma(vv - bz, ud.x, fma(bx, uu.x, -by * uu.y));
@@ -251,9 +262,9 @@ __global__ void __launch_bounds__(ColCfg<P, L>::NT) __maxnreg__((P >= 4 && P <= 
 #pragma unroll
                                     for (int nt = 0; nt < L / 8; ++nt) col_dmma(c[nt][0], c[nt][1], a[tl][s], b[s][nt]);
                                 if (loc[tl] >= 0) {
-                                    double2* ep = reinterpret_cast<double2*>(X + loc[tl] * L + 2 * kk);
+                                    T2* ep = reinterpret_cast<T2*>(X + loc[tl] * L + 2 * kk);
 #pragma unroll
-                                    for (int nt = 0; nt < L / 8; ++nt) { double2 v = ep[4 * nt]; v.x += c[nt][0]; v.y += c[nt][1]; ep[4 * nt] = v; }
+                                    for (int nt = 0; nt < L / 8; ++nt) { T2 v = ep[4 * nt]; v.x += (T)c[nt][0]; v.y += (T)c[nt][1]; ep[4 * nt] = v; }
                                 }
                             }
                         }
@@ -297,16 +308,16 @@ __global__ void __launch_bounds__(ColCfg<P, L>::NT) __maxnreg__((P >= 4 && P <= 
     }
 #define XO(i) (FAST ? ((i) < P ? x0f + (i) : xPf) : xo_[FAST ? 0 : (i)])
 #define YO(j) (FAST ? ((j) < P ? y0f + (j) * A.nfx : yPf) : yo_[FAST ? 0 : (j)])
-    const double* sp = A.src + ((long long)spin * (A.rs >> 2) + vec) * 2 + ri;
+    const T* sp = static_cast<const T*>(A.src) + ((long long)spin * (A.rs >> 2) + vec) * 2 + ri;
     const int slot_out = ri ^ (A.rot & 1);
     const unsigned sgn = (A.rot == 2 || (A.rot == 1 && ri == 1) || (A.rot == 3 && ri == 0)) ? 0x80000000u : 0u;
-    double* dp = A.dst + ((long long)spin * (A.rd >> 2) + vec) * 2 + slot_out;
-    const double scax = A.sc * A.ax;
+    T* dp = static_cast<T*>(A.dst) + ((long long)spin * (A.rd >> 2) + vec) * 2 + slot_out;
+    const T scax = (T)(A.sc * A.ax);
 
-    double u[N][N];
-    double carry[N];
+    T u[N][N];
+    T carry[N];
 #pragma unroll
-    for (int i = 0; i < N; ++i) carry[i] = 0.0;
+    for (int i = 0; i < N; ++i) carry[i] = (T)0;
 
     // plane of the segment handled by this thread in iteration t (segment-local plane index g), or -1
     auto plane_of = [&](int t) -> int {
@@ -326,7 +337,7 @@ __global__ void __launch_bounds__(ColCfg<P, L>::NT) __maxnreg__((P >= 4 && P <= 
             for (int i = 0; i < N; ++i) {
                 const int node = yz + (FAST ? XO(i) : max(XO(i), 0));
                 if (FAST) u[j][i] = __ldg(sp + (long long)node * A.rs);       // idle threads read plane 0 and drop it
-                else u[j][i] = (pz && XO(i) >= 0 && YO(j) >= 0) ? __ldg(sp + (long long)node * A.rs) : 0.0;
+                else u[j][i] = (pz && XO(i) >= 0 && YO(j) >= 0) ? __ldg(sp + (long long)node * A.rs) : (T)0;
             }
         }
     };
@@ -339,13 +350,13 @@ __global__ void __launch_bounds__(ColCfg<P, L>::NT) __maxnreg__((P >= 4 && P <= 
             const int g = plane_of(t);
             const bool act = g >= 0;
             const int slot = act ? g % N : 0;
-            double* r1 = R1 + slot * PLANE + lane;
-            double* r2 = R2 + slot * PLANE + lane;
+            T* r1 = R1 + slot * PLANE + lane;
+            T* r2 = R2 + slot * PLANE + lane;
             // x-step bookkeeping: d[j] = uh . u[j][:]
-            double d[N];
+            T d[N];
 #pragma unroll
             for (int j = 0; j < N; ++j) {
-                double s = 0.0;
+                T s = (T)0;
 #pragma unroll
                 for (int i = 0; i < N; ++i) s = fma(UH(i), u[j][i], s);
                 d[j] = s;
@@ -353,26 +364,26 @@ __global__ void __launch_bounds__(ColCfg<P, L>::NT) __maxnreg__((P >= 4 && P <= 
             // output column i: a1 = (Ah u)[:, i], b1 = (Bx u)[:, i]; then the y-step on the column
 #pragma unroll
             for (int i = 0; i < N; ++i) {
-                double a1[N], b1[N], b1s[N];
+                T a1[N], b1[N], b1s[N];
 #pragma unroll
                 for (int j = 0; j < N; ++j) {
-                    double s = 0.0;
+                    T s = (T)0;
 #pragma unroll
                     for (int ii = 0; ii < N; ++ii) s = fma(AH(i, ii), u[j][ii], s);
                     a1[j] = s;
                     b1[j] = fma(-UH(i), d[j], BETA(i) * u[j][i]);
-                    b1s[j] = FAST ? b1[j] : A.rho_y * b1[j];
+                    b1s[j] = FAST ? b1[j] : (T)A.rho_y * b1[j];
                 }
-                double da = 0.0, db = 0.0;
+                T da = (T)0, db = (T)0;
 #pragma unroll
                 for (int j = 0; j < N; ++j) { da = fma(UH(j), a1[j], da); db = fma(UH(j), b1[j], db); }
 #pragma unroll
                 for (int j = 0; j < N; ++j) {
-                    double a2 = fma(-UH(j), da, BETA(j) * a1[j]);
+                    T a2 = fma(-UH(j), da, BETA(j) * a1[j]);
 #pragma unroll
                     for (int jj = 0; jj < N; ++jj) a2 = fma(AH(j, jj), b1s[jj], a2);
-                    double b2 = fma(-UH(j), db, BETA(j) * b1[j]);
-                    if (!FAST) b2 *= A.rho_z;
+                    T b2 = fma(-UH(j), db, BETA(j) * b1[j]);
+                    if (!FAST) b2 *= (T)A.rho_z;
                     if (act) { r1[(j * N + i) * L] = a2; r2[(j * N + i) * L] = b2; }
                 }
             }
@@ -380,7 +391,7 @@ __global__ void __launch_bounds__(ColCfg<P, L>::NT) __maxnreg__((P >= 4 && P <= 
         if (t + 1 < S) load_plane(plane_of(t + 1));          // in flight during phase B
         col_bar_sync(1, NTM);                                 // ring written
         col_bar_sync(2 + (t & 1), Cfg::NT);                   // X(t) complete
-        const double* X = reinterpret_cast<const double*>(xbase + (t & 1) * Cfg::XBYTES);
+        const T* X = reinterpret_cast<const T*>(xbase + (t & 1) * Cfg::XBYTES);
         // ------------------------------------------------------------------ phase B
         if (q_on) {
             const int j = q;
@@ -394,24 +405,24 @@ __global__ void __launch_bounds__(ColCfg<P, L>::NT) __maxnreg__((P >= 4 && P <= 
                 const int gz = col_free_index(cz * P + k, A.ncz, P, A.bcz);
                 zn[k] = gz < 0 ? -1 : gz * plane_nodes;
             }
-            const double* r1 = R1 + j * N * L + lane;
-            const double* r2 = R2 + j * N * L + lane;
-            const double* xp = X + j * P * L + lane;
+            const T* r1 = R1 + j * N * L + lane;
+            const T* r2 = R2 + j * N * L + lane;
+            const T* xp = X + j * P * L + lane;
 #pragma unroll
             for (int i = 0; i < N; ++i) {
-                double f1[N], f2[N];
+                T f1[N], f2[N];
 #pragma unroll
                 for (int k = 0; k < N; ++k) {
                     f1[k] = r1[so[k] * PLANE + i * L];
                     f2[k] = r2[so[k] * PLANE + i * L];
                 }
-                double d1 = 0.0;
+                T d1 = (T)0;
 #pragma unroll
                 for (int k = 0; k < N; ++k) d1 = fma(UH(k), f1[k], d1);
-                double o[N];
+                T o[N];
 #pragma unroll
                 for (int k = 0; k < N; ++k) {
-                    double s = fma(-UH(k), d1, BETA(k) * f1[k]);
+                    T s = fma(-UH(k), d1, BETA(k) * f1[k]);
 #pragma unroll
                     for (int k2 = 0; k2 < N; ++k2) s = fma(AH(k, k2), f2[k2], s);
                     o[k] = s;
@@ -422,18 +433,20 @@ __global__ void __launch_bounds__(ColCfg<P, L>::NT) __maxnreg__((P >= 4 && P <= 
                 const int xy = FAST ? XO(i) + YO(j) : max(XO(i), 0) + max(YO(j), 0);
 #pragma unroll
                 for (int k = 0; k < P; ++k) {
-                    double v;
-                    if (j < P && i < P) v = fma(scax, o[k], A.sc * xp[k * EPLANE + i * L]);
+                    T v;
+                    if (j < P && i < P) v = fma(scax, o[k], (T)A.sc * xp[k * EPLANE + i * L]);
                     else v = scax * o[k];
                     if (FAST || (xy_ok && zn[k] >= 0)) atomicAdd(dp + (long long)(xy + zn[k]) * A.rd, col_flip(v, sgn));
                 }
-                if (t == S - 1 && (FAST || (xy_ok && zn[P] >= 0))) atomicAdd(dp + (long long)(xy + zn[P]) * A.rd, col_flip(scax * carry[i], sgn));
+                if (t == S - 1 && (FAST || (xy_ok && zn[P] >= 0))) atomicAdd(dp + (long long)(xy + zn[P]) * A.rd, col_flip((T)(scax * carry[i]), sgn));
             }
         }
         if (t + 2 < S) col_bar_arrive(4 + (t & 1), Cfg::NT);  // this X buffer is free
         col_bar_sync(1, NTM);                                 // ring free
     }
 #undef AH
+#undef TAB_A
+#undef TAB_U
 #undef XO
 #undef YO
 #undef UH

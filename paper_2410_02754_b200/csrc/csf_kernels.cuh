@@ -30,7 +30,7 @@ constexpr int kTabN = 8;
 // (spin, 8 vectors) and read the same P~ rows (L1), every src element is read exactly once per H apply.
 // ---------------------------------------------------------------------------------------------------
 struct GatherParams {
-    const double* src; long long ld; int nvec;
+    const void* src; long long ld; int nvec;       // src: complex128 or complex64 block (template parameter T)
     const int* gb_atom; const int* gb_beg; const int* gb_end;   // gather blocks over the entry list
     const int* gb_k0;                                            // first k-step (4 entries) of the block in g_pack
     const int* ent_node; const double* g_pack;                   // P~^T in A-fragment order [k-step][MT][32]
@@ -44,7 +44,7 @@ __device__ __forceinline__ void gather_dmma(double& d0, double& d1, double a, do
 
 constexpr int kGatherNT = 4;     // n-tiles (of 4 vectors) per warp
 
-template <int MT>      // projector tiles of 8 (npjp <= 8 MT)
+template <int MT, typename T>      // projector tiles of 8 (npjp <= 8 MT); T = real type of src
 __global__ void __launch_bounds__(256) proj_gather_kernel(const __grid_constant__ GatherParams A) {
     const int wl = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int kk = wl & 3, rw = wl >> 2;
@@ -59,7 +59,7 @@ __global__ void __launch_bounds__(256) proj_gather_kernel(const __grid_constant_
     for (int m = 0; m < MT; ++m)
 #pragma unroll
         for (int nt = 0; nt < kGatherNT; ++nt) { acc[m][nt][0] = 0.0; acc[m][nt][1] = 0.0; }
-    const double* sb = A.src + ((long long)spin * A.ld + v0 + (rw >> 1)) * 2 + (rw & 1);
+    const T* sb = static_cast<const T*>(A.src) + ((long long)spin * A.ld + v0 + (rw >> 1)) * 2 + (rw & 1);
     const double* gp = A.g_pack + (long long)A.gb_k0[blockIdx.x] * (MT * 32) + wl;
     auto load_step = [&](int e, int ks, double (&a)[MT], double (&b)[kGatherNT]) {
         const int er = e + kk;
@@ -67,9 +67,9 @@ __global__ void __launch_bounds__(256) proj_gather_kernel(const __grid_constant_
         const int node = __ldg(A.ent_node + (ok ? er : e0));
 #pragma unroll
         for (int m = 0; m < MT; ++m) a[m] = (e < e1) ? __ldg(gp + ((long long)ks * MT + m) * 32) : 0.0;
-        const double* xp = sb + (long long)node * A.ld * 4;
+        const T* xp = sb + (long long)node * A.ld * 4;
 #pragma unroll
-        for (int nt = 0; nt < kGatherNT; ++nt) b[nt] = (ok && v0 + nt * 4 + (rw >> 1) < A.nvec) ? __ldg(xp + nt * 8) : 0.0;
+        for (int nt = 0; nt < kGatherNT; ++nt) b[nt] = (ok && v0 + nt * 4 + (rw >> 1) < A.nvec) ? (double)__ldg(xp + nt * 8) : 0.0;
     };
     // two k-steps are multiplied while the next two are in flight
     double a0[MT], b0[kGatherNT], a1[MT], b1[kGatherNT];
@@ -159,6 +159,33 @@ __global__ void __launch_bounds__(256) rot_copy_kernel(const double2* __restrict
         else if (rot == 2) o = make_double2(-z.x, -z.y);
         else o = make_double2(z.y, -z.x);
         dst[r * ld_dst + v] = o;
+    }
+}
+
+// complex128 [rows][ld] -> complex64 [rows][ld_dst], times i^rot (CSF_FP32_INTERMEDIATE: W_0 = i^m X)
+__global__ void __launch_bounds__(256) rot_narrow_kernel(const double2* __restrict__ src, long long ld, float2* __restrict__ dst,
+                                                         long long ld_dst, long long rows, int nvec, int rot) {
+    const long long total = rows * nvec;
+    for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < total; t += (long long)gridDim.x * blockDim.x) {
+        const long long r = t / nvec; const int v = (int)(t % nvec);
+        const double2 z = src[r * ld + v];
+        double2 o;
+        if (rot == 0) o = z;
+        else if (rot == 1) o = make_double2(-z.y, z.x);
+        else if (rot == 2) o = make_double2(-z.x, -z.y);
+        else o = make_double2(z.y, -z.x);
+        dst[r * ld_dst + v] = make_float2((float)o.x, (float)o.y);
+    }
+}
+
+// complex64 [rows][ld] -> complex128 [rows][ld_dst]
+__global__ void __launch_bounds__(256) widen_kernel(const float2* __restrict__ src, long long ld, double2* __restrict__ dst,
+                                                    long long ld_dst, long long rows, int nvec) {
+    const long long total = rows * nvec;
+    for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < total; t += (long long)gridDim.x * blockDim.x) {
+        const long long r = t / nvec; const int v = (int)(t % nvec);
+        const float2 z = src[r * ld + v];
+        dst[r * ld_dst + v] = make_double2((double)z.x, (double)z.y);
     }
 }
 
