@@ -203,7 +203,8 @@ def main_ours(args):
     t_setup = time.perf_counter()
     sysm = build_system(cfg, ctx, with_projectors=not args.no_projectors)
     M = ctx.M; rows = 2 * M
-    wb = ctx.workspace_bytes(nvec)
+    mode = binding.CSF_FP32_INTERMEDIATE if args.mode == "fp32" else binding.CSF_FP64
+    wb = max(ctx.workspace_bytes(nvec, mode), ctx.workspace_bytes(nvec))
     work = torch.empty(max(wb, 16), dtype=torch.uint8, device="cuda")
 
     # bounds [a, b]: Lanczos on the library's own apply_H (input generation; see bounds.py)
@@ -231,7 +232,7 @@ def main_ours(args):
         torch.cuda.synchronize()
 
     for _ in range(args.warmup):
-        ctx.filter(X, Y, nvec, nvec, degree, a, b, 0, work)
+        ctx.filter(X, Y, nvec, nvec, degree, a, b, mode, work)
     barrier()
     for k in range(binding.KIND_AUX + 1):
         ctx.profile_read(k)
@@ -244,7 +245,7 @@ def main_ours(args):
     e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
     e0.record(stream)
     for _ in range(args.steps):
-        ctx.filter(X, Y, nvec, nvec, degree, a, b, 0, work)
+        ctx.filter(X, Y, nvec, nvec, degree, a, b, mode, work)
     e1.record(stream)
     barrier()
     clocks = sampler.stop() if rank == 0 else None
@@ -311,11 +312,11 @@ def main_ours(args):
         hY = torch.empty((rows, e2e_nvec), dtype=torch.complex128, pin_memory=True)
         ctx.set_host_chunk(args.host_chunk)
         e2e_steps = max(1, min(args.steps, args.e2e_steps))
-        ctx.filter_host(hX, hY, e2e_nvec, min(e2e_nvec, 2 * args.host_chunk), min(degree, 2), a, b, 0)   # warm-up: allocates both staging slots
+        ctx.filter_host(hX, hY, e2e_nvec, min(e2e_nvec, 2 * args.host_chunk), min(degree, 2), a, b, mode)   # warm-up: allocates both staging slots
         barrier()
         t0 = time.perf_counter()
         for _ in range(e2e_steps):
-            ctx.filter_host(hX, hY, e2e_nvec, e2e_nvec, degree, a, b, 0)
+            ctx.filter_host(hX, hY, e2e_nvec, e2e_nvec, degree, a, b, mode)
         torch.cuda.synchronize()
         dt_ms = (time.perf_counter() - t0) * 1e3
         barrier()
@@ -334,10 +335,10 @@ def main_ours(args):
 
     if rank == 0:
         conf = workload_dict(cfg, sysm)
-        conf.update({"block_vectors": nvec, "degree": degree, "bounds": [a, b], "lanczos_ritz": [tmin, tmax], "parallelism": f"replicas x{world}" if world > 1 else "single GPU",
+        conf.update({"block_vectors": nvec, "degree": degree, "bounds": [a, b], "lanczos_ritz": [tmin, tmax], "parallelism": f"replicas x{world}" if world > 1 else "single GPU", "mode": args.mode,
                      "setup_s": round(t_setup, 2)})
         out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step,
-               "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": conf,
+               "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32" if args.mode == "fp32" else "f64", "data": "synthetic", "config": conf,
                "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roof, "step_roofline": step, "cpu_baseline": cpu, "finite": finite}
         print(json.dumps(out))
     if world > 1:
@@ -354,6 +355,7 @@ def main():
     ap.add_argument("--config", type=int, default=3, choices=sorted(synth.CONFIGS))
     ap.add_argument("--nvec", type=int, default=0, help="override the block width (not a bench value)")
     ap.add_argument("--degree", type=int, default=0, help="override the degree (not a bench value)")
+    ap.add_argument("--mode", default="fp64", choices=["fp64", "fp32"], help="fp32 = CSF_FP32_INTERMEDIATE (complex128 in/out, complex64 buffers)")
     ap.add_argument("--variant", type=int, default=0)
     ap.add_argument("--host-chunk", type=int, default=64)
     ap.add_argument("--e2e-steps", type=int, default=2)
