@@ -268,7 +268,10 @@ def main_ours(args):
     except OSError:
         pass
     sm_max = float(peaks.get("sm_max_mhz", 1965.0))
-    peak_alu = SM_COUNT * FP64_FMA_PER_CLK_PER_SM * 2 * sm_max * 1e6 / 1e12
+    fp32 = args.mode == "fp32"
+    # FP32-intermediate mode: the cell arithmetic runs on the FP32 FMA pipe (128 lanes/clk/SM) and moves 24 B/unit
+    peak_alu = SM_COUNT * FP64_FMA_PER_CLK_PER_SM * (2 if fp32 else 1) * 2 * sm_max * 1e6 / 1e12
+    bytes_unit = 24.0 if fp32 else 48.0
     hbm = float(peaks.get("hbm_gbs", 6650.0))
     cell_ms, cell_n = kinds["cell"]
     roof = None
@@ -278,22 +281,22 @@ def main_ours(args):
         traffic = None
         try:
             with open(os.path.join(ROOT, "profiles", "r1_traffic.json")) as f:
-                traffic = float(json.load(f)["dram_bytes_per_unit"]) * rows * nvec    # ncu --set full capture, scaled to this launch
+                traffic = None if fp32 else float(json.load(f)["dram_bytes_per_unit"]) * rows * nvec    # ncu --set full capture (FP64 kernel), scaled to this launch
         except (OSError, KeyError, ValueError):
             pass
         roof = {"kernel": "column_kernel (a1-a4, a7, a8)", "bound": "alu", "achieved": ach, "peak": peak_alu, "unit": "TFLOP/s", "frac": ach / peak_alu,
-                "peak_source": "148 SMs x 64 FP64 FMA/clk x 2 x %.0f MHz (DESIGN.md)" % sm_max, "traffic": traffic,
-                "algorithmic_bytes": 48.0 * rows * nvec,
+                "peak_source": ("148 SMs x 128 FP32 FMA/clk x 2 x %.0f MHz (DESIGN.md)" if fp32 else "148 SMs x 64 FP64 FMA/clk x 2 x %.0f MHz (DESIGN.md)") % sm_max, "traffic": traffic,
+                "algorithmic_bytes": bytes_unit * rows * nvec,
                 "flops_per_unit": f_cell, "avg_launch_ms": t_cell * 1e3, "launches": cell_n,
                 "share_of_step": cell_ms / ms_local,
-                "hbm_achieved_gbs": 48.0 * rows * nvec / t_cell / 1e9, "hbm_peak_gbs": hbm, "hbm_frac": 48.0 * rows * nvec / t_cell / 1e9 / hbm,
+                "hbm_achieved_gbs": bytes_unit * rows * nvec / t_cell / 1e9, "hbm_peak_gbs": hbm, "hbm_frac": bytes_unit * rows * nvec / t_cell / 1e9 / hbm,
                 "hbm_peak_source": "measured (MEASURED_PEAKS.json)" if peaks else "fallback"}
         if not args.no_probe:
             pf, pm = binding.probe_fp64_peak(local)
             roof["peak_measured_dfma"] = pf; roof["peak_measured_dmma"] = pm; roof["frac_of_measured_dfma"] = ach / pf
     step = {"flops_per_unit": f_total, "tflops": f_total * units_step / (ms_per_step * 1e-3) / 1e12,
             "frac_alu": f_total * units_step / (ms_per_step * 1e-3) / 1e12 / peak_alu,
-            "hbm_gbs": 48.0 * units_step / (ms_per_step * 1e-3) / 1e9, "frac_hbm": 48.0 * units_step / (ms_per_step * 1e-3) / 1e9 / hbm,
+            "hbm_gbs": bytes_unit * units_step / (ms_per_step * 1e-3) / 1e9, "frac_hbm": bytes_unit * units_step / (ms_per_step * 1e-3) / 1e9 / hbm,
             "kernel_ms": {k: round(v[0] / args.steps, 3) for k, v in kinds.items()}}
 
     # ---- end to end: host buffers through csf_filter_host (H2D + filter + D2H inside the timed region)
