@@ -45,6 +45,10 @@ constexpr int kColTab = 8;
 #ifndef CSF_AUX_WARPS
 #define CSF_AUX_WARPS 2
 #endif
+#ifndef CSF_XBUF
+#define CSF_XBUF 2
+#endif
+constexpr int kColXBuf = CSF_XBUF;             // X / potential-stage buffers (2: the expansion warps run one cell ahead)
 constexpr int kColAuxWarps = CSF_AUX_WARPS;   // expansion warps per CTA; each owns an equal share of the owned-node rows of X
 constexpr int kColAux = 32 * kColAuxWarps;
 
@@ -121,8 +125,8 @@ template <typename T, int P, int L> struct ColCfg {
     static constexpr size_t XOFF = ((size_t)2 * N * PLANE * sizeof(T) + 127) / 128 * 128;
     static constexpr size_t XBYTES = ((size_t)P * EPLANE * sizeof(T) + 127) / 128 * 128;          // one X buffer
     static constexpr size_t VBYTES = ((size_t)VCELL * sizeof(double) + 127) / 128 * 128;          // one potential stage
-    static constexpr size_t VOFF = XOFF + 2 * XBYTES;          // X and the stage are double-buffered (cell t uses t & 1)
-    static constexpr size_t MOFF = VOFF + 2 * VBYTES;
+    static constexpr size_t VOFF = XOFF + kColXBuf * XBYTES;          // X and the stage are double-buffered (cell t uses t & 1)
+    static constexpr size_t MOFF = VOFF + kColXBuf * VBYTES;
     static constexpr size_t SMEM = MOFF + 32;
 };
 
@@ -189,9 +193,10 @@ __global__ void __launch_bounds__(ColCfg<T, P, L>::NT) __maxnreg__((P >= 4 && P 
                 for (int nt = 0; nt < L / 8; ++nt) bb[s][nt] = __ldg(cb + (s * (L / 8) + nt) * 32);
         };
         for (int t = 0; t < S; ++t) {
-            T* X = reinterpret_cast<T*>(xbase + (t & 1) * Cfg::XBYTES);
-            double* VS = reinterpret_cast<double*>(vbase + (t & 1) * Cfg::VBYTES);
-            const unsigned mbar = mbar0 + 8 * (t & 1);
+            const int xb = t % kColXBuf;
+            T* X = reinterpret_cast<T*>(xbase + xb * Cfg::XBYTES);
+            double* VS = reinterpret_cast<double*>(vbase + xb * Cfg::VBYTES);
+            const unsigned mbar = mbar0 + 8 * xb;
             // the first sub-pair's descriptor and C~ fragments do not depend on X: fetch them before any waiting
             int sp0 = 0, sp1 = 0;
             int4 ds = make_int4(0, 0, 0, 0);           // {atom, first tile in a_pack, entry begin, entry end}
@@ -201,7 +206,7 @@ __global__ void __launch_bounds__(ColCfg<T, P, L>::NT) __maxnreg__((P >= 4 && P 
                 sp0 = A.sub_ptr[cell * kColAuxWarps + aw]; sp1 = A.sub_ptr[cell * kColAuxWarps + aw + 1];
                 if (sp0 < sp1) { ds = __ldg(A.sub_desc + sp0); load_b(ds, b); }
             }
-            if (t >= 2) col_bar_sync(4 + (t & 1), Cfg::NT);      // phase B(t - 2) has consumed this X buffer
+            if (t >= kColXBuf) col_bar_sync(4 + xb, Cfg::NT);    // phase B(t - kColXBuf) has consumed this X buffer
             // TMA: the owned nodes of cell t (src rows of both spins, this CTA's vectors) land in X, their nodal
             // potential in VS; nodes outside the mesh (Dirichlet faces) and vectors >= nvec are zero-filled
             if (aw == 0 && wl == 0) {
@@ -216,7 +221,7 @@ __global__ void __launch_bounds__(ColCfg<T, P, L>::NT) __maxnreg__((P >= 4 && P 
             {
                 unsigned done = 0;
                 while (!done)
-                    asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }" : "=r"(done) : "r"(mbar), "r"((unsigned)((t >> 1) & 1)) : "memory");
+                    asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }" : "=r"(done) : "r"(mbar), "r"((unsigned)((t / kColXBuf) & 1)) : "memory");
             }
             // X = (V + B.sigma - c) X in place on this warp's rows: thread = (node, vector), both spins and re/im in
             // registers, so the 2x2 spin block needs no exchange between threads
@@ -280,7 +285,7 @@ __global__ void __launch_bounds__(ColCfg<T, P, L>::NT) __maxnreg__((P >= 4 && P 
                 }
             }
             __threadfence_block();
-            col_bar_arrive(2 + (t & 1), Cfg::NT);                // X(t) is complete
+            col_bar_arrive(2 + xb, Cfg::NT);                     // X(t) is complete
         }
         return;
     }
@@ -390,8 +395,8 @@ __global__ void __launch_bounds__(ColCfg<T, P, L>::NT) __maxnreg__((P >= 4 && P 
         }
         if (t + 1 < S) load_plane(plane_of(t + 1));          // in flight during phase B
         col_bar_sync(1, NTM);                                 // ring written
-        col_bar_sync(2 + (t & 1), Cfg::NT);                   // X(t) complete
-        const T* X = reinterpret_cast<const T*>(xbase + (t & 1) * Cfg::XBYTES);
+        col_bar_sync(2 + t % kColXBuf, Cfg::NT);              // X(t) complete
+        const T* X = reinterpret_cast<const T*>(xbase + (t % kColXBuf) * Cfg::XBYTES);
         // ------------------------------------------------------------------ phase B
         if (q_on) {
             const int j = q;
@@ -441,7 +446,7 @@ __global__ void __launch_bounds__(ColCfg<T, P, L>::NT) __maxnreg__((P >= 4 && P 
                 if (t == S - 1 && (FAST || (xy_ok && zn[P] >= 0))) atomicAdd(dp + (long long)(xy + zn[P]) * A.rd, col_flip((T)(scax * carry[i]), sgn));
             }
         }
-        if (t + 2 < S) col_bar_arrive(4 + (t & 1), Cfg::NT);  // this X buffer is free
+        if (t + kColXBuf < S) col_bar_arrive(4 + t % kColXBuf, Cfg::NT);   // this X buffer is free
         col_bar_sync(1, NTM);                                 // ring free
     }
 #undef AH
