@@ -88,15 +88,15 @@ struct ProfScope {
     ~ProfScope() { if (e1) { cudaEventRecord(e1, c->stream); c->prof_ev[kind].push_back({e0, e1}); } }
 };
 
-cudaError_t launch_column(int p, int ks, bool fast, bool f32, const ColParams& cp, long long nblocks, cudaStream_t s) {
+cudaError_t launch_column(int p, int ks, int mode, bool f32, const ColParams& cp, long long nblocks, cudaStream_t s) {
     switch (p) {
-        case 1: return launch_column_p1(ks, fast, f32, cp, nblocks, s);
-        case 2: return launch_column_p2(ks, fast, f32, cp, nblocks, s);
-        case 3: return launch_column_p3(ks, fast, f32, cp, nblocks, s);
-        case 4: return launch_column_p4(ks, fast, f32, cp, nblocks, s);
-        case 5: return launch_column_p5(ks, fast, f32, cp, nblocks, s);
-        case 6: return launch_column_p6(ks, fast, f32, cp, nblocks, s);
-        case 7: return launch_column_p7(ks, fast, f32, cp, nblocks, s);
+        case 1: return launch_column_p1(ks, mode, f32, cp, nblocks, s);
+        case 2: return launch_column_p2(ks, mode, f32, cp, nblocks, s);
+        case 3: return launch_column_p3(ks, mode, f32, cp, nblocks, s);
+        case 4: return launch_column_p4(ks, mode, f32, cp, nblocks, s);
+        case 5: return launch_column_p5(ks, mode, f32, cp, nblocks, s);
+        case 6: return launch_column_p6(ks, mode, f32, cp, nblocks, s);
+        case 7: return launch_column_p7(ks, mode, f32, cp, nblocks, s);
     }
     return cudaErrorInvalidValue;
 }
@@ -211,9 +211,11 @@ int enqueue_step(csf_ctx* c, const void* src, long long ld, void* dst, long long
         if (nblocks > 0x7fffffffLL) return fail(c, CSF_EUNSUPPORTED, "grid too large");
         {
             ProfScope ps(c, CSF_KIND_CELL);
-            const bool fast = c->bc[0] == CSF_BC_PERIODIC && c->bc[1] == CSF_BC_PERIODIC && c->bc[2] == CSF_BC_PERIODIC && nvec % vpc == 0 &&
-                              q.rho_y == 1.0 && q.rho_z == 1.0 && c->variant != 1;
-            CSF_CUDA(c, launch_column(c->p, c->natoms > 0 ? c->npjp / 4 : 5, fast, f32, q, nblocks, c->stream));
+            // 2: periodic cubic-cell mesh, full vector chunks; 1: x, y periodic, full chunks (z and the cell shape general); 0: general
+            int kmode = 0;
+            if (c->bc[0] == CSF_BC_PERIODIC && c->bc[1] == CSF_BC_PERIODIC && nvec % vpc == 0 && c->variant != 1)
+                kmode = (c->bc[2] == CSF_BC_PERIODIC && q.rho_y == 1.0 && q.rho_z == 1.0) ? 2 : (f32 ? 1 : 0);   // mode 1 measured slower than 0 in FP64 (register spills)
+            CSF_CUDA(c, launch_column(c->p, c->natoms > 0 ? c->npjp / 4 : 5, kmode, f32, q, nblocks, c->stream));
         }
         c->launches += 1;
         return CSF_OK;

@@ -130,12 +130,14 @@ template <typename T, int P, int L> struct ColCfg {
     static constexpr size_t SMEM = MOFF + 32;
 };
 
-// FAST: every node of the mesh is unconstrained (all directions periodic), nvec is a multiple of L/4 and the cells
+// MODE 2: every node of the mesh is unconstrained (all directions periodic), nvec is a multiple of L/4 and the cells
 // are cubes (rho_y = rho_z = 1), so no load, store or RED needs a predicate and no rho multiply is issued.
-template <typename T, int P, int KS, bool FAST, int L>
+template <typename T, int P, int KS, int MODE, int L>
 __global__ void __launch_bounds__(ColCfg<T, P, L>::NT) __maxnreg__((P >= 4 && P <= 5) ? (sizeof(T) == 4 ? (P == 4 ? 96 : 128) : (P == 4 ? 128 : (kColAuxWarps == 2 ? 136 : 144))) : 255) column_kernel(const __grid_constant__ ColParams A) {
     using Cfg = ColCfg<T, P, L>;
     using T2 = typename ColVec2<T>::type;
+    constexpr bool FAST = MODE >= 1;      // x, y periodic and all lanes live: no per-access predicate
+    constexpr bool ZISO = MODE == 2;      // z periodic too and cubic cells: no z check, no rho multiply
     constexpr int N = Cfg::N, NTM = Cfg::NTM, VPC = L / 4;        // VPC vectors per CTA
     constexpr int PLANE = Cfg::PLANE, EPLANE = Cfg::EPLANE;
     extern __shared__ __align__(128) unsigned char smem[];
@@ -341,7 +343,7 @@ __global__ void __launch_bounds__(ColCfg<T, P, L>::NT) __maxnreg__((P >= 4 && P 
 #pragma unroll
             for (int i = 0; i < N; ++i) {
                 const int node = yz + (FAST ? XO(i) : max(XO(i), 0));
-                if (FAST) u[j][i] = __ldg(sp + (long long)node * A.rs);       // idle threads read plane 0 and drop it
+                if (FAST) u[j][i] = (ZISO || gz >= 0) ? __ldg(sp + (long long)node * A.rs) : (T)0;   // idle threads read plane 0 and drop it
                 else u[j][i] = (pz && XO(i) >= 0 && YO(j) >= 0) ? __ldg(sp + (long long)node * A.rs) : (T)0;
             }
         }
@@ -377,7 +379,7 @@ __global__ void __launch_bounds__(ColCfg<T, P, L>::NT) __maxnreg__((P >= 4 && P 
                     for (int ii = 0; ii < N; ++ii) s = fma(AH(i, ii), u[j][ii], s);
                     a1[j] = s;
                     b1[j] = fma(-UH(i), d[j], BETA(i) * u[j][i]);
-                    b1s[j] = FAST ? b1[j] : (T)A.rho_y * b1[j];
+                    b1s[j] = ZISO ? b1[j] : (T)A.rho_y * b1[j];
                 }
                 T da = (T)0, db = (T)0;
 #pragma unroll
@@ -388,7 +390,7 @@ __global__ void __launch_bounds__(ColCfg<T, P, L>::NT) __maxnreg__((P >= 4 && P 
 #pragma unroll
                     for (int jj = 0; jj < N; ++jj) a2 = fma(AH(j, jj), b1s[jj], a2);
                     T b2 = fma(-UH(j), db, BETA(j) * b1[j]);
-                    if (!FAST) b2 *= (T)A.rho_z;
+                    if (!ZISO) b2 *= (T)A.rho_z;
                     if (act) { r1[(j * N + i) * L] = a2; r2[(j * N + i) * L] = b2; }
                 }
             }
@@ -441,9 +443,9 @@ __global__ void __launch_bounds__(ColCfg<T, P, L>::NT) __maxnreg__((P >= 4 && P 
                     T v;
                     if (j < P && i < P) v = fma(scax, o[k], (T)A.sc * xp[k * EPLANE + i * L]);
                     else v = scax * o[k];
-                    if (FAST || (xy_ok && zn[k] >= 0)) atomicAdd(dp + (long long)(xy + zn[k]) * A.rd, col_flip(v, sgn));
+                    if (ZISO || (xy_ok && zn[k] >= 0)) atomicAdd(dp + (long long)(xy + zn[k]) * A.rd, col_flip(v, sgn));
                 }
-                if (t == S - 1 && (FAST || (xy_ok && zn[P] >= 0))) atomicAdd(dp + (long long)(xy + zn[P]) * A.rd, col_flip((T)(scax * carry[i]), sgn));
+                if (t == S - 1 && (ZISO || (xy_ok && zn[P] >= 0))) atomicAdd(dp + (long long)(xy + zn[P]) * A.rd, col_flip((T)(scax * carry[i]), sgn));
             }
         }
         if (t + kColXBuf < S) col_bar_arrive(4 + t % kColXBuf, Cfg::NT);   // this X buffer is free

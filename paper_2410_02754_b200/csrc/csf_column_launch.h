@@ -9,7 +9,7 @@ struct ColParams;
 struct ColInfo { int lanes; size_t smem; };    // real lanes per CTA (4 per spinor vector), dynamic shared memory
 
 #define CSF_DECL_COL(P) \
-    cudaError_t launch_column_p##P(int ks, bool fast, bool f32, const ColParams& cp, long long nblocks, cudaStream_t s); \
+    cudaError_t launch_column_p##P(int ks, int mode, bool f32, const ColParams& cp, long long nblocks, cudaStream_t s); \
     ColInfo column_info_p##P();
 CSF_DECL_COL(1) CSF_DECL_COL(2) CSF_DECL_COL(3) CSF_DECL_COL(4) CSF_DECL_COL(5) CSF_DECL_COL(6) CSF_DECL_COL(7)
 #undef CSF_DECL_COL

@@ -12,10 +12,10 @@ namespace csf {
 namespace {
 constexpr int kLanes = CSF_P <= 6 ? 16 : 8;      // order 7 does not fit shared memory with 4 vectors per CTA
 
-template <typename T, int KS, bool FAST>
+template <typename T, int KS, int MODE>
 cudaError_t launch_t(const ColParams& cp, long long nblocks, cudaStream_t s) {
     static bool configured = false;
-    auto kern = column_kernel<T, CSF_P, KS, FAST, kLanes>;
+    auto kern = column_kernel<T, CSF_P, KS, MODE, kLanes>;
     using Cfg = ColCfg<T, CSF_P, kLanes>;
     if (!configured) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM);
@@ -31,13 +31,13 @@ cudaError_t launch_t(const ColParams& cp, long long nblocks, cudaStream_t s) {
 #define CSF_CAT(a, b) CSF_CAT2(a, b)
 
 template <typename T>
-cudaError_t launch_real(int ks, bool fast, const ColParams& cp, long long nblocks, cudaStream_t s) {
-    if (ks <= 5) return fast ? launch_t<T, 5, true>(cp, nblocks, s) : launch_t<T, 5, false>(cp, nblocks, s);
-    return fast ? launch_t<T, 8, true>(cp, nblocks, s) : launch_t<T, 8, false>(cp, nblocks, s);
+cudaError_t launch_real(int ks, int mode, const ColParams& cp, long long nblocks, cudaStream_t s) {
+    if (ks <= 5) return mode == 2 ? launch_t<T, 5, 2>(cp, nblocks, s) : mode == 1 ? launch_t<T, 5, 1>(cp, nblocks, s) : launch_t<T, 5, 0>(cp, nblocks, s);
+    return mode == 2 ? launch_t<T, 8, 2>(cp, nblocks, s) : mode == 1 ? launch_t<T, 8, 1>(cp, nblocks, s) : launch_t<T, 8, 0>(cp, nblocks, s);
 }
 
-cudaError_t CSF_CAT(launch_column_p, CSF_P)(int ks, bool fast, bool f32, const ColParams& cp, long long nblocks, cudaStream_t s) {
-    return f32 ? launch_real<float>(ks, fast, cp, nblocks, s) : launch_real<double>(ks, fast, cp, nblocks, s);
+cudaError_t CSF_CAT(launch_column_p, CSF_P)(int ks, int mode, bool f32, const ColParams& cp, long long nblocks, cudaStream_t s) {
+    return f32 ? launch_real<float>(ks, mode, cp, nblocks, s) : launch_real<double>(ks, mode, cp, nblocks, s);
 }
 
 ColInfo CSF_CAT(column_info_p, CSF_P)() { return ColInfo{kLanes, ColCfg<double, CSF_P, kLanes>::SMEM}; }
