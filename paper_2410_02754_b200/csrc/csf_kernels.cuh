@@ -44,8 +44,10 @@ __device__ __forceinline__ void gather_dmma(double& d0, double& d1, double a, do
 
 constexpr int kGatherNT = 4;     // n-tiles (of 4 vectors) per warp
 
-template <int MT, typename T>      // projector tiles of 8 (npjp <= 8 MT); T = real type of src
-__global__ void __launch_bounds__(256) proj_gather_kernel(const __grid_constant__ GatherParams A) {
+// MT projector tiles of 8 in g_pack (npjp <= 8 MT); the first MD of them go through DMMA, NX further projectors
+// (8 MD .. 8 MD + NX - 1, e.g. 16 and 17 of 18) by plain FMAs, which saves a mostly empty tensor tile; T = real type of src
+template <int MT, typename T, int MD = MT, int NX = 0>
+__global__ void __launch_bounds__(256, 2) proj_gather_kernel(const __grid_constant__ GatherParams A) {
     const int wl = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int kk = wl & 3, rw = wl >> 2;
     const int spin = warp & 1;
@@ -54,48 +56,70 @@ __global__ void __launch_bounds__(256) proj_gather_kernel(const __grid_constant_
     const int atom = A.gb_atom[blockIdx.x];
     const int e0 = A.gb_beg[blockIdx.x], e1 = A.gb_end[blockIdx.x];
     const int npj = A.atom_npj[atom];
-    double acc[MT][kGatherNT][2];
+    double acc[MD][kGatherNT][2];
+    double accx[NX > 0 ? NX : 1][kGatherNT];
 #pragma unroll
-    for (int m = 0; m < MT; ++m)
+    for (int m = 0; m < MD; ++m)
 #pragma unroll
         for (int nt = 0; nt < kGatherNT; ++nt) { acc[m][nt][0] = 0.0; acc[m][nt][1] = 0.0; }
+#pragma unroll
+    for (int x = 0; x < (NX > 0 ? NX : 1); ++x)
+#pragma unroll
+        for (int nt = 0; nt < kGatherNT; ++nt) accx[x][nt] = 0.0;
     const T* sb = static_cast<const T*>(A.src) + ((long long)spin * A.ld + v0 + (rw >> 1)) * 2 + (rw & 1);
     const double* gp = A.g_pack + (long long)A.gb_k0[blockIdx.x] * (MT * 32) + wl;
-    auto load_step = [&](int e, int ks, double (&a)[MT], double (&b)[kGatherNT]) {
+    constexpr int NA = MD + (NX > 0 ? NX : 0);      // a[0..MD) = DMMA A fragments, a[MD..) = this thread's row of the extra projectors
+    auto load_step = [&](int e, int ks, double (&a)[NA], double (&b)[kGatherNT]) {
         const int er = e + kk;
         const bool ok = er < e1;
         const int node = __ldg(A.ent_node + (ok ? er : e0));
 #pragma unroll
-        for (int m = 0; m < MT; ++m) a[m] = (e < e1) ? __ldg(gp + ((long long)ks * MT + m) * 32) : 0.0;
+        for (int m = 0; m < MD; ++m) a[m] = (e < e1) ? __ldg(gp + ((long long)ks * MT + m) * 32) : 0.0;
+#pragma unroll
+        for (int x = 0; x < NX; ++x) a[MD + x] = (e < e1) ? __ldg(gp - wl + ((long long)ks * MT + MD) * 32 + x * 4 + kk) : 0.0;
         const T* xp = sb + (long long)node * A.ld * 4;
 #pragma unroll
         for (int nt = 0; nt < kGatherNT; ++nt) b[nt] = (ok && v0 + nt * 4 + (rw >> 1) < A.nvec) ? (double)__ldg(xp + nt * 8) : 0.0;
     };
     // two k-steps are multiplied while the next two are in flight
-    double a0[MT], b0[kGatherNT], a1[MT], b1[kGatherNT];
+    double a0[NA], b0[kGatherNT], a1[NA], b1[kGatherNT];
     load_step(e0, 0, a0, b0);
     load_step(e0 + 4, 1, a1, b1);
     int ks = 0;
     for (int e = e0; e < e1; e += 8, ks += 2) {
-        double a2[MT], b2[kGatherNT], a3[MT], b3[kGatherNT];
+        double a2[NA], b2[kGatherNT], a3[NA], b3[kGatherNT];
         load_step(e + 8, ks + 2, a2, b2);
         load_step(e + 12, ks + 3, a3, b3);
 #pragma unroll
-        for (int m = 0; m < MT; ++m)
+        for (int m = 0; m < MD; ++m)
 #pragma unroll
             for (int nt = 0; nt < kGatherNT; ++nt) gather_dmma(acc[m][nt][0], acc[m][nt][1], a0[m], b0[nt]);
 #pragma unroll
-        for (int m = 0; m < MT; ++m)
+        for (int m = 0; m < MD; ++m)
 #pragma unroll
             for (int nt = 0; nt < kGatherNT; ++nt) gather_dmma(acc[m][nt][0], acc[m][nt][1], a1[m], b1[nt]);
 #pragma unroll
-        for (int m = 0; m < MT; ++m) { a0[m] = a2[m]; a1[m] = a3[m]; }
+        for (int x = 0; x < NX; ++x)
+#pragma unroll
+            for (int nt = 0; nt < kGatherNT; ++nt) accx[x][nt] = fma(a0[MD + x], b0[nt], fma(a1[MD + x], b1[nt], accx[x][nt]));
+#pragma unroll
+        for (int m = 0; m < NA; ++m) { a0[m] = a2[m]; a1[m] = a3[m]; }
 #pragma unroll
         for (int nt = 0; nt < kGatherNT; ++nt) { b0[nt] = b2[nt]; b1[nt] = b3[nt]; }
     }
     const long long coff = A.atom_coff[atom];
+    // extra projectors: sum the four support rows of a k-step (lanes kk = 0..3), lane kk = 0 adds real lane rw of its vector
 #pragma unroll
-    for (int m = 0; m < MT; ++m) {
+    for (int x = 0; x < NX; ++x)
+#pragma unroll
+        for (int nt = 0; nt < kGatherNT; ++nt) {
+            double v = accx[x][nt];
+            v += __shfl_xor_sync(0xffffffffu, v, 1); v += __shfl_xor_sync(0xffffffffu, v, 2);
+            const int vv = v0 + nt * 4 + (rw >> 1);
+            if (kk == 0 && 8 * MD + x < npj && vv < A.nvec) atomicAdd(A.C + ((coff + 2 * (8 * MD + x) + spin) * A.ldc + vv) * 2 + (rw & 1), v);
+        }
+#pragma unroll
+    for (int m = 0; m < MD; ++m) {
         const int chi = m * 8 + rw;
         if (chi < npj) {
 #pragma unroll
