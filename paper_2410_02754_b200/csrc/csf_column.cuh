@@ -133,7 +133,7 @@ template <typename T, int P, int L> struct ColCfg {
 // MODE 2: every node of the mesh is unconstrained (all directions periodic), nvec is a multiple of L/4 and the cells
 // are cubes (rho_y = rho_z = 1), so no load, store or RED needs a predicate and no rho multiply is issued.
 template <typename T, int P, int KS, int MODE, int L>
-__global__ void __launch_bounds__(ColCfg<T, P, L>::NT) __maxnreg__((P >= 4 && P <= 5) ? (sizeof(T) == 4 ? (P == 4 ? 96 : 128) : (P == 4 ? 128 : (kColAuxWarps == 2 ? 136 : 144))) : 255) column_kernel(const __grid_constant__ ColParams A) {
+__global__ void __launch_bounds__(ColCfg<T, P, L>::NT) __maxnreg__((P >= 4 && P <= 5) ? (sizeof(T) == 4 ? (P == 4 ? 96 : 128) : (P == 4 ? 128 : 168)) : 255) column_kernel(const __grid_constant__ ColParams A) {
     using Cfg = ColCfg<T, P, L>;
     using T2 = typename ColVec2<T>::type;
     constexpr bool FAST = MODE >= 1;      // x, y periodic and all lanes live: no per-access predicate
