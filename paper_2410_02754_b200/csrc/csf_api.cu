@@ -150,7 +150,7 @@ int enqueue_step(csf_ctx* c, const void* src, long long ld, void* dst, long long
         dim3 gg(c->n_gather_blocks, (nvec + 16 * kGatherNT - 1) / (16 * kGatherNT));
         {
             ProfScope ps(c, CSF_KIND_PGATHER);
-            if (c->npj_uniform == 18) { if (f32) proj_gather_kernel<3, float, 2, 2><<<gg, 256, 0, c->stream>>>(gp); else proj_gather_kernel<3, double, 2, 2><<<gg, 256, 0, c->stream>>>(gp); }
+            if (c->npj_uniform == 18 && !f32) proj_gather_kernel<3, double, 2, 2><<<gg, 256, 0, c->stream>>>(gp);     // (slower than the full-DMMA form with float loads)
             else if (c->npjp <= 24) { if (f32) proj_gather_kernel<3, float><<<gg, 256, 0, c->stream>>>(gp); else proj_gather_kernel<3, double><<<gg, 256, 0, c->stream>>>(gp); }
             else { if (f32) proj_gather_kernel<4, float><<<gg, 256, 0, c->stream>>>(gp); else proj_gather_kernel<4, double><<<gg, 256, 0, c->stream>>>(gp); }
         }
