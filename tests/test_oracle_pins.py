@@ -395,3 +395,21 @@ def test_error_codes():
         ctx.filter(X, -1, 0.0, 1.0)
     with pytest.raises(RuntimeError):
         O.RefCtx((2, 2, 2), (2.0, 2.0, 2.0), 0, (0, 0, 0))
+
+
+def test_golden_kinetic_spectrum_file():
+    """tests/golden/kinetic_spectrum_cfg0.txt (written by tests/golden/make_golden.py from the oracle; the numbers are
+    those SURVEY.md section 9 lists) still matches the oracle, and its levels obey the closed forms: a zero mode, a
+    six-fold level just below the plane-wave value 1/2 (2 pi / 6)^2, lambda_max = 22.5."""
+    import os
+    from oracle import oracle as O
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "kinetic_spectrum_cfg0.txt")
+    rows = [ln.split() for ln in open(path) if not ln.startswith("#")]
+    idx = [int(r[0]) for r in rows]; val = np.array([float(r[1]) for r in rows])
+    ref = O.RefCtx((3, 3, 3), (6.0, 6.0, 6.0), 3, (0, 0, 0))
+    ref.set_potential(np.zeros(ref.M), None)
+    lam = np.linalg.eigvalsh(ref.dense_H()[0::2, 0::2].real)
+    assert np.allclose(lam[idx], val, atol=2e-9)
+    pw = 0.5 * (2 * np.pi / 6) ** 2
+    assert abs(val[0]) < 1e-9 and np.all(np.abs(val[1:7] - val[1]) < 1e-9) and 0 < pw - val[1] < 3e-4 * pw * 2
+    assert abs(val[-1] - 22.5) < 1e-9
