@@ -33,7 +33,9 @@
 //   - X += sum_a P~^a C~^a per (cell, atom) sub-pair as DMMA tiles (8 support rows x 8 lanes x 4 projectors); both
 //     operands are stored in fragment order, so each fragment is one coalesced 256-byte load. Each warp owns one half
 //     of the rows. The tensor pipe works while the FP64 pipe does phase A.
-// Main and auxiliary warps meet at two named barriers ("X full" / "X free", bar.arrive + bar.sync).
+// X and the stage are double-buffered: the auxiliary warps work one cell ahead and meet the main warps at named
+// barriers ("X[b] full" / "X[b] free", bar.arrive + bar.sync). The real type T is double (complex128 blocks) or float
+// (CSF_FP32_INTERMEDIATE: complex64 blocks, FP32 cell arithmetic; the DMMA tiles and their operands stay FP64).
 #pragma once
 #include <cuda.h>
 #include <cuda_runtime.h>

@@ -12,8 +12,9 @@
 //
 // Data layout: multivector element (node I, spin s, vector v) = complex128 at [(2I+s)*ld + v]. The operator
 // tables are real, so the real and imaginary parts are independent batch entries: a "lane" is one double of
-// the (spin, vector, re/im) batch, lanes of a warp cover contiguous 8-byte words of one or two 128-byte
-// segments (fully coalesced), and the spin 2x2 potential is applied with warp shuffles between lanes.
+// the (spin, vector, re/im) batch and the lanes of a warp cover contiguous 8-byte words of 64-byte row pieces.
+// The projector contractions (a5, a7) are FP64 tensor-core tiles (mma.sync m8n8k4) with both operands stored in
+// fragment order; rot_narrow_kernel / widen_kernel convert between complex128 and complex64 for CSF_FP32_INTERMEDIATE.
 #pragma once
 #include <cuda_runtime.h>
 #include <cstdint>
