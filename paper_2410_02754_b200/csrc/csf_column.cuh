@@ -88,6 +88,10 @@ __device__ __forceinline__ double col_flip(double x, unsigned mask) {
 }
 __device__ __forceinline__ float col_flip(float x, unsigned mask) { return __int_as_float(__float_as_int(x) ^ (int)mask); }
 
+// fire-and-forget reduction (REDG): plain atomicAdd compiles to ATOMG with a discarded result inside this kernel
+__device__ __forceinline__ void col_red(double* p, double v) { asm volatile("red.relaxed.gpu.global.add.f64 [%0], %1;" ::"l"(p), "d"(v) : "memory"); }
+__device__ __forceinline__ void col_red(float* p, float v) { asm volatile("red.relaxed.gpu.global.add.f32 [%0], %1;" ::"l"(p), "f"(v) : "memory"); }
+
 template <typename T> struct ColVec2;
 template <> struct ColVec2<double> { using type = double2; };
 template <> struct ColVec2<float> { using type = float2; };
@@ -445,9 +449,9 @@ __global__ void __launch_bounds__(ColCfg<T, P, L>::NT) __maxnreg__((P >= 4 && P 
                     T v;
                     if (j < P && i < P) v = fma(scax, o[k], (T)A.sc * xp[k * EPLANE + i * L]);
                     else v = scax * o[k];
-                    if (ZISO || (xy_ok && zn[k] >= 0)) atomicAdd(dp + (long long)(xy + zn[k]) * A.rd, col_flip(v, sgn));
+                    if (ZISO || (xy_ok && zn[k] >= 0)) col_red(dp + (long long)(xy + zn[k]) * A.rd, col_flip(v, sgn));
                 }
-                if (t == S - 1 && (ZISO || (xy_ok && zn[P] >= 0))) atomicAdd(dp + (long long)(xy + zn[P]) * A.rd, col_flip((T)(scax * carry[i]), sgn));
+                if (t == S - 1 && (ZISO || (xy_ok && zn[P] >= 0))) col_red(dp + (long long)(xy + zn[P]) * A.rd, col_flip((T)(scax * carry[i]), sgn));
             }
         }
         if (t + kColXBuf < S) col_bar_arrive(4 + t % kColXBuf, Cfg::NT);   // this X buffer is free
