@@ -44,7 +44,7 @@ struct csf_ctx {
     Gll1D gll; Dir1D dir[3];
     bool have_pot = false;
     DevBuf d_cell_order, d_col_order, d_vb;
-    DevBuf d_sub_ptr, d_sub_desc, d_ent_locf, d_a_pack;
+    DevBuf d_sub_ptr[2], d_sub_desc[2], d_a_pack[2], d_ent_locf;     // [0]: 2 expansion warps per CTA, [1]: 3 (order 5 only)
     int seg_len = 16, chunk_group = 16;
     // projectors
     int natoms = 0, npj_uniform = 0, npjp = 0; long long crows = 0;
@@ -202,20 +202,21 @@ int enqueue_step(csf_ctx* c, const void* src, long long ld, void* dst, long long
         q.seg_len = std::min(c->seg_len, c->ncell[2]); q.nseg = (c->ncell[2] + q.seg_len - 1) / q.seg_len;
         q.nchunks = (nvec + vpc - 1) / vpc; q.chunk_group = std::min(c->chunk_group, q.nchunks);
         q.vb = c->d_vb.as<double>(); q.shift = shift; q.sc = sc; q.rot = rot & 3;
+        // 2: periodic cubic-cell mesh, full vector chunks; 1: x, y periodic, full chunks (z and the cell shape general); 0: general
+        int kmode = 0;
+        if (c->bc[0] == CSF_BC_PERIODIC && c->bc[1] == CSF_BC_PERIODIC && nvec % vpc == 0 && c->variant != 1)
+            kmode = (c->bc[2] == CSF_BC_PERIODIC && q.rho_y == 1.0 && q.rho_z == 1.0) ? 2 : (f32 ? 1 : 0);   // mode 1 measured slower than 0 in FP64
+        const int lv = col_aux_warps(c->p, f32, kmode) - 2;      // which sub-pair lists match the kernel's expansion-warp count
         if (c->natoms > 0) {
-            q.sub_ptr = c->d_sub_ptr.as<int>(); q.sub_desc = c->d_sub_desc.as<int4>();
+            q.sub_ptr = c->d_sub_ptr[lv].as<int>(); q.sub_desc = c->d_sub_desc[lv].as<int4>();
             q.ent_loc = c->d_ent_locf.as<int>(); q.ent_p = c->d_ent_p.as<double>();
-            q.Ct = dCt; q.npjp = c->npjp; q.a_pack = c->d_a_pack.as<double>();
+            q.Ct = dCt; q.npjp = c->npjp; q.a_pack = c->d_a_pack[lv].as<double>();
         }
         const long long ngroups = (q.nchunks + q.chunk_group - 1) / q.chunk_group;
         const long long nblocks = (long long)q.chunk_group * q.ncols * q.nseg * ngroups;
         if (nblocks > 0x7fffffffLL) return fail(c, CSF_EUNSUPPORTED, "grid too large");
         {
             ProfScope ps(c, CSF_KIND_CELL);
-            // 2: periodic cubic-cell mesh, full vector chunks; 1: x, y periodic, full chunks (z and the cell shape general); 0: general
-            int kmode = 0;
-            if (c->bc[0] == CSF_BC_PERIODIC && c->bc[1] == CSF_BC_PERIODIC && nvec % vpc == 0 && c->variant != 1)
-                kmode = (c->bc[2] == CSF_BC_PERIODIC && q.rho_y == 1.0 && q.rho_z == 1.0) ? 2 : (f32 ? 1 : 0);   // mode 1 measured slower than 0 in FP64 (register spills)
             CSF_CUDA(c, launch_column(c->p, c->natoms > 0 ? c->npjp / 4 : 5, kmode, f32, q, nblocks, c->stream));
         }
         c->launches += 1;
@@ -466,10 +467,11 @@ int csf_set_projectors(csf_ctx* c, int natoms, const int64_t* node_ptr, const in
     }
     // sub-pairs for the column kernel: every (cell, atom) pair split at the owned-node index XSPLIT = ceil(p^3 / 2)
     // (entries of a pair are sorted by that index), grouped by (cell, half)
-    const int nq = kColAuxWarps, xsplit = (p * p * p + nq - 1) / nq;
+    if (crows >= (1LL << 31)) return fail(c, CSF_EUNSUPPORTED, "too many projector rows");
+    for (int lv = 0; lv < (p == 5 ? 2 : 1); ++lv) {
+    const int nq = 2 + lv, xsplit = (p * p * p + nq - 1) / nq;
     struct Sub { int key; int4 d; };
     std::vector<Sub> subs; subs.reserve(nq * pairs.size());
-    if (crows >= (1LL << 31)) return fail(c, CSF_EUNSUPPORTED, "too many projector rows");
     for (const Pair& pr : pairs) {
         const int e1 = pr.off[p];
         int e = pr.off[0];
@@ -497,11 +499,13 @@ int csf_set_projectors(csf_ctx* c, int natoms, const int64_t* node_ptr, const in
             const size_t tile = (size_t)sb.d.y + (e - sb.d.z) / 8; const int row = (e - sb.d.z) % 8;
             for (int x = 0; x < npjp; ++x) a_pack[(tile * ks + x / 4) * 32 + row * 4 + x % 4] = ent_p[(size_t)e * npjp + x];
         }
+    CSF_CUDA(c, c->d_sub_ptr[lv].upload(sub_ptr)); CSF_CUDA(c, c->d_sub_desc[lv].upload(sub_desc)); CSF_CUDA(c, c->d_a_pack[lv].upload(a_pack));
+    }
     std::vector<double2> dl((size_t)delta_ptr[ntypes]);
     for (size_t i = 0; i < dl.size(); ++i) dl[i] = make_double2(delta[i].re, delta[i].im);
     std::vector<long long> dptr(delta_ptr, delta_ptr + ntypes + 1);
     CSF_CUDA(c, c->d_pair_ptr.upload(pair_ptr)); CSF_CUDA(c, c->d_pair_atom.upload(pair_atom)); CSF_CUDA(c, c->d_pair_off.upload(pair_off));
-    CSF_CUDA(c, c->d_sub_ptr.upload(sub_ptr)); CSF_CUDA(c, c->d_sub_desc.upload(sub_desc)); CSF_CUDA(c, c->d_a_pack.upload(a_pack)); CSF_CUDA(c, c->d_ent_locf.upload(ent_locf));
+    CSF_CUDA(c, c->d_ent_locf.upload(ent_locf));
     CSF_CUDA(c, c->d_ent_loc.upload(ent_loc)); CSF_CUDA(c, c->d_ent_node.upload(ent_node)); CSF_CUDA(c, c->d_ent_p.upload(ent_p));
     CSF_CUDA(c, c->d_atom_coff.upload(atom_coff)); CSF_CUDA(c, c->d_atom_npj.upload(atom_npj)); CSF_CUDA(c, c->d_atom_type.upload(atom_ty));
     CSF_CUDA(c, c->d_delta.upload(dl)); CSF_CUDA(c, c->d_delta_ptr.upload(dptr));

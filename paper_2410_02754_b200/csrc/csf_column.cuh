@@ -44,15 +44,13 @@
 namespace csf {
 
 constexpr int kColTab = 8;
-#ifndef CSF_AUX_WARPS
-#define CSF_AUX_WARPS 2
-#endif
 #ifndef CSF_XBUF
 #define CSF_XBUF 2
 #endif
 constexpr int kColXBuf = CSF_XBUF;             // X / potential-stage buffers (2: the expansion warps run one cell ahead)
-constexpr int kColAuxWarps = CSF_AUX_WARPS;   // expansion warps per CTA; each owns an equal share of the owned-node rows of X
-constexpr int kColAux = 32 * kColAuxWarps;
+// expansion warps per CTA (each owns an equal share of the owned-node rows of X): 3 for the FP64 kernel of order 5 on
+// periodic cubic meshes (measured: 48.9 -> 44.1 ms at config 3), 2 everywhere else (3 costs a CTA per SM there)
+constexpr int col_aux_warps(int p, bool f32, int mode) { return (p == 5 && !f32 && mode == 2) ? 3 : 2; }
 
 struct ColParams {
     // TMA descriptors (cuTensorMapEncodeTiled): src viewed as [nfz][nfy][2 nfx rows][2 nvec doubles], box = the owned
@@ -120,10 +118,11 @@ template <int N> __host__ __device__ constexpr int col_canon(int i, int j) {
     return best;
 }
 
-template <typename T, int P, int L> struct ColCfg {
+template <typename T, int P, int L, int AUXW = 2> struct ColCfg {
     static constexpr int N = P + 1;
     static constexpr int NTM = (N * L + 31) / 32 * 32;               // main threads
-    static constexpr int NT = NTM + kColAux;                         // threads per CTA
+    static constexpr int NAUX = 32 * AUXW;                           // auxiliary (expansion) threads
+    static constexpr int NT = NTM + NAUX;                            // threads per CTA
     static constexpr int PLANE = N * N * L;                          // reals per ring plane and field
     static constexpr int EPLANE = P * P * L;
     static constexpr int VCELL = P * P * P * 4;                      // V, Bx, By, Bz of the owned nodes of one cell
@@ -138,9 +137,10 @@ template <typename T, int P, int L> struct ColCfg {
 
 // MODE 2: every node of the mesh is unconstrained (all directions periodic), nvec is a multiple of L/4 and the cells
 // are cubes (rho_y = rho_z = 1), so no load, store or RED needs a predicate and no rho multiply is issued.
-template <typename T, int P, int KS, int MODE, int L>
-__global__ void __launch_bounds__(ColCfg<T, P, L>::NT) __maxnreg__((P >= 4 && P <= 5) ? (sizeof(T) == 4 ? (P == 4 ? 96 : 128) : (P == 4 ? 128 : 168)) : 255) column_kernel(const __grid_constant__ ColParams A) {
-    using Cfg = ColCfg<T, P, L>;
+template <typename T, int P, int KS, int MODE, int L, int AUXW = col_aux_warps(P, sizeof(T) == 4, MODE)>
+__global__ void __launch_bounds__(ColCfg<T, P, L, AUXW>::NT) __maxnreg__((P >= 4 && P <= 5) ? (sizeof(T) == 4 ? (P == 4 ? 96 : 128) : (P == 4 ? 128 : 168)) : 255) column_kernel(const __grid_constant__ ColParams A) {
+    using Cfg = ColCfg<T, P, L, AUXW>;
+    constexpr int kColAuxWarps = AUXW, kColAux = Cfg::NAUX;
     using T2 = typename ColVec2<T>::type;
     constexpr bool FAST = MODE >= 1;      // x, y periodic and all lanes live: no per-access predicate
     constexpr bool ZISO = MODE == 2;      // z periodic too and cubic cells: no z check, no rho multiply

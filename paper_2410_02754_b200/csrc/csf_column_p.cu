@@ -16,7 +16,7 @@ template <typename T, int KS, int MODE>
 cudaError_t launch_t(const ColParams& cp, long long nblocks, cudaStream_t s) {
     static bool configured = false;
     auto kern = column_kernel<T, CSF_P, KS, MODE, kLanes>;
-    using Cfg = ColCfg<T, CSF_P, kLanes>;
+    using Cfg = ColCfg<T, CSF_P, kLanes, col_aux_warps(CSF_P, sizeof(T) == 4, MODE)>;
     if (!configured) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM);
         if (e != cudaSuccess) return e;
