@@ -469,14 +469,14 @@ int csf_set_projectors(csf_ctx* c, int natoms, const int64_t* node_ptr, const in
     // (entries of a pair are sorted by that index), grouped by (cell, half)
     if (crows >= (1LL << 31)) return fail(c, CSF_EUNSUPPORTED, "too many projector rows");
     for (int lv = 0; lv < (p == 5 ? 2 : 1); ++lv) {
-    const int nq = 2 + lv, xsplit = (p * p * p + nq - 1) / nq;
+    const int nq = 2 + lv;
     struct Sub { int key; int4 d; };
     std::vector<Sub> subs; subs.reserve(nq * pairs.size());
     for (const Pair& pr : pairs) {
         const int e1 = pr.off[p];
         int e = pr.off[0];
         for (int r = 0; r < nq; ++r) {
-            int em = e; while (em < e1 && ent_locf[em] < (r + 1) * xsplit) ++em;
+            int em = e; while (em < e1 && ent_locf[em] < col_aux_row0(p * p * p, nq, r + 1)) ++em;
             if (em > e) subs.push_back({pr.cell * nq + r, make_int4(pr.atom, 0, e, em)});
             e = em;
         }

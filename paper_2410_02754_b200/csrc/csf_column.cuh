@@ -44,13 +44,19 @@
 namespace csf {
 
 constexpr int kColTab = 8;
-#ifndef CSF_XBUF
-#define CSF_XBUF 2
-#endif
-constexpr int kColXBuf = CSF_XBUF;             // X / potential-stage buffers (2: the expansion warps run one cell ahead)
+// X / potential-stage buffers: the expansion warps run one cell ahead. (A third buffer fits at order 5 with 2 CTAs/SM
+// but measured slower, 47.1 against 44.7 ms: it takes the shared-memory carve-out to 228 KB and leaves ~28 KB of L1.)
+constexpr int kColXBuf = 2;
 // expansion warps per CTA (each owns an equal share of the owned-node rows of X): 3 for the FP64 kernel of order 5 on
-// periodic cubic meshes (measured: 48.9 -> 44.1 ms at config 3), 2 everywhere else (3 costs a CTA per SM there)
+// periodic cubic meshes (measured: 48.9 -> 44.1 ms at config 3), 2 everywhere else (3 costs a CTA per SM at order 4, and
+// the general order-5 kernel of config 2 measured 49.7 against 43.4 ms with 3)
 constexpr int col_aux_warps(int p, bool f32, int mode) { return (p == 5 && !f32 && mode == 2) ? 3 : 2; }
+// first owned-node row of expansion warp r of nq (r = nq: one past the end); giving the warp that shares its SM
+// sub-partition with two main warps a smaller share measured slower
+__host__ __device__ constexpr int col_aux_row0(int nodes, int nq, int r) {
+    const int split = (nodes + nq - 1) / nq;
+    return r * split < nodes ? r * split : nodes;
+}
 
 struct ColParams {
     // TMA descriptors (cuTensorMapEncodeTiled): src viewed as [nfz][nfy][2 nfx rows][2 nvec doubles], box = the owned
@@ -105,7 +111,7 @@ __device__ __forceinline__ void col_dmma(double& d0, double& d1, double a, doubl
 }
 
 // named barriers: 1 = main threads only; 2 + b = "X buffer b is full" (expansion warps arrive, main threads wait);
-// 4 + b = "X buffer b is free" (main threads arrive, expansion warps wait)
+// 4 + b = "X buffer b is free" (main threads arrive, expansion warps wait; only when an expansion warp issues the TMA)
 __device__ __forceinline__ void col_bar_sync(int id, int count) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(count) : "memory"); }
 __device__ __forceinline__ void col_bar_arrive(int id, int count) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(count) : "memory"); }
 
@@ -117,6 +123,12 @@ template <int N> __host__ __device__ constexpr int col_canon(int i, int j) {
     c = (N - 1 - j) * kColTab + (N - 1 - i); if (c < best) best = c;
     return best;
 }
+
+// Who issues the TMA loads of a cell: a main thread right after phase B has released the buffer, so that the expansion
+// warps find their data waiting (orders >= 5: config 3 44.0 -> 40.9 ms), or the first expansion warp itself after a
+// "buffer free" barrier (orders <= 4, where a cell is short and the extra work of the main thread costs more than the
+// exposed TMA latency: config 4 44.9 against 45.5 ms).
+__host__ __device__ constexpr bool col_main_tma(int p) { return p >= 5; }
 
 template <typename T, int P, int L, int AUXW = 2> struct ColCfg {
     static constexpr int N = P + 1;
@@ -130,7 +142,7 @@ template <typename T, int P, int L, int AUXW = 2> struct ColCfg {
     static constexpr size_t XOFF = ((size_t)2 * N * PLANE * sizeof(T) + 127) / 128 * 128;
     static constexpr size_t XBYTES = ((size_t)P * EPLANE * sizeof(T) + 127) / 128 * 128;          // one X buffer
     static constexpr size_t VBYTES = ((size_t)VCELL * sizeof(double) + 127) / 128 * 128;          // one potential stage
-    static constexpr size_t VOFF = XOFF + kColXBuf * XBYTES;          // X and the stage are double-buffered (cell t uses t & 1)
+    static constexpr size_t VOFF = XOFF + kColXBuf * XBYTES;          // X and the stage are multi-buffered (cell t uses t % kColXBuf)
     static constexpr size_t MOFF = VOFF + kColXBuf * VBYTES;
     static constexpr size_t SMEM = MOFF + 32;
 };
@@ -141,6 +153,7 @@ template <typename T, int P, int KS, int MODE, int L, int AUXW = col_aux_warps(P
 __global__ void __launch_bounds__(ColCfg<T, P, L, AUXW>::NT) __maxnreg__((P >= 4 && P <= 5) ? (sizeof(T) == 4 ? (P == 4 ? 96 : 128) : (P == 4 ? 128 : 168)) : 255) column_kernel(const __grid_constant__ ColParams A) {
     using Cfg = ColCfg<T, P, L, AUXW>;
     constexpr int kColAuxWarps = AUXW, kColAux = Cfg::NAUX;
+    constexpr bool kMainTma = col_main_tma(P), kPot2 = P >= 5;
     using T2 = typename ColVec2<T>::type;
     constexpr bool FAST = MODE >= 1;      // x, y periodic and all lanes live: no per-access predicate
     constexpr bool ZISO = MODE == 2;      // z periodic too and cubic cells: no z check, no rho multiply
@@ -175,8 +188,8 @@ __global__ void __launch_bounds__(ColCfg<T, P, L, AUXW>::NT) __maxnreg__((P >= 4
     const int plane_nodes = A.nfx * A.nfy;
 
     if (tid == 0) {
-        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(mbar0));
-        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(mbar0 + 8));
+#pragma unroll
+        for (int b = 0; b < kColXBuf; ++b) asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(mbar0 + 8 * b));
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
@@ -191,8 +204,8 @@ __global__ void __launch_bounds__(ColCfg<T, P, L, AUXW>::NT) __maxnreg__((P >= 4
         // same row and need no barrier between them. Its sub-pairs (cell, atom, range) come from the host.
         const int aw = warp_id, wl = tid & 31;
         const int kk = wl & 3, rw = wl >> 2;
-        constexpr int XSPLIT = (P * P * P + kColAuxWarps - 1) / kColAuxWarps, TMAX = (XSPLIT + 7) / 8, TCH = TMAX < 5 ? TMAX : 5;
-        const int xr0 = aw * XSPLIT, xr1 = min(P * P * P, xr0 + XSPLIT);
+        constexpr int TMAX = (P * P * P + 7) / 8, TCH = TMAX < 5 ? TMAX : 5;
+        const int xr0 = col_aux_row0(P * P * P, kColAuxWarps, aw), xr1 = col_aux_row0(P * P * P, kColAuxWarps, aw + 1);
         auto load_b = [&](const int4& ds, double (&bb)[KS][L / 8]) {
             const double* cb = A.Ct + ((long long)ds.x * A.nchunks + chunk) * (KS * (L / 8) * 32) + wl;
 #pragma unroll
@@ -214,37 +227,56 @@ __global__ void __launch_bounds__(ColCfg<T, P, L, AUXW>::NT) __maxnreg__((P >= 4
                 sp0 = A.sub_ptr[cell * kColAuxWarps + aw]; sp1 = A.sub_ptr[cell * kColAuxWarps + aw + 1];
                 if (sp0 < sp1) { ds = __ldg(A.sub_desc + sp0); load_b(ds, b); }
             }
-            if (t >= kColXBuf) col_bar_sync(4 + xb, Cfg::NT);    // phase B(t - kColXBuf) has consumed this X buffer
-            // TMA: the owned nodes of cell t (src rows of both spins, this CTA's vectors) land in X, their nodal
-            // potential in VS; nodes outside the mesh (Dirichlet faces) and vectors >= nvec are zero-filled
-            if (aw == 0 && wl == 0) {
-                const int bx0 = cx * P - (A.bcx == 0 ? 0 : 1), by0 = cy * P - (A.bcy == 0 ? 0 : 1), bz0 = (cz0 + t) * P - (A.bcz == 0 ? 0 : 1);
-                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-                asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mbar), "r"((unsigned)(P * EPLANE * sizeof(T) + Cfg::VCELL * sizeof(double))) : "memory");
-                asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];"
-                             ::"r"((unsigned)__cvta_generic_to_shared(X)), "l"(&A.tm_src), "r"(chunk * VPC * 2), "r"(bx0 * 2), "r"(by0), "r"(bz0), "r"(mbar) : "memory");
-                asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
-                             ::"r"((unsigned)__cvta_generic_to_shared(VS)), "l"(&A.tm_vb), "r"(bx0 * 4), "r"(by0), "r"(bz0), "r"(mbar) : "memory");
+            if constexpr (!kMainTma) {
+                if (t >= kColXBuf) col_bar_sync(4 + xb, Cfg::NT);    // phase B(t - kColXBuf) has consumed this X buffer
+                if (aw == 0 && wl == 0) {
+                    const int bx0 = cx * P - (A.bcx == 0 ? 0 : 1), by0 = cy * P - (A.bcy == 0 ? 0 : 1), bz0 = (cz0 + t) * P - (A.bcz == 0 ? 0 : 1);
+                    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mbar), "r"((unsigned)(P * EPLANE * sizeof(T) + Cfg::VCELL * sizeof(double))) : "memory");
+                    asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];"
+                                 ::"r"((unsigned)__cvta_generic_to_shared(X)), "l"(&A.tm_src), "r"(chunk * VPC * 2), "r"(bx0 * 2), "r"(by0), "r"(bz0), "r"(mbar) : "memory");
+                    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+                                 ::"r"((unsigned)__cvta_generic_to_shared(VS)), "l"(&A.tm_vb), "r"(bx0 * 4), "r"(by0), "r"(bz0), "r"(mbar) : "memory");
+                }
             }
+            // the TMA loads of cell t have landed
             {
                 unsigned done = 0;
-                while (!done)
+                while (true) {
                     asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }" : "=r"(done) : "r"(mbar), "r"((unsigned)((t / kColXBuf) & 1)) : "memory");
+                    if (done) break;
+                    if constexpr (kMainTma) __nanosleep(200);       // the buffer is still in use by phase B: stay out of the main warps' way
+                }
             }
             // X = (V + B.sigma - c) X in place on this warp's rows: thread = (node, vector), both spins and re/im in
-            // registers, so the 2x2 spin block needs no exchange between threads
-            for (int task = wl; task < (xr1 - xr0) * VPC; task += 32) {
-                const int loc = xr0 + task / VPC, vl = task % VPC;
-                T2* xu = reinterpret_cast<T2*>(X + loc * L) + vl;
-                const T2 uu = xu[0], ud = xu[L / 4];
-                const double2 v01 = reinterpret_cast<const double2*>(VS)[2 * loc], v23 = reinterpret_cast<const double2*>(VS)[2 * loc + 1];
-                const T vv = (T)(v01.x - A.shift), bx = (T)v01.y, by = (T)v23.x, bz = (T)v23.y;
-                T2 ou, od;
-                ou.x = fma(vv + bz, uu.x, fma(bx, ud.x, by * ud.y));
-                ou.y = fma(vv + bz, uu.y, fma(bx, ud.y, -by * ud.x));
-                od.x = fma(vv - bz, ud.x, fma(bx, uu.x, -by * uu.y));
-                od.y = fma(vv - bz, ud.y, fma(bx, uu.y, by * uu.x));
-                xu[0] = ou; xu[L / 4] = od;
+            // registers, so the 2x2 spin block needs no exchange between threads; PW tasks per pass (independent chains).
+            // (Swapping the spin halves of neighbouring nodes would remove the 2-way bank conflict of these accesses;
+            // measured slower: the selects cost more than the conflicts.)
+            {
+                constexpr int PW = kPot2 ? 2 : 1;
+                const int ntask = (xr1 - xr0) * VPC;
+                for (int task0 = wl; task0 < ntask; task0 += 32 * PW) {
+                    T2* xu[PW]; T2 uu[PW], ud[PW]; double2 v01[PW], v23[PW]; bool on[PW];
+#pragma unroll
+                    for (int w = 0; w < PW; ++w) {
+                        const int task = task0 + 32 * w;
+                        on[w] = PW == 1 || task < ntask;
+                        const int loc = on[w] ? xr0 + task / VPC : xr0, vl = task % VPC;
+                        xu[w] = reinterpret_cast<T2*>(X + loc * L) + vl;
+                        uu[w] = xu[w][0]; ud[w] = xu[w][L / 4];
+                        v01[w] = reinterpret_cast<const double2*>(VS)[2 * loc]; v23[w] = reinterpret_cast<const double2*>(VS)[2 * loc + 1];
+                    }
+#pragma unroll
+                    for (int w = 0; w < PW; ++w) {
+                        const T vv = (T)(v01[w].x - A.shift), bx = (T)v01[w].y, by = (T)v23[w].x, bz = (T)v23[w].y;
+                        T2 ou, od;
+                        ou.x = fma(vv + bz, uu[w].x, fma(bx, ud[w].x, by * ud[w].y));
+                        ou.y = fma(vv + bz, uu[w].y, fma(bx, ud[w].y, -by * ud[w].x));
+                        od.x = fma(vv - bz, ud[w].x, fma(bx, uu[w].x, -by * uu[w].y));
+                        od.y = fma(vv - bz, ud[w].y, fma(bx, uu[w].y, by * uu[w].x));
+                        if (on[w]) { xu[w][0] = ou; xu[w][L / 4] = od; }
+                    }
+                }
             }
             __syncwarp();
             {
@@ -355,6 +387,25 @@ __global__ void __launch_bounds__(ColCfg<T, P, L, AUXW>::NT) __maxnreg__((P >= 4
         }
     };
 
+    // TMA: the owned nodes of cell t (src rows of both spins, this CTA's vectors) land in X buffer t % kColXBuf, their
+    // nodal potential in its stage; nodes outside the mesh (Dirichlet faces) and vectors >= nvec are zero-filled. Issued
+    // by one main thread as soon as phase B has consumed the buffer, so the expansion warps find their data waiting.
+    auto issue_tma = [&](int t) {
+        const int xb = t % kColXBuf;
+        const unsigned xs = (unsigned)__cvta_generic_to_shared(xbase + xb * Cfg::XBYTES), vs = (unsigned)__cvta_generic_to_shared(vbase + xb * Cfg::VBYTES);
+        const unsigned mbar = mbar0 + 8 * xb;
+        const int bx0 = cx * P - (A.bcx == 0 ? 0 : 1), by0 = cy * P - (A.bcy == 0 ? 0 : 1), bz0 = (cz0 + t) * P - (A.bcz == 0 ? 0 : 1);
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mbar), "r"((unsigned)(P * EPLANE * sizeof(T) + Cfg::VCELL * sizeof(double))) : "memory");
+        asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];"
+                     ::"r"(xs), "l"(&A.tm_src), "r"(chunk * VPC * 2), "r"(bx0 * 2), "r"(by0), "r"(bz0), "r"(mbar) : "memory");
+        asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+                     ::"r"(vs), "l"(&A.tm_vb), "r"(bx0 * 4), "r"(by0), "r"(bz0), "r"(mbar) : "memory");
+    };
+    if constexpr (kMainTma)
+        if (mtid == 0)
+            for (int t = 0; t < kColXBuf && t < S; ++t) issue_tma(t);
+
     load_plane(plane_of(0));
 
     for (int t = 0; t < S; ++t) {
@@ -454,8 +505,11 @@ __global__ void __launch_bounds__(ColCfg<T, P, L, AUXW>::NT) __maxnreg__((P >= 4
                 if (t == S - 1 && (ZISO || (xy_ok && zn[P] >= 0))) col_red(dp + (long long)(xy + zn[P]) * A.rd, col_flip((T)(scax * carry[i]), sgn));
             }
         }
-        if (t + kColXBuf < S) col_bar_arrive(4 + t % kColXBuf, Cfg::NT);   // this X buffer is free
-        col_bar_sync(1, NTM);                                 // ring free
+        if constexpr (!kMainTma)
+            if (t + kColXBuf < S) col_bar_arrive(4 + t % kColXBuf, Cfg::NT);   // this X buffer is free
+        col_bar_sync(1, NTM);                                 // ring and X(t) free
+        if constexpr (kMainTma)
+            if (mtid == 0 && t + kColXBuf < S) issue_tma(t + kColXBuf);
     }
 #undef AH
 #undef TAB_A
