@@ -36,10 +36,12 @@ def build(force: bool = False, verbose: bool = False) -> str:
     objdir = os.path.join(HERE, "build")
     os.makedirs(objdir, exist_ok=True)
     cflags = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
+    cflags += os.environ.get("CSF_NVCC_EXTRA", "").split()         # e.g. -DCSF_WIDE_AUXW=2 for a tuning build
     jobs = [(os.path.join(CSRC, "csf_api.cu"), os.path.join(objdir, "csf_api.o"), []),
             (os.path.join(CSRC, "csf_tables.cpp"), os.path.join(objdir, "csf_tables.o"), [])]
     jobs += [(os.path.join(CSRC, "csf_column_p.cu"), os.path.join(objdir, f"csf_column_p{p}.o"), [f"-DCSF_P={p}"]) for p in range(1, 8)]
-    with ThreadPoolExecutor(max_workers=min(8, os.cpu_count() or 2)) as ex:
+    jobs += [(os.path.join(CSRC, "csf_column_p.cu"), os.path.join(objdir, f"csf_column_wide_p{p}.o"), [f"-DCSF_P={p}", "-DCSF_WIDE=1"]) for p in (4, 5)]
+    with ThreadPoolExecutor(max_workers=min(12, os.cpu_count() or 2)) as ex:
         results = list(ex.map(lambda j: _run(["nvcc"] + cflags + j[2] + ["-c", j[0], "-o", j[1]]), jobs))
     log = "".join(out for _, out in results)
     if verbose or any(rc != 0 for rc, _ in results):

@@ -44,8 +44,9 @@ struct csf_ctx {
     Gll1D gll; Dir1D dir[3];
     bool have_pot = false;
     DevBuf d_cell_order, d_col_order, d_vb;
-    DevBuf d_sub_ptr[2], d_sub_desc[2], d_a_pack[2], d_ent_locf;     // [0]: 2 expansion warps per CTA, [1]: 3 (order 5 only)
+    DevBuf d_sub_ptr[kColMaxAuxWarps - 1], d_sub_desc[kColMaxAuxWarps - 1], d_a_pack[kColMaxAuxWarps - 1], d_ent_locf;     // [nq - 2]: nq expansion warps per CTA
     int seg_len = 16, chunk_group = 16;
+    bool wide = false;                      // column kernel with 8 vectors per CTA instead of 4 (orders 4, 5)
     // projectors
     int natoms = 0, npj_uniform = 0, npjp = 0; long long crows = 0;
     DevBuf d_pair_ptr, d_pair_atom, d_pair_off, d_ent_loc, d_ent_node, d_ent_p, d_atom_coff, d_atom_npj, d_atom_type,
@@ -88,7 +89,11 @@ struct ProfScope {
     ~ProfScope() { if (e1) { cudaEventRecord(e1, c->stream); c->prof_ev[kind].push_back({e0, e1}); } }
 };
 
-cudaError_t launch_column(int p, int ks, int mode, bool f32, const ColParams& cp, long long nblocks, cudaStream_t s) {
+bool have_wide(int p) { return p == 4 || p == 5; }
+
+cudaError_t launch_column(int p, int ks, int mode, bool f32, bool wide, const ColParams& cp, long long nblocks, cudaStream_t s) {
+    if (wide && p == 4) return launch_column_wide_p4(ks, mode, f32, cp, nblocks, s);
+    if (wide && p == 5) return launch_column_wide_p5(ks, mode, f32, cp, nblocks, s);
     switch (p) {
         case 1: return launch_column_p1(ks, mode, f32, cp, nblocks, s);
         case 2: return launch_column_p2(ks, mode, f32, cp, nblocks, s);
@@ -101,7 +106,9 @@ cudaError_t launch_column(int p, int ks, int mode, bool f32, const ColParams& cp
     return cudaErrorInvalidValue;
 }
 
-ColInfo column_info(int p) {
+ColInfo column_info(int p, bool wide) {
+    if (wide && p == 4) return column_info_wide_p4();
+    if (wide && p == 5) return column_info_wide_p5();
     switch (p) {
         case 1: return column_info_p1(); case 2: return column_info_p2(); case 3: return column_info_p3(); case 4: return column_info_p4();
         case 5: return column_info_p5(); case 6: return column_info_p6(); default: return column_info_p7();
@@ -156,7 +163,7 @@ int enqueue_step(csf_ctx* c, const void* src, long long ld, void* dst, long long
         }
         CSF_CUDA(c, cudaGetLastError());
         DeltaParams dp{};
-        const int lanes = column_info(c->p).lanes, nchunks = (nvec + lanes / 4 - 1) / (lanes / 4);
+        const int lanes = column_info(c->p, c->wide).lanes, nchunks = (nvec + lanes / 4 - 1) / (lanes / 4);
         CSF_CUDA(c, cudaMemsetAsync(dCt, 0, ctp_bytes(c, nvec), c->stream));
         dp.C = reinterpret_cast<const double2*>(dC); dp.Ct = dCt; dp.ldc = ldc; dp.nvec = nvec;
         dp.lanes = lanes; dp.ks = c->npjp / 4; dp.nchunks = nchunks;
@@ -168,7 +175,7 @@ int enqueue_step(csf_ctx* c, const void* src, long long ld, void* dst, long long
         c->launches += 2;
     }
     {
-        const ColInfo ci = column_info(c->p);
+        const ColInfo ci = column_info(c->p, c->wide);
         if (ci.smem > c->smem_optin) return fail(c, CSF_EUNSUPPORTED, "column tile does not fit shared memory");
         if (4 * ld >= (1LL << 31) || 4 * ld_dst >= (1LL << 31)) return fail(c, CSF_EUNSUPPORTED, "leading dimension too large");
         const int vpc = ci.lanes / 4;               // spinor vectors per CTA
@@ -206,7 +213,7 @@ int enqueue_step(csf_ctx* c, const void* src, long long ld, void* dst, long long
         int kmode = 0;
         if (c->bc[0] == CSF_BC_PERIODIC && c->bc[1] == CSF_BC_PERIODIC && nvec % vpc == 0 && c->variant != 1)
             kmode = (c->bc[2] == CSF_BC_PERIODIC && q.rho_y == 1.0 && q.rho_z == 1.0) ? 2 : (f32 ? 1 : 0);   // mode 1 measured slower than 0 in FP64
-        const int lv = col_aux_warps(c->p, f32, kmode) - 2;      // which sub-pair lists match the kernel's expansion-warp count
+        const int lv = col_aux_warps(c->p, f32, kmode, ci.lanes) - 2;      // which sub-pair lists match the kernel's expansion-warp count
         if (c->natoms > 0) {
             q.sub_ptr = c->d_sub_ptr[lv].as<int>(); q.sub_desc = c->d_sub_desc[lv].as<int4>();
             q.ent_loc = c->d_ent_locf.as<int>(); q.ent_p = c->d_ent_p.as<double>();
@@ -217,7 +224,7 @@ int enqueue_step(csf_ctx* c, const void* src, long long ld, void* dst, long long
         if (nblocks > 0x7fffffffLL) return fail(c, CSF_EUNSUPPORTED, "grid too large");
         {
             ProfScope ps(c, CSF_KIND_CELL);
-            CSF_CUDA(c, launch_column(c->p, c->natoms > 0 ? c->npjp / 4 : 5, kmode, f32, q, nblocks, c->stream));
+            CSF_CUDA(c, launch_column(c->p, c->natoms > 0 ? c->npjp / 4 : 5, kmode, f32, c->wide, q, nblocks, c->stream));
         }
         c->launches += 1;
         return CSF_OK;
@@ -228,7 +235,7 @@ size_t f32_block_bytes(const csf_ctx* c, int nvec) { return ((size_t)2 * c->M * 
 size_t block_bytes(const csf_ctx* c, int nvec) { return (size_t)2 * c->M * nvec * sizeof(double2); }
 // C~ in fragment order: [atom][chunk][KS][L/8][32] doubles
 size_t ctp_bytes(const csf_ctx* c, int nvec) {
-    const int lanes = column_info(c->p).lanes, nchunks = (nvec + lanes / 4 - 1) / (lanes / 4);
+    const int lanes = column_info(c->p, c->wide).lanes, nchunks = (nvec + lanes / 4 - 1) / (lanes / 4);
     return ((size_t)c->natoms * nchunks * (c->npjp / 4) * (lanes / 8) * 32 * sizeof(double) + 255) / 256 * 256;
 }
 size_t coef_bytes(const csf_ctx* c, int nvec) { return ((size_t)c->crows * nvec * sizeof(double2) + 255) / 256 * 256; }
@@ -295,6 +302,7 @@ int csf_create(csf_ctx** out, const int ncell[3], const double box[3], int order
     c->sm_count = prop.multiProcessorCount; c->smem_optin = prop.sharedMemPerBlockOptin;
     // tuning hooks for sweeps (defaults are the measured best on B200): cells per z-segment, vector chunks per group
     if (const char* e = std::getenv("CSF_SEG_LEN")) { int v = std::atoi(e); if (v >= 1) c->seg_len = v; }
+    if (const char* e = std::getenv("CSF_LANES")) c->wide = std::atoi(e) == 32;
     if (const char* e = std::getenv("CSF_CHUNK_GROUP")) { int v = std::atoi(e); if (v >= 1) c->chunk_group = v; }
     // traversal order of the cells: 8x8x8 bricks, x fastest inside, so that the faces shared between
     // neighbouring cells are combined in L2 before they are evicted
@@ -468,8 +476,12 @@ int csf_set_projectors(csf_ctx* c, int natoms, const int64_t* node_ptr, const in
     // sub-pairs for the column kernel: every (cell, atom) pair split at the owned-node index XSPLIT = ceil(p^3 / 2)
     // (entries of a pair are sorted by that index), grouped by (cell, half)
     if (crows >= (1LL << 31)) return fail(c, CSF_EUNSUPPORTED, "too many projector rows");
-    for (int lv = 0; lv < (p == 5 ? 2 : 1); ++lv) {
+    const int lanes_col = column_info(c->p, c->wide).lanes;
+    for (int lv = 0; lv < kColMaxAuxWarps - 1; ++lv) {
     const int nq = 2 + lv;
+    bool used = false;                          // does any kernel of this order and lane count run nq expansion warps?
+    for (int f = 0; f < 2; ++f) for (int md = 0; md < 3; ++md) used = used || col_aux_warps(p, f != 0, md, lanes_col) == nq;
+    if (!used) continue;
     struct Sub { int key; int4 d; };
     std::vector<Sub> subs; subs.reserve(nq * pairs.size());
     for (const Pair& pr : pairs) {

@@ -49,8 +49,16 @@ constexpr int kColTab = 8;
 constexpr int kColXBuf = 2;
 // expansion warps per CTA (each owns an equal share of the owned-node rows of X): 3 for the FP64 kernel of order 5 on
 // periodic cubic meshes (measured: 48.9 -> 44.1 ms at config 3), 2 everywhere else (3 costs a CTA per SM at order 4, and
-// the general order-5 kernel of config 2 measured 49.7 against 43.4 ms with 3)
-constexpr int col_aux_warps(int p, bool f32, int mode) { return (p == 5 && !f32 && mode == 2) ? 3 : 2; }
+// the general order-5 kernel of config 2 measured 49.7 against 43.4 ms with 3). Wide kernels (32 lanes) of order 5 in
+// FP64: CSF_WIDE_AUXW (the expansion work per CTA doubles with the lane count).
+#ifndef CSF_WIDE_AUXW
+#define CSF_WIDE_AUXW 4
+#endif
+constexpr int kColMaxAuxWarps = 4;
+constexpr int col_aux_warps(int p, bool f32, int mode, int lanes = 16) {
+    if (lanes == 32) return (p == 5 && !f32) ? CSF_WIDE_AUXW : 2;
+    return (p == 5 && !f32 && mode == 2) ? 3 : 2;
+}
 // first owned-node row of expansion warp r of nq (r = nq: one past the end); giving the warp that shares its SM
 // sub-partition with two main warps a smaller share measured slower
 __host__ __device__ constexpr int col_aux_row0(int nodes, int nq, int r) {
@@ -130,6 +138,16 @@ template <int N> __host__ __device__ constexpr int col_canon(int i, int j) {
 // exposed TMA latency: config 4 44.9 against 45.5 ms).
 __host__ __device__ constexpr bool col_main_tma(int p) { return p >= 5; }
 
+// register cap per thread: what the CTAs/SM allowed by shared memory leave (orders 4, 5; other orders uncapped).
+// L = 16: order 4 runs 3 CTAs/SM (FP32: 4), order 5 two (FP32: 3); L = 32 (8 vectors per CTA): order 4 two CTAs/SM of
+// 224 threads (FP32: 3), order 5 one CTA of 288 threads (FP32: two of 256).
+__host__ __device__ constexpr int col_maxreg(int p, bool f32, int lanes, int auxw) {
+    if (p < 4 || p > 5) return 255;
+    // order 5, FP64, 32 lanes: 6 main warps + auxw: up to 8 warps sit 2 per SM sub-partition (16384 registers each), more sit 3
+    if (lanes == 32) return f32 ? (p == 4 ? 96 : 128) : (p == 4 ? 144 : (auxw <= 2 ? 224 : 168));
+    return f32 ? (p == 4 ? 96 : 128) : (p == 4 ? 128 : 168);
+}
+
 template <typename T, int P, int L, int AUXW = 2> struct ColCfg {
     static constexpr int N = P + 1;
     static constexpr int NTM = (N * L + 31) / 32 * 32;               // main threads
@@ -149,12 +167,13 @@ template <typename T, int P, int L, int AUXW = 2> struct ColCfg {
 
 // MODE 2: every node of the mesh is unconstrained (all directions periodic), nvec is a multiple of L/4 and the cells
 // are cubes (rho_y = rho_z = 1), so no load, store or RED needs a predicate and no rho multiply is issued.
-template <typename T, int P, int KS, int MODE, int L, int AUXW = col_aux_warps(P, sizeof(T) == 4, MODE)>
-__global__ void __launch_bounds__(ColCfg<T, P, L, AUXW>::NT) __maxnreg__((P >= 4 && P <= 5) ? (sizeof(T) == 4 ? (P == 4 ? 96 : 128) : (P == 4 ? 128 : 168)) : 255) column_kernel(const __grid_constant__ ColParams A) {
+template <typename T, int P, int KS, int MODE, int L, int AUXW = col_aux_warps(P, sizeof(T) == 4, MODE, L)>
+__global__ void __launch_bounds__(ColCfg<T, P, L, AUXW>::NT) __maxnreg__(col_maxreg(P, sizeof(T) == 4, L, AUXW)) column_kernel(const __grid_constant__ ColParams A) {
     using Cfg = ColCfg<T, P, L, AUXW>;
     constexpr int kColAuxWarps = AUXW, kColAux = Cfg::NAUX;
     constexpr bool kMainTma = col_main_tma(P), kPot2 = P >= 5;
     using T2 = typename ColVec2<T>::type;
+    constexpr bool kWarpPlane = L % 32 == 0;      // a main warp holds exactly one plane
     constexpr bool FAST = MODE >= 1;      // x, y periodic and all lanes live: no per-access predicate
     constexpr bool ZISO = MODE == 2;      // z periodic too and cubic cells: no z check, no rho multiply
     constexpr int N = Cfg::N, NTM = Cfg::NTM, VPC = L / 4;        // VPC vectors per CTA
@@ -204,7 +223,7 @@ __global__ void __launch_bounds__(ColCfg<T, P, L, AUXW>::NT) __maxnreg__((P >= 4
         // same row and need no barrier between them. Its sub-pairs (cell, atom, range) come from the host.
         const int aw = warp_id, wl = tid & 31;
         const int kk = wl & 3, rw = wl >> 2;
-        constexpr int TMAX = (P * P * P + 7) / 8, TCH = TMAX < 5 ? TMAX : 5;
+        constexpr int TMAX = (P * P * P + 7) / 8, TCH = TMAX < 5 ? TMAX : ((L == 32 && sizeof(T) == 4) ? 3 : 5);   // FP32 wide kernels: fewer tiles in flight (registers)
         const int xr0 = col_aux_row0(P * P * P, kColAuxWarps, aw), xr1 = col_aux_row0(P * P * P, kColAuxWarps, aw + 1);
         auto load_b = [&](const int4& ds, double (&bb)[KS][L / 8]) {
             const double* cb = A.Ct + ((long long)ds.x * A.nchunks + chunk) * (KS * (L / 8) * 32) + wl;
@@ -372,6 +391,7 @@ __global__ void __launch_bounds__(ColCfg<T, P, L, AUXW>::NT) __maxnreg__((P >= 4
         return rr < P ? t * P + rr + 1 : -1;
     };
     auto load_plane = [&](int g) {
+        if (kWarpPlane && g < 0) return;
         const int gz = g < 0 ? (FAST ? 0 : -1) : col_free_index(cz0 * P + g, A.ncz, P, A.bcz);
         const bool pz = g >= 0 && lane_on && gz >= 0;
         const int zn = (gz < 0 ? 0 : gz) * plane_nodes;
@@ -416,6 +436,8 @@ __global__ void __launch_bounds__(ColCfg<T, P, L, AUXW>::NT) __maxnreg__((P >= 4
             const int slot = act ? g % N : 0;
             T* r1 = R1 + slot * PLANE + lane;
             T* r2 = R2 + slot * PLANE + lane;
+            // with 32 lanes a warp is one plane: the warp whose plane is not new in this cell skips the phase
+            if (!kWarpPlane || act) {
             // x-step bookkeeping: d[j] = uh . u[j][:]
             T d[N];
 #pragma unroll
@@ -450,6 +472,7 @@ __global__ void __launch_bounds__(ColCfg<T, P, L, AUXW>::NT) __maxnreg__((P >= 4
                     if (!ZISO) b2 *= (T)A.rho_z;
                     if (act) { r1[(j * N + i) * L] = a2; r2[(j * N + i) * L] = b2; }
                 }
+            }
             }
         }
         if (t + 1 < S) load_plane(plane_of(t + 1));          // in flight during phase B

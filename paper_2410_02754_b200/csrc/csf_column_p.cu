@@ -7,16 +7,26 @@
 #error "compile with -DCSF_P=<order>"
 #endif
 
+#define CSF_CAT2(a, b) a##b
+#define CSF_CAT(a, b) CSF_CAT2(a, b)
+
 namespace csf {
 
 namespace {
+#ifdef CSF_WIDE
+// wide variant (its own translation unit, orders 4 and 5): 8 vectors per CTA, 128-byte row pieces, a main warp = one plane
+constexpr int kLanes = 32;
+#define CSF_FN(name) CSF_CAT(CSF_CAT(name, _wide_p), CSF_P)
+#else
 constexpr int kLanes = CSF_P <= 6 ? 16 : 8;      // order 7 does not fit shared memory with 4 vectors per CTA
+#define CSF_FN(name) CSF_CAT(CSF_CAT(name, _p), CSF_P)
+#endif
 
 template <typename T, int KS, int MODE>
 cudaError_t launch_t(const ColParams& cp, long long nblocks, cudaStream_t s) {
     static bool configured = false;
     auto kern = column_kernel<T, CSF_P, KS, MODE, kLanes>;
-    using Cfg = ColCfg<T, CSF_P, kLanes, col_aux_warps(CSF_P, sizeof(T) == 4, MODE)>;
+    using Cfg = ColCfg<T, CSF_P, kLanes, col_aux_warps(CSF_P, sizeof(T) == 4, MODE, kLanes)>;
     if (!configured) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM);
         if (e != cudaSuccess) return e;
@@ -25,21 +35,20 @@ cudaError_t launch_t(const ColParams& cp, long long nblocks, cudaStream_t s) {
     kern<<<(unsigned)nblocks, Cfg::NT, Cfg::SMEM, s>>>(cp);
     return cudaGetLastError();
 }
-}  // namespace
 
-#define CSF_CAT2(a, b) a##b
-#define CSF_CAT(a, b) CSF_CAT2(a, b)
-
+// (inside the unnamed namespace: every order's translation unit instantiates launch_real<T>, and with external linkage
+// the linker would keep one of them for all orders)
 template <typename T>
 cudaError_t launch_real(int ks, int mode, const ColParams& cp, long long nblocks, cudaStream_t s) {
     if (ks <= 5) return mode == 2 ? launch_t<T, 5, 2>(cp, nblocks, s) : mode == 1 ? launch_t<T, 5, 1>(cp, nblocks, s) : launch_t<T, 5, 0>(cp, nblocks, s);
     return mode == 2 ? launch_t<T, 8, 2>(cp, nblocks, s) : mode == 1 ? launch_t<T, 8, 1>(cp, nblocks, s) : launch_t<T, 8, 0>(cp, nblocks, s);
 }
+}  // namespace
 
-cudaError_t CSF_CAT(launch_column_p, CSF_P)(int ks, int mode, bool f32, const ColParams& cp, long long nblocks, cudaStream_t s) {
+cudaError_t CSF_FN(launch_column)(int ks, int mode, bool f32, const ColParams& cp, long long nblocks, cudaStream_t s) {
     return f32 ? launch_real<float>(ks, mode, cp, nblocks, s) : launch_real<double>(ks, mode, cp, nblocks, s);
 }
 
-ColInfo CSF_CAT(column_info_p, CSF_P)() { return ColInfo{kLanes, ColCfg<double, CSF_P, kLanes>::SMEM}; }
+ColInfo CSF_FN(column_info)() { return ColInfo{kLanes, ColCfg<double, CSF_P, kLanes>::SMEM}; }
 
 }  // namespace csf
