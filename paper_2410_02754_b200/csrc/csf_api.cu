@@ -46,7 +46,7 @@ struct csf_ctx {
     DevBuf d_cell_order, d_col_order, d_vb;
     DevBuf d_sub_ptr[kColMaxAuxWarps - 1], d_sub_desc[kColMaxAuxWarps - 1], d_a_pack[kColMaxAuxWarps - 1], d_ent_locf;     // [nq - 2]: nq expansion warps per CTA
     int seg_len = 16, chunk_group = 16;
-    bool wide = false;                      // column kernel with 8 vectors per CTA instead of 4 (orders 4, 5)
+    int lanes_force = 0;                    // CSF_LANES=16|32 pins the column kernel variant (tests, sweeps); 0 = measured policy
     // projectors
     int natoms = 0, npj_uniform = 0, npjp = 0; long long crows = 0;
     DevBuf d_pair_ptr, d_pair_atom, d_pair_off, d_ent_loc, d_ent_node, d_ent_p, d_atom_coff, d_atom_npj, d_atom_type,
@@ -141,11 +141,31 @@ bool encode_map(CUtensorMap* tm, const void* base, int rank, const cuuint64_t* d
 size_t ctp_bytes(const csf_ctx* c, int nvec);
 size_t f32_block_bytes(const csf_ctx* c, int nvec);
 
+// kernel mode for a block of nvec vectors with vpc vectors per CTA. 2: periodic cubic-cell mesh, full vector chunks;
+// 1: x, y periodic, full chunks (z and the cell shape general); 0: general
+int column_mode(const csf_ctx* c, int nvec, int vpc, bool f32) {
+    if (!(c->bc[0] == CSF_BC_PERIODIC && c->bc[1] == CSF_BC_PERIODIC && nvec % vpc == 0 && c->variant != 1)) return 0;
+    const bool cubic = c->h[0] * c->h[0] / (c->h[1] * c->h[1]) == 1.0 && c->h[0] * c->h[0] / (c->h[2] * c->h[2]) == 1.0;
+    return (c->bc[2] == CSF_BC_PERIODIC && cubic) ? 2 : (f32 ? 1 : 0);   // mode 1 measured slower than 0 in FP64
+}
+
+// Which column kernel runs: the wide one (8 vectors per CTA) where it measured faster on B200 — FP64 at orders 4 and 5
+// (config 3: 41.3 -> 38.1 ms, config 2: 43.4 -> 42.2, config 4: 44.8 -> 42.6, config 1: 0.56 -> 0.50 per launch) and the
+// FP32 variant of order 5 off the fully periodic cubic mode (config 2: 31.0 -> 24.6; config 3: 30.8 against 31.3 and
+// config 4: 33.4 against 36.2 stay narrow).
+bool wide_possible(const csf_ctx* c, bool f32, int mode) { return (c->p == 4 && !f32) || (c->p == 5 && (!f32 || mode != 2)); }
+bool use_wide(const csf_ctx* c, int nvec, bool f32) {
+    if (!have_wide(c->p) || c->lanes_force == 16) return false;
+    if (c->lanes_force == 32) return true;
+    return wide_possible(c, f32, column_mode(c, nvec, column_info(c->p, true).lanes / 4, f32));
+}
+
 // one step: dst += sc * i^rot * (Hhat - shift) src
 // src, dst: complex128 blocks, or complex64 blocks when f32 (CSF_FP32_INTERMEDIATE)
 int enqueue_step(csf_ctx* c, const void* src, long long ld, void* dst, long long ld_dst, int nvec, double sc, int rot, double shift,
                  double* dC, double* dCt, bool f32 = false) {
     const long long ldc = nvec;
+    const bool wide = use_wide(c, nvec, f32);
     if (c->natoms > 0) {
         CSF_CUDA(c, cudaMemsetAsync(dC, 0, (size_t)c->crows * ldc * sizeof(double2), c->stream));
         GatherParams gp{};
@@ -163,7 +183,7 @@ int enqueue_step(csf_ctx* c, const void* src, long long ld, void* dst, long long
         }
         CSF_CUDA(c, cudaGetLastError());
         DeltaParams dp{};
-        const int lanes = column_info(c->p, c->wide).lanes, nchunks = (nvec + lanes / 4 - 1) / (lanes / 4);
+        const int lanes = column_info(c->p, wide).lanes, nchunks = (nvec + lanes / 4 - 1) / (lanes / 4);
         CSF_CUDA(c, cudaMemsetAsync(dCt, 0, ctp_bytes(c, nvec), c->stream));
         dp.C = reinterpret_cast<const double2*>(dC); dp.Ct = dCt; dp.ldc = ldc; dp.nvec = nvec;
         dp.lanes = lanes; dp.ks = c->npjp / 4; dp.nchunks = nchunks;
@@ -175,7 +195,7 @@ int enqueue_step(csf_ctx* c, const void* src, long long ld, void* dst, long long
         c->launches += 2;
     }
     {
-        const ColInfo ci = column_info(c->p, c->wide);
+        const ColInfo ci = column_info(c->p, wide);
         if (ci.smem > c->smem_optin) return fail(c, CSF_EUNSUPPORTED, "column tile does not fit shared memory");
         if (4 * ld >= (1LL << 31) || 4 * ld_dst >= (1LL << 31)) return fail(c, CSF_EUNSUPPORTED, "leading dimension too large");
         const int vpc = ci.lanes / 4;               // spinor vectors per CTA
@@ -209,10 +229,7 @@ int enqueue_step(csf_ctx* c, const void* src, long long ld, void* dst, long long
         q.seg_len = std::min(c->seg_len, c->ncell[2]); q.nseg = (c->ncell[2] + q.seg_len - 1) / q.seg_len;
         q.nchunks = (nvec + vpc - 1) / vpc; q.chunk_group = std::min(c->chunk_group, q.nchunks);
         q.vb = c->d_vb.as<double>(); q.shift = shift; q.sc = sc; q.rot = rot & 3;
-        // 2: periodic cubic-cell mesh, full vector chunks; 1: x, y periodic, full chunks (z and the cell shape general); 0: general
-        int kmode = 0;
-        if (c->bc[0] == CSF_BC_PERIODIC && c->bc[1] == CSF_BC_PERIODIC && nvec % vpc == 0 && c->variant != 1)
-            kmode = (c->bc[2] == CSF_BC_PERIODIC && q.rho_y == 1.0 && q.rho_z == 1.0) ? 2 : (f32 ? 1 : 0);   // mode 1 measured slower than 0 in FP64
+        const int kmode = column_mode(c, nvec, vpc, f32);
         const int lv = col_aux_warps(c->p, f32, kmode, ci.lanes) - 2;      // which sub-pair lists match the kernel's expansion-warp count
         if (c->natoms > 0) {
             q.sub_ptr = c->d_sub_ptr[lv].as<int>(); q.sub_desc = c->d_sub_desc[lv].as<int4>();
@@ -224,7 +241,7 @@ int enqueue_step(csf_ctx* c, const void* src, long long ld, void* dst, long long
         if (nblocks > 0x7fffffffLL) return fail(c, CSF_EUNSUPPORTED, "grid too large");
         {
             ProfScope ps(c, CSF_KIND_CELL);
-            CSF_CUDA(c, launch_column(c->p, c->natoms > 0 ? c->npjp / 4 : 5, kmode, f32, c->wide, q, nblocks, c->stream));
+            CSF_CUDA(c, launch_column(c->p, c->natoms > 0 ? c->npjp / 4 : 5, kmode, f32, wide, q, nblocks, c->stream));
         }
         c->launches += 1;
         return CSF_OK;
@@ -235,8 +252,12 @@ size_t f32_block_bytes(const csf_ctx* c, int nvec) { return ((size_t)2 * c->M * 
 size_t block_bytes(const csf_ctx* c, int nvec) { return (size_t)2 * c->M * nvec * sizeof(double2); }
 // C~ in fragment order: [atom][chunk][KS][L/8][32] doubles
 size_t ctp_bytes(const csf_ctx* c, int nvec) {
-    const int lanes = column_info(c->p, c->wide).lanes, nchunks = (nvec + lanes / 4 - 1) / (lanes / 4);
-    return ((size_t)c->natoms * nchunks * (c->npjp / 4) * (lanes / 8) * 32 * sizeof(double) + 255) / 256 * 256;
+    size_t best = 0;                           // the larger of the two lane counts the column kernel may run with
+    for (int w = 0; w < 2; ++w) {
+        const int lanes = column_info(c->p, w != 0).lanes, nchunks = (nvec + lanes / 4 - 1) / (lanes / 4);
+        best = std::max(best, (size_t)c->natoms * nchunks * (c->npjp / 4) * (lanes / 8) * 32 * sizeof(double));
+    }
+    return (best + 255) / 256 * 256;
 }
 size_t coef_bytes(const csf_ctx* c, int nvec) { return ((size_t)c->crows * nvec * sizeof(double2) + 255) / 256 * 256; }
 
@@ -302,7 +323,7 @@ int csf_create(csf_ctx** out, const int ncell[3], const double box[3], int order
     c->sm_count = prop.multiProcessorCount; c->smem_optin = prop.sharedMemPerBlockOptin;
     // tuning hooks for sweeps (defaults are the measured best on B200): cells per z-segment, vector chunks per group
     if (const char* e = std::getenv("CSF_SEG_LEN")) { int v = std::atoi(e); if (v >= 1) c->seg_len = v; }
-    if (const char* e = std::getenv("CSF_LANES")) c->wide = std::atoi(e) == 32;
+    if (const char* e = std::getenv("CSF_LANES")) { int v = std::atoi(e); if (v == 16 || v == 32) c->lanes_force = v; }
     if (const char* e = std::getenv("CSF_CHUNK_GROUP")) { int v = std::atoi(e); if (v >= 1) c->chunk_group = v; }
     // traversal order of the cells: 8x8x8 bricks, x fastest inside, so that the faces shared between
     // neighbouring cells are combined in L2 before they are evicted
@@ -476,11 +497,15 @@ int csf_set_projectors(csf_ctx* c, int natoms, const int64_t* node_ptr, const in
     // sub-pairs for the column kernel: every (cell, atom) pair split at the owned-node index XSPLIT = ceil(p^3 / 2)
     // (entries of a pair are sorted by that index), grouped by (cell, half)
     if (crows >= (1LL << 31)) return fail(c, CSF_EUNSUPPORTED, "too many projector rows");
-    const int lanes_col = column_info(c->p, c->wide).lanes;
     for (int lv = 0; lv < kColMaxAuxWarps - 1; ++lv) {
     const int nq = 2 + lv;
     bool used = false;                          // does any kernel of this order and lane count run nq expansion warps?
-    for (int f = 0; f < 2; ++f) for (int md = 0; md < 3; ++md) used = used || col_aux_warps(p, f != 0, md, lanes_col) == nq;
+    for (int w = 0; w < 2; ++w) {
+        if ((w == 1 && (!have_wide(p) || c->lanes_force == 16)) || (w == 0 && have_wide(p) && c->lanes_force == 32)) continue;
+        for (int f = 0; f < 2; ++f) for (int md = 0; md < 3; ++md)
+            if (c->lanes_force != 0 || !have_wide(p) || wide_possible(c, f != 0, md) == (w == 1))
+                used = used || col_aux_warps(p, f != 0, md, column_info(p, w != 0).lanes) == nq;
+    }
     if (!used) continue;
     struct Sub { int key; int4 d; };
     std::vector<Sub> subs; subs.reserve(nq * pairs.size());

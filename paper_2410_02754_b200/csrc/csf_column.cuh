@@ -54,9 +54,9 @@ constexpr int kColXBuf = 2;
 #ifndef CSF_WIDE_AUXW
 #define CSF_WIDE_AUXW 4
 #endif
-constexpr int kColMaxAuxWarps = 4;
+constexpr int kColMaxAuxWarps = 6;
 constexpr int col_aux_warps(int p, bool f32, int mode, int lanes = 16) {
-    if (lanes == 32) return (p == 5 && !f32) ? CSF_WIDE_AUXW : 2;
+    if (lanes == 32) return (p == 5 && !f32) ? CSF_WIDE_AUXW : (p == 4 ? 3 : 2);
     return (p == 5 && !f32 && mode == 2) ? 3 : 2;
 }
 // first owned-node row of expansion warp r of nq (r = nq: one past the end); giving the warp that shares its SM
@@ -139,12 +139,13 @@ template <int N> __host__ __device__ constexpr int col_canon(int i, int j) {
 __host__ __device__ constexpr bool col_main_tma(int p) { return p >= 5; }
 
 // register cap per thread: what the CTAs/SM allowed by shared memory leave (orders 4, 5; other orders uncapped).
-// L = 16: order 4 runs 3 CTAs/SM (FP32: 4), order 5 two (FP32: 3); L = 32 (8 vectors per CTA): order 4 two CTAs/SM of
-// 224 threads (FP32: 3), order 5 one CTA of 288 threads (FP32: two of 256).
+// L = 16: order 4 runs 3 CTAs/SM (FP32: 4), order 5 two (FP32: 3).
 __host__ __device__ constexpr int col_maxreg(int p, bool f32, int lanes, int auxw) {
     if (p < 4 || p > 5) return 255;
-    // order 5, FP64, 32 lanes: 6 main warps + auxw: up to 8 warps sit 2 per SM sub-partition (16384 registers each), more sit 3
-    if (lanes == 32) return f32 ? (p == 4 ? 96 : 128) : (p == 4 ? 144 : (auxw <= 2 ? 224 : 168));
+    // The register file is per SM sub-partition (16384 registers): w warps per SM sit ceil(w / 4) per sub-partition.
+    // 32 lanes, order 5: 6 main warps + auxw in one CTA/SM (FP64; up to 8 warps sit 2 per sub-partition, up to 12 sit 3) or
+    // two CTAs of 8 warps (FP32); order 4: two CTAs of 5 + 3 warps.
+    if (lanes == 32) return p == 4 ? 128 : (f32 ? 128 : (auxw <= 2 ? 224 : 168));
     return f32 ? (p == 4 ? 96 : 128) : (p == 4 ? 128 : 168);
 }
 
