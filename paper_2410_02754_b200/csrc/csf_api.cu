@@ -146,11 +146,12 @@ size_t f32_block_bytes(const csf_ctx* c, int nvec);
 int column_mode(const csf_ctx* c, int nvec, int vpc, bool f32) {
     if (!(c->bc[0] == CSF_BC_PERIODIC && c->bc[1] == CSF_BC_PERIODIC && nvec % vpc == 0 && c->variant != 1)) return 0;
     const bool cubic = c->h[0] * c->h[0] / (c->h[1] * c->h[1]) == 1.0 && c->h[0] * c->h[0] / (c->h[2] * c->h[2]) == 1.0;
-    return (c->bc[2] == CSF_BC_PERIODIC && cubic) ? 2 : (f32 ? 1 : 0);   // mode 1 measured slower than 0 in FP64
+    // mode 1 measured slower than 0 for the narrow FP64 kernel, faster for the wide one (config 2: 42.2 -> 36.0 ms per launch)
+    return (c->bc[2] == CSF_BC_PERIODIC && cubic) ? 2 : ((f32 || vpc == 8) ? 1 : 0);
 }
 
 // Which column kernel runs: the wide one (8 vectors per CTA) where it measured faster on B200 — FP64 at orders 4 and 5
-// (config 3: 41.3 -> 38.1 ms, config 2: 43.4 -> 42.2, config 4: 44.8 -> 42.6, config 1: 0.56 -> 0.50 per launch) and the
+// (config 3: 41.3 -> 38.1 ms, config 2: 43.4 -> 36.0 with mode 1, config 4: 44.8 -> 42.6, config 1: 0.56 -> 0.50 per launch) and the
 // FP32 variant of order 5 off the fully periodic cubic mode (config 2: 31.0 -> 24.6; config 3: 30.8 against 31.3 and
 // config 4: 33.4 against 36.2 stay narrow).
 bool wide_possible(const csf_ctx* c, bool f32, int mode) { return (c->p == 4 && !f32) || (c->p == 5 && (!f32 || mode != 2)); }
