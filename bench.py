@@ -339,6 +339,7 @@ def main_ours(args):
     if rank == 0:
         conf = workload_dict(cfg, sysm)
         conf.update({"block_vectors": nvec, "degree": degree, "bounds": [a, b], "lanczos_ritz": [tmin, tmax], "parallelism": f"replicas x{world}" if world > 1 else "single GPU", "mode": args.mode,
+                     "column_kernel_lanes": ctx.column_lanes(nvec, 1 if args.mode == "fp32" else 0),
                      "setup_s": round(t_setup, 2)})
         out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step,
                "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32" if args.mode == "fp32" else "f64", "data": "synthetic", "config": conf,

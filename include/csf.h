@@ -140,6 +140,11 @@ int csf_profile_read(csf_ctx* ctx, int kind, double* ms_total, int64_t* launches
  * independent DFMA chains, tflops_mma from mma.sync m8n8k4 f64 (DMMA) chains. Synchronises. Either pointer may be NULL. */
 int csf_probe_fp64_peak(int device, double* tflops_fma, double* tflops_mma);
 
+/* Which column-kernel variant a block of nvec vectors runs with in `mode` on this context: *lanes = 16 (4 vectors per CTA;
+ * 8 lanes = 2 vectors at order 7) or 32 (8 vectors per CTA, orders 4 and 5). The library chooses per call by measurement
+ * on B200; the environment variable CSF_LANES=16|32, read by csf_create, pins it. Host-only query. */
+int csf_column_lanes(const csf_ctx* ctx, int nvec, int mode, int* lanes);
+
 /* Number of kernel launches (own kernels only, memsets excluded) enqueued by this context so far. */
 int csf_launch_count(const csf_ctx* ctx, int64_t* launches);
 

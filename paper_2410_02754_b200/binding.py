@@ -17,7 +17,7 @@ CSF_FP64, CSF_FP32_INTERMEDIATE = 0, 1
 
 EXPORTS = ["csf_create", "csf_destroy", "csf_set_stream", "csf_num_nodes", "csf_node_coords", "csf_mass_diag", "csf_set_potential",
            "csf_set_projectors", "csf_workspace_bytes", "csf_apply_H", "csf_filter", "csf_filter_host", "csf_set_host_chunk",
-           "csf_profile_enable", "csf_profile_read", "csf_probe_fp64_peak", "csf_launch_count", "csf_set_variant", "csf_last_error"]
+           "csf_profile_enable", "csf_profile_read", "csf_probe_fp64_peak", "csf_launch_count", "csf_column_lanes", "csf_set_variant", "csf_last_error"]
 KIND_CELL, KIND_PGATHER, KIND_DELTA, KIND_AUX = 0, 1, 2, 3
 KIND_NAMES = ("cell", "proj_gather", "delta", "aux")
 
@@ -145,6 +145,9 @@ class Csf:
         ms = C.c_double(); n = C.c_int64()
         self._chk(self._L.csf_profile_read(self._h, C.c_int(int(kind)), C.byref(ms), C.byref(n)))
         return float(ms.value), int(n.value)
+
+    def column_lanes(self, nvec, mode=0):
+        n = C.c_int(); self._chk(self._L.csf_column_lanes(self._h, C.c_int(int(nvec)), C.c_int(int(mode)), C.byref(n))); return int(n.value)
 
     def launch_count(self):
         n = C.c_int64(); self._chk(self._L.csf_launch_count(self._h, C.byref(n))); return int(n.value)

@@ -752,6 +752,13 @@ int csf_probe_fp64_peak(int device, double* tflops_fma, double* tflops_mma) {
     return CSF_OK;
 }
 
+int csf_column_lanes(const csf_ctx* c, int nvec, int mode, int* lanes) {
+    if (!c || !lanes || nvec < 1 || (mode != CSF_FP64 && mode != CSF_FP32_INTERMEDIATE)) return CSF_EINVAL;
+    const bool f32 = mode == CSF_FP32_INTERMEDIATE;
+    *lanes = column_info(c->p, use_wide(c, nvec, f32)).lanes;
+    return CSF_OK;
+}
+
 int csf_launch_count(const csf_ctx* c, int64_t* launches) { if (!c || !launches) return CSF_EINVAL; *launches = c->launches; return CSF_OK; }
 
 int csf_set_variant(csf_ctx* c, int variant) {

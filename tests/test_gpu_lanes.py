@@ -49,3 +49,23 @@ def test_policy_and_pinned_variants_agree():
     assert rel_fro(gpu_filter(gpu, X, 6, a, b), Yref) < TOL
     assert rel_fro(gpu_filter32(gpu, X, 6, a, b), Yref) < TOL32
     assert rel_fro(gpu_filter(gpu, X[:, :13], 6, a, b, ld=16), Yref[:, :13]) < TOL
+
+
+def test_column_lanes_query(monkeypatch):
+    """csf_column_lanes reports the variant a call runs with: the measured policy by default, CSF_LANES pins it."""
+    from paper_2410_02754_b200 import binding
+    monkeypatch.delenv("CSF_LANES", raising=False)
+    slab = binding.Csf((2, 2, 3), (4.0, 4.0, 6.0), 5, (0, 0, 1))
+    bulk = binding.Csf((2, 2, 2), (4.0, 4.0, 4.0), 5, (0, 0, 0))
+    p4 = binding.Csf((2, 2, 2), (4.0, 4.0, 4.0), 4, (0, 0, 0))
+    p3 = binding.Csf((2, 2, 2), (4.0, 4.0, 4.0), 3, (0, 0, 0))
+    assert slab.column_lanes(16, binding.CSF_FP64) == 32 and slab.column_lanes(16, binding.CSF_FP32_INTERMEDIATE) == 32
+    assert bulk.column_lanes(16, binding.CSF_FP64) == 32 and bulk.column_lanes(16, binding.CSF_FP32_INTERMEDIATE) == 16
+    assert bulk.column_lanes(13, binding.CSF_FP32_INTERMEDIATE) == 32          # ragged block: general mode
+    assert p4.column_lanes(16, binding.CSF_FP64) == 32 and p4.column_lanes(16, binding.CSF_FP32_INTERMEDIATE) == 16
+    assert p3.column_lanes(16, binding.CSF_FP64) == 16
+    monkeypatch.setenv("CSF_LANES", "16")
+    assert binding.Csf((2, 2, 2), (4.0, 4.0, 4.0), 5, (0, 0, 0)).column_lanes(16, binding.CSF_FP64) == 16
+    monkeypatch.setenv("CSF_LANES", "32")
+    assert binding.Csf((2, 2, 2), (4.0, 4.0, 4.0), 4, (0, 0, 0)).column_lanes(16, binding.CSF_FP32_INTERMEDIATE) == 32
+    assert binding.Csf((2, 2, 2), (4.0, 4.0, 4.0), 3, (0, 0, 0)).column_lanes(16, binding.CSF_FP64) == 16
