@@ -135,8 +135,9 @@ template <int N> __host__ __device__ constexpr int col_canon(int i, int j) {
 // Who issues the TMA loads of a cell: a main thread right after phase B has released the buffer, so that the expansion
 // warps find their data waiting (orders >= 5: config 3 44.0 -> 40.9 ms), or the first expansion warp itself after a
 // "buffer free" barrier (orders <= 4, where a cell is short and the extra work of the main thread costs more than the
-// exposed TMA latency: config 4 44.9 against 45.5 ms).
-__host__ __device__ constexpr bool col_main_tma(int p) { return p >= 5; }
+// exposed TMA latency: config 4 44.9 against 45.5 ms). The wide kernel of order 4 (8 vectors per CTA, a cell takes twice
+// as long) is on the main-thread side again: config 4 44.3 -> 39.8 ms, config 1 0.52 -> 0.47 ms per launch.
+__host__ __device__ constexpr bool col_main_tma(int p, int lanes = 16) { return p >= 5 || (p == 4 && lanes == 32); }
 
 // x-split of the main threads (compile-time option, off): two threads per (plane, lane), each computing one half of the
 // output columns i of phase A and of the z-lines of phase B. The second half works on the x-mirrored plane, which by the
@@ -183,7 +184,7 @@ template <typename T, int P, int KS, int MODE, int L, int AUXW = col_aux_warps(P
 __global__ void __launch_bounds__(ColCfg<T, P, L, AUXW>::NT) __maxnreg__(col_maxreg(P, sizeof(T) == 4, L, AUXW)) column_kernel(const __grid_constant__ ColParams A) {
     using Cfg = ColCfg<T, P, L, AUXW>;
     constexpr int kColAuxWarps = AUXW, kColAux = Cfg::NAUX;
-    constexpr bool kMainTma = col_main_tma(P), kPot2 = P >= 5;
+    constexpr bool kMainTma = col_main_tma(P, L), kPot2 = P >= 5;
     using T2 = typename ColVec2<T>::type;
     constexpr bool kWarpPlane = L % 32 == 0;      // a main warp holds exactly one plane
     constexpr bool FAST = MODE >= 1;      // x, y periodic and all lanes live: no per-access predicate
