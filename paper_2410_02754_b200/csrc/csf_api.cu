@@ -150,11 +150,11 @@ int column_mode(const csf_ctx* c, int nvec, int vpc, bool f32) {
     return (c->bc[2] == CSF_BC_PERIODIC && cubic) ? 2 : ((f32 || vpc == 8) ? 1 : 0);
 }
 
-// Which column kernel runs: the wide one (8 vectors per CTA) where it measured faster on B200 — FP64 at orders 4 and 5
-// (config 3: 41.3 -> 38.1 ms, config 2: 43.4 -> 36.0 with mode 1, config 4: 44.8 -> 42.6, config 1: 0.56 -> 0.50 per launch) and the
-// FP32 variant of order 5 off the fully periodic cubic mode (config 2: 31.0 -> 24.6; config 3: 30.8 against 31.3 and
-// config 4: 33.4 against 36.2 stay narrow).
-bool wide_possible(const csf_ctx* c, bool f32, int mode) { return (c->p == 4 && !f32) || (c->p == 5 && (!f32 || mode != 2)); }
+// Which column kernel runs: the wide one (8 vectors per CTA) where it measured faster on B200 — order 4 (FP64 config 4:
+// 44.8 -> 39.8 ms per launch, config 1: 0.56 -> 0.47; FP32 config 4: 33.5 -> 30.8, config 1: 0.41 -> 0.36), order 5 in FP64
+// (config 3: 41.3 -> 38.1, config 2: 43.4 -> 36.0 with mode 1) and the FP32 variant of order 5 off the fully periodic
+// cubic mode (config 2: 31.0 -> 24.6; config 3 stays narrow: 30.8 against 31.3).
+bool wide_possible(const csf_ctx* c, bool f32, int mode) { return c->p == 4 || (c->p == 5 && (!f32 || mode != 2)); }
 bool use_wide(const csf_ctx* c, int nvec, bool f32) {
     if (!have_wide(c->p) || c->lanes_force == 16) return false;
     if (c->lanes_force == 32) return true;

@@ -62,10 +62,10 @@ def test_column_lanes_query(monkeypatch):
     assert slab.column_lanes(16, binding.CSF_FP64) == 32 and slab.column_lanes(16, binding.CSF_FP32_INTERMEDIATE) == 32
     assert bulk.column_lanes(16, binding.CSF_FP64) == 32 and bulk.column_lanes(16, binding.CSF_FP32_INTERMEDIATE) == 16
     assert bulk.column_lanes(13, binding.CSF_FP32_INTERMEDIATE) == 32          # ragged block: general mode
-    assert p4.column_lanes(16, binding.CSF_FP64) == 32 and p4.column_lanes(16, binding.CSF_FP32_INTERMEDIATE) == 16
+    assert p4.column_lanes(16, binding.CSF_FP64) == 32 and p4.column_lanes(16, binding.CSF_FP32_INTERMEDIATE) == 32
     assert p3.column_lanes(16, binding.CSF_FP64) == 16
     monkeypatch.setenv("CSF_LANES", "16")
     assert binding.Csf((2, 2, 2), (4.0, 4.0, 4.0), 5, (0, 0, 0)).column_lanes(16, binding.CSF_FP64) == 16
     monkeypatch.setenv("CSF_LANES", "32")
-    assert binding.Csf((2, 2, 2), (4.0, 4.0, 4.0), 4, (0, 0, 0)).column_lanes(16, binding.CSF_FP32_INTERMEDIATE) == 32
+    assert binding.Csf((2, 2, 2), (4.0, 4.0, 4.0), 5, (0, 0, 0)).column_lanes(16, binding.CSF_FP32_INTERMEDIATE) == 32
     assert binding.Csf((2, 2, 2), (4.0, 4.0, 4.0), 3, (0, 0, 0)).column_lanes(16, binding.CSF_FP64) == 16
