@@ -68,6 +68,7 @@ typedef struct ref_ctx {
     /* projectors */
     int natoms; int64_t *node_ptr; int64_t *node_idx; int *nproj; int64_t *pval_ptr; double *pvals;
     int *atom_type; int ntypes; ref_c128 *delta; int64_t *delta_ptr;
+    int *atom_distinct; /* [natoms] 1 if the atom's support lists every node once (then its rows of Y can be updated in parallel) */
 } ref_ctx;
 
 /* ------------------------------------------------------------------ */
@@ -289,7 +290,7 @@ int ref_destroy(ref_ctx *c) {
     free(c->conn); free(c->mass); free(c->Ke); free(c->rowptr); free(c->col); free(c->val);
     free(c->veff); free(c->bxyz);
     free(c->node_ptr); free(c->node_idx); free(c->nproj); free(c->pval_ptr); free(c->pvals);
-    free(c->atom_type); free(c->delta); free(c->delta_ptr);
+    free(c->atom_type); free(c->delta); free(c->delta_ptr); free(c->atom_distinct);
     free(c);
     return REF_OK;
 }
@@ -388,7 +389,7 @@ int ref_set_projectors(ref_ctx *c, int natoms, const int64_t *node_ptr, const in
                        const double *pvals, const int *atom_type, int ntypes, const ref_c128 *delta, const int64_t *delta_ptr) {
     if (!c || natoms < 0) return REF_EINVAL;
     free(c->node_ptr); free(c->node_idx); free(c->nproj); free(c->pval_ptr); free(c->pvals);
-    free(c->atom_type); free(c->delta); free(c->delta_ptr);
+    free(c->atom_type); free(c->delta); free(c->delta_ptr); free(c->atom_distinct); c->atom_distinct = NULL;
     c->node_ptr = NULL; c->node_idx = NULL; c->nproj = NULL; c->pval_ptr = NULL; c->pvals = NULL;
     c->atom_type = NULL; c->delta = NULL; c->delta_ptr = NULL; c->natoms = 0; c->ntypes = 0;
     if (natoms == 0) return REF_OK;
@@ -417,6 +418,15 @@ int ref_set_projectors(ref_ctx *c, int natoms, const int64_t *node_ptr, const in
     memcpy(c->pvals, pvals, (size_t)c->pval_ptr[natoms] * sizeof(double));
     c->delta = (ref_c128 *)malloc((size_t)delta_ptr[ntypes] * sizeof(ref_c128));
     memcpy(c->delta, delta, (size_t)delta_ptr[ntypes] * sizeof(ref_c128));
+    c->atom_distinct = (int *)malloc((size_t)natoms * sizeof(int));
+    for (int a = 0; a < natoms; a++) {
+        int64_t na = node_ptr[a + 1] - node_ptr[a];
+        int64_t *tmp = (int64_t *)malloc((size_t)(na ? na : 1) * sizeof(int64_t));
+        memcpy(tmp, node_idx + node_ptr[a], (size_t)na * sizeof(int64_t));
+        qsort(tmp, (size_t)na, sizeof(int64_t), cmp_i64);
+        int ok = 1; for (int64_t t = 1; t < na; t++) if (tmp[t] == tmp[t - 1]) ok = 0;
+        c->atom_distinct[a] = ok; free(tmp);
+    }
     c->natoms = natoms; c->ntypes = ntypes;
     return REF_OK;
 }
@@ -471,16 +481,20 @@ int ref_apply_H(ref_ctx *c, const ref_c128 *X, ref_c128 *Y, int64_t ld, int nvec
         const ref_c128 *D = c->delta + c->delta_ptr[c->atom_type[a]];
         size_t csz = (size_t)2 * np * (nvec ? nvec : 1);
         ref_c128 *C = (ref_c128 *)calloc(csz, sizeof(ref_c128)), *Ct = (ref_c128 *)calloc(csz, sizeof(ref_c128));
-        /* C_{2X+s, v} = sum_I conj(P_{I X}) Z_{2I+s, v} */
-        for (int64_t t = 0; t < na; t++) { int64_t I = c->node_idx[n0 + t];
-            for (int x = 0; x < np; x++) { double pv = P[t * np + x];
+        /* C_{2X+s, v} = sum_I conj(P_{I X}) Z_{2I+s, v}.  (OpenMP over the projector index X: every C entry is still
+         * summed over the support nodes t in the same order by one thread, so the arithmetic is unchanged.) */
+#pragma omp parallel for schedule(static)
+        for (int x = 0; x < np; x++) {
+            for (int64_t t = 0; t < na; t++) { int64_t I = c->node_idx[n0 + t]; double pv = P[t * np + x];
                 for (int s = 0; s < 2; s++) for (int v = 0; v < nvec; v++) {
                     C[(size_t)(2 * x + s) * nvec + v].re += pv * Z[(2 * I + s) * (int64_t)nvec + v].re;
                     C[(size_t)(2 * x + s) * nvec + v].im += pv * Z[(2 * I + s) * (int64_t)nvec + v].im; } } }
         /* Ct = Delta C */
         for (int r = 0; r < 2 * np; r++) for (int q = 0; q < 2 * np; q++) { ref_c128 d = D[(size_t)r * 2 * np + q];
             for (int v = 0; v < nvec; v++) { ref_c128 t = cmul(d, C[(size_t)q * nvec + v]); Ct[(size_t)r * nvec + v].re += t.re; Ct[(size_t)r * nvec + v].im += t.im; } }
-        /* Y_{2I+s} += sum_X P_{I X} Ct_{2X+s} */
+        /* Y_{2I+s} += sum_X P_{I X} Ct_{2X+s}.  (OpenMP over the support nodes of this atom: they are distinct rows of Y,
+         * and every row still adds its projector terms X in the same order.) */
+#pragma omp parallel for schedule(static) if (c->atom_distinct[a])
         for (int64_t t = 0; t < na; t++) { int64_t I = c->node_idx[n0 + t];
             for (int x = 0; x < np; x++) { double pv = P[t * np + x];
                 for (int s = 0; s < 2; s++) for (int v = 0; v < nvec; v++) {

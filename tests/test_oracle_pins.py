@@ -340,6 +340,30 @@ def test_apply_H_rows_matches_full(cfg0_oracle):
     assert np.allclose(ctx.apply_H_rows(X, rows), Y[rows], atol=1e-12 * np.abs(Y).max())
 
 
+@pytest.mark.parametrize("bc,ncell,box,order", [((0, 0, 1), (2, 3, 4), (3.0, 4.5, 3.0), 5), ((1, 0, 1), (2, 2, 3), (2.4, 3.0, 2.1), 4)])
+def test_apply_H_rows_matches_full_on_dirichlet_noncubic_mesh(bc, ncell, box, order):
+    """ref_apply_H_rows is the oracle of the full-size GPU tests of configs 2-4 (tests/test_gpu_fullsize.py), where the global
+    CSR may not fit. Its constrained-node skip (conn < 0) and its per-row 1/sqrt(m_J) folding are pinned here against
+    ref_apply_H (itself pinned above: exactness, spectra, Hermiticity, second construction) on EVERY row of meshes that
+    have what configs 2-4 have and config 0 has not: Dirichlet faces, non-cubic cells (config 2: 1.5 x 1.5 x 0.75),
+    orders 4 and 5, atoms whose projector support is cut by the Dirichlet face and wraps around the periodic ones."""
+    cfg = synth.Config(9, "rows_pin", ncell, box, order, bc, 3, "uniform", 3, 4, 0, 4321)
+    ctx = O.RefCtx(cfg.ncell, cfg.box, cfg.order, cfg.bc)
+    s = synth.make_system(cfg, ctx.node_coords(), ctx.mass_diag())
+    ctx.set_potential(s.veff, s.bxyz)
+    ctx.set_projectors(s.node_ptr, s.node_idx, s.nproj, s.pvals, s.atom_type, s.delta, s.delta_ptr)
+    assert len(s.node_idx) > 0
+    X = synth.random_block(s.rng, 2 * ctx.M, 3)
+    Y = ctx.apply_H(X)
+    rows = np.arange(2 * ctx.M, dtype=np.int64)
+    got = ctx.apply_H_rows(X, rows)
+    err = np.linalg.norm(got - Y, axis=1) / np.linalg.norm(Y, axis=1)
+    assert float(err.max()) < 1e-12
+    # a subset in scrambled order with repeats gives the same rows
+    pick = np.array([2 * ctx.M - 1, 0, 17, 17, ctx.M, 3], dtype=np.int64)
+    assert np.array_equal(ctx.apply_H_rows(X, pick), got[pick])
+
+
 # ---------------------------------------------------------------- the filter
 def _cheb(m, x):
     x = np.asarray(x, float); out = np.empty_like(x)
