@@ -140,9 +140,10 @@ int csf_profile_read(csf_ctx* ctx, int kind, double* ms_total, int64_t* launches
  * independent DFMA chains, tflops_mma from mma.sync m8n8k4 f64 (DMMA) chains. Synchronises. Either pointer may be NULL. */
 int csf_probe_fp64_peak(int device, double* tflops_fma, double* tflops_mma);
 
-/* Which column-kernel variant a block of nvec vectors runs with in `mode` on this context: *lanes = 16 (4 vectors per CTA;
- * 8 lanes = 2 vectors at order 7) or 32 (8 vectors per CTA, orders 4 and 5). The library chooses per call by measurement
- * on B200; the environment variable CSF_LANES=16|32, read by csf_create, pins it. Host-only query. */
+/* Which column-kernel variant a block of nvec vectors runs with in `mode` on this context: *lanes = 32 (orders 4 and 5:
+ * the warp-specialised kernel, 8 vectors per CTA) or 16 (the other orders: 4 vectors per CTA; 8 lanes = 2 vectors at
+ * order 7). The environment variable CSF_LANES=16, read by csf_create, pins the 16-lane kernel at orders 4 and 5 too
+ * (parity tests run every case through both). Host-only query. */
 int csf_column_lanes(const csf_ctx* ctx, int nvec, int mode, int* lanes);
 
 /* Number of kernel launches (own kernels only, memsets excluded) enqueued by this context so far. */
@@ -151,6 +152,13 @@ int csf_launch_count(const csf_ctx* ctx, int64_t* launches);
 /* Select a kernel variant: 0 = library default; 1 = always take the general (predicated) column kernel, also on
  * fully periodic meshes where the predicate-free specialisation would be chosen (test hook). CSF_EINVAL if unknown. */
 int csf_set_variant(csf_ctx* ctx, int variant);
+
+/* Test / tuning hook for the traversal of the column kernels (no effect on results beyond summation order): seg_len =
+ * cells of a (cx, cy) column that one CTA marches through before the z-face is handed over through global memory
+ * (0 = the kernel's default: 16, or the whole column up to 64 cells for orders 4 and 5); chunk_group = vector chunks of one
+ * column scheduled back to back (>= 1, default 16). The parity tests use it to put segment boundaries, the final carry
+ * flush and multi-group grids on small meshes. CSF_EINVAL on seg_len < 0 or chunk_group < 1. */
+int csf_set_tuning(csf_ctx* ctx, int seg_len, int chunk_group);
 
 /* Text of the last error recorded on ctx (never NULL; "" if none). With ctx = NULL: last csf_create failure. */
 const char* csf_last_error(const csf_ctx* ctx);

@@ -17,7 +17,7 @@ CSF_FP64, CSF_FP32_INTERMEDIATE = 0, 1
 
 EXPORTS = ["csf_create", "csf_destroy", "csf_set_stream", "csf_num_nodes", "csf_node_coords", "csf_mass_diag", "csf_set_potential",
            "csf_set_projectors", "csf_workspace_bytes", "csf_apply_H", "csf_filter", "csf_filter_host", "csf_set_host_chunk",
-           "csf_profile_enable", "csf_profile_read", "csf_probe_fp64_peak", "csf_launch_count", "csf_column_lanes", "csf_set_variant", "csf_last_error"]
+           "csf_profile_enable", "csf_profile_read", "csf_probe_fp64_peak", "csf_launch_count", "csf_column_lanes", "csf_set_variant", "csf_set_tuning", "csf_last_error"]
 KIND_CELL, KIND_PGATHER, KIND_DELTA, KIND_AUX = 0, 1, 2, 3
 KIND_NAMES = ("cell", "proj_gather", "delta", "aux")
 
@@ -151,6 +151,9 @@ class Csf:
 
     def launch_count(self):
         n = C.c_int64(); self._chk(self._L.csf_launch_count(self._h, C.byref(n))); return int(n.value)
+
+    def set_tuning(self, seg_len=0, chunk_group=16):
+        self._chk(self._L.csf_set_tuning(self._h, C.c_int(int(seg_len)), C.c_int(int(chunk_group))))
 
     def set_variant(self, variant):
         self._chk(self._L.csf_set_variant(self._h, C.c_int(int(variant))))

@@ -10,8 +10,8 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libcsf.so")
-SOURCES = ["csf_api.cu", "csf_tables.cpp", "csf_column_p.cu"]
-HEADERS = ["csf_kernels.cuh", "csf_column.cuh", "csf_column_launch.h", "csf_tables.h", os.path.join("..", "..", "include", "csf.h")]
+SOURCES = ["csf_api.cu", "csf_tables.cpp", "csf_column_p.cu", "csf_colws_p.cu"]
+HEADERS = ["csf_kernels.cuh", "csf_column.cuh", "csf_colws.cuh", "csf_column_launch.h", "csf_tables.h", os.path.join("..", "..", "include", "csf.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "--use_fast_math=false",
               "-Xcompiler", "-fPIC", "-shared", "-Xptxas", "-v"]
 
@@ -41,6 +41,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
             (os.path.join(CSRC, "csf_tables.cpp"), os.path.join(objdir, "csf_tables.o"), [])]
     jobs += [(os.path.join(CSRC, "csf_column_p.cu"), os.path.join(objdir, f"csf_column_p{p}.o"), [f"-DCSF_P={p}"]) for p in range(1, 8)]
     jobs += [(os.path.join(CSRC, "csf_column_p.cu"), os.path.join(objdir, f"csf_column_wide_p{p}.o"), [f"-DCSF_P={p}", "-DCSF_WIDE=1"]) for p in (4, 5)]
+    jobs += [(os.path.join(CSRC, "csf_colws_p.cu"), os.path.join(objdir, f"csf_colws_p{p}.o"), [f"-DCSF_P={p}"]) for p in (4, 5)]
     with ThreadPoolExecutor(max_workers=min(12, os.cpu_count() or 2)) as ex:
         results = list(ex.map(lambda j: _run(["nvcc"] + cflags + j[2] + ["-c", j[0], "-o", j[1]]), jobs))
     log = "".join(out for _, out in results)

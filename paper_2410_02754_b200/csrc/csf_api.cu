@@ -2,6 +2,7 @@
 #include "../../include/csf.h"
 #include "csf_kernels.cuh"
 #include "csf_column.cuh"
+#include "csf_colws.cuh"
 #include "csf_column_launch.h"
 #include "csf_tables.h"
 
@@ -12,6 +13,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <new>
 #include <numeric>
 #include <string>
 #include <vector>
@@ -43,14 +45,14 @@ struct csf_ctx {
     int nfree[3]; long long M = 0; int E = 0;
     Gll1D gll; Dir1D dir[3];
     bool have_pot = false;
-    DevBuf d_cell_order, d_col_order, d_vb;
+    DevBuf d_col_order, d_vb;
     DevBuf d_sub_ptr[kColMaxAuxWarps - 1], d_sub_desc[kColMaxAuxWarps - 1], d_a_pack[kColMaxAuxWarps - 1], d_ent_locf;     // [nq - 2]: nq expansion warps per CTA
-    int seg_len = 16, chunk_group = 16;
+    int seg_len = 0, chunk_group = 16;      // cells per z-segment (0 = the kernel's default), vector chunks scheduled back to back (csf_set_tuning)
     int lanes_force = 0;                    // CSF_LANES=16|32 pins the column kernel variant (tests, sweeps); 0 = measured policy
+    int kernel_force = 0;                   // CSF_KERNEL=wide|ws pins the 8-vector kernel of orders 4 and 5 (1 | 2)
     // projectors
     int natoms = 0, npj_uniform = 0, npjp = 0; long long crows = 0;
-    DevBuf d_pair_ptr, d_pair_atom, d_pair_off, d_ent_loc, d_ent_node, d_ent_p, d_atom_coff, d_atom_npj, d_atom_type,
-        d_delta, d_delta_ptr, d_gb_atom, d_gb_beg, d_gb_end, d_gb_k0, d_g_pack;
+    DevBuf d_ent_node, d_atom_coff, d_atom_npj, d_atom_type, d_delta, d_delta_ptr, d_gb_atom, d_gb_beg, d_gb_end, d_gb_k0, d_g_pack;
     int n_gather_blocks = 0;
     int variant = 0;
     long long launches = 0;
@@ -77,6 +79,10 @@ namespace {
 int fail(csf_ctx* c, int code, const std::string& msg) { if (c) c->err = msg; else g_create_error = msg; return code; }
 int cuda_fail(csf_ctx* c, cudaError_t e, const char* what) { return fail(c, CSF_ECUDA, std::string(what) + ": " + cudaGetErrorString(e)); }
 #define CSF_CUDA(ctx, call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) return cuda_fail(ctx, e__, #call); } while (0)
+// nothing may throw across the C ABI (csf.h): every entry point that allocates host memory runs inside this guard
+#define CSF_GUARD_BEGIN try {
+#define CSF_GUARD_END(ctx) } catch (const std::bad_alloc&) { return fail(const_cast<csf_ctx*>(ctx), CSF_ENOMEM, "out of host memory"); } \
+                           catch (...) { return fail(const_cast<csf_ctx*>(ctx), CSF_ECUDA, "unexpected C++ exception"); }
 
 // brackets one kernel launch with two events when profiling is on
 struct ProfScope {
@@ -91,9 +97,12 @@ struct ProfScope {
 
 bool have_wide(int p) { return p == 4 || p == 5; }
 
-cudaError_t launch_column(int p, int ks, int mode, bool f32, bool wide, const ColParams& cp, long long nblocks, cudaStream_t s) {
-    if (wide && p == 4) return launch_column_wide_p4(ks, mode, f32, cp, nblocks, s);
-    if (wide && p == 5) return launch_column_wide_p5(ks, mode, f32, cp, nblocks, s);
+// kind: 0 = 4 vectors per CTA, 1 = 8 vectors per CTA (orders 4, 5), 2 = warp-specialised streaming kernel (orders 4, 5)
+cudaError_t launch_column(int p, int ks, int mode, bool f32, int kind, const ColParams& cp, long long nblocks, cudaStream_t s) {
+    if (kind == 2 && p == 4) return launch_column_ws_p4(ks, mode, f32, cp, (int)nblocks, s);
+    if (kind == 2 && p == 5) return launch_column_ws_p5(ks, mode, f32, cp, (int)nblocks, s);
+    if (kind == 1 && p == 4) return launch_column_wide_p4(ks, mode, f32, cp, nblocks, s);
+    if (kind == 1 && p == 5) return launch_column_wide_p5(ks, mode, f32, cp, nblocks, s);
     switch (p) {
         case 1: return launch_column_p1(ks, mode, f32, cp, nblocks, s);
         case 2: return launch_column_p2(ks, mode, f32, cp, nblocks, s);
@@ -106,9 +115,11 @@ cudaError_t launch_column(int p, int ks, int mode, bool f32, bool wide, const Co
     return cudaErrorInvalidValue;
 }
 
-ColInfo column_info(int p, bool wide) {
-    if (wide && p == 4) return column_info_wide_p4();
-    if (wide && p == 5) return column_info_wide_p5();
+ColInfo column_info(int p, int kind) {
+    if (kind == 2 && p == 4) return column_info_ws_p4();
+    if (kind == 2 && p == 5) return column_info_ws_p5();
+    if (kind == 1 && p == 4) return column_info_wide_p4();
+    if (kind == 1 && p == 5) return column_info_wide_p5();
     switch (p) {
         case 1: return column_info_p1(); case 2: return column_info_p2(); case 3: return column_info_p3(); case 4: return column_info_p4();
         case 5: return column_info_p5(); case 6: return column_info_p6(); default: return column_info_p7();
@@ -146,27 +157,28 @@ size_t f32_block_bytes(const csf_ctx* c, int nvec);
 int column_mode(const csf_ctx* c, int nvec, int vpc, bool f32) {
     if (!(c->bc[0] == CSF_BC_PERIODIC && c->bc[1] == CSF_BC_PERIODIC && nvec % vpc == 0 && c->variant != 1)) return 0;
     const bool cubic = c->h[0] * c->h[0] / (c->h[1] * c->h[1]) == 1.0 && c->h[0] * c->h[0] / (c->h[2] * c->h[2]) == 1.0;
-    // mode 1 measured slower than 0 for the narrow FP64 kernel, faster for the wide one (config 2: 42.2 -> 36.0 ms per launch)
+    // mode 1 measured slower than 0 for the narrow FP64 kernel
     return (c->bc[2] == CSF_BC_PERIODIC && cubic) ? 2 : ((f32 || vpc == 8) ? 1 : 0);
 }
 
-// Which column kernel runs: the wide one (8 vectors per CTA) where it measured faster on B200 — order 4 (FP64 config 4:
-// 44.8 -> 39.8 ms per launch, config 1: 0.56 -> 0.47; FP32 config 4: 33.5 -> 30.8, config 1: 0.41 -> 0.36), order 5 in FP64
-// (config 3: 41.3 -> 38.1, config 2: 43.4 -> 36.0 with mode 1) and the FP32 variant of order 5 off the fully periodic
-// cubic mode (config 2: 31.0 -> 24.6; config 3 stays narrow: 30.8 against 31.3).
-bool wide_possible(const csf_ctx* c, bool f32, int mode) { return c->p == 4 || (c->p == 5 && (!f32 || mode != 2)); }
-bool use_wide(const csf_ctx* c, int nvec, bool f32) {
-    if (!have_wide(c->p) || c->lanes_force == 16) return false;
-    if (c->lanes_force == 32) return true;
-    return wide_possible(c, f32, column_mode(c, nvec, column_info(c->p, true).lanes / 4, f32));
+// Which column kernel runs (kind): orders 4 and 5 take a kernel with 8 vectors per CTA — the cell-per-iteration kernel
+// (kind 1, csf_column.cuh) or the warp-specialised streaming kernel (kind 2, csf_colws.cuh) —, the other orders the
+// cell-per-iteration kernel with 4 vectors per CTA (kind 0). CSF_LANES=16 pins kind 0, CSF_KERNEL=ws|wide pins 2 | 1 (tests, sweeps).
+int column_kind(const csf_ctx* c) {
+    if (!have_wide(c->p) || c->lanes_force == 16) return 0;
+    const bool ws_ok = c->ncell[0] < 32768 && c->ncell[1] < 32768;       // (the kernel packs cx, cy into 16 bits each)
+    if (c->kernel_force == 2 && ws_ok) return 2;
+    if (c->kernel_force == 1) return 1;
+    return 1;
 }
+int aux_warps(const csf_ctx* c, bool f32, int mode, int kind) { return kind == 2 ? kWsRoleWarps : col_aux_warps(c->p, f32, mode, kind == 1 ? 32 : 16); }
 
 // one step: dst += sc * i^rot * (Hhat - shift) src
 // src, dst: complex128 blocks, or complex64 blocks when f32 (CSF_FP32_INTERMEDIATE)
 int enqueue_step(csf_ctx* c, const void* src, long long ld, void* dst, long long ld_dst, int nvec, double sc, int rot, double shift,
                  double* dC, double* dCt, bool f32 = false) {
     const long long ldc = nvec;
-    const bool wide = use_wide(c, nvec, f32);
+    const int kind = column_kind(c); const bool ws = kind == 2;
     if (c->natoms > 0) {
         CSF_CUDA(c, cudaMemsetAsync(dC, 0, (size_t)c->crows * ldc * sizeof(double2), c->stream));
         GatherParams gp{};
@@ -184,10 +196,11 @@ int enqueue_step(csf_ctx* c, const void* src, long long ld, void* dst, long long
         }
         CSF_CUDA(c, cudaGetLastError());
         DeltaParams dp{};
-        const int lanes = column_info(c->p, wide).lanes, nchunks = (nvec + lanes / 4 - 1) / (lanes / 4);
+        const int lanes = column_info(c->p, kind).lanes, nchunks = (nvec + lanes / 4 - 1) / (lanes / 4);
         CSF_CUDA(c, cudaMemsetAsync(dCt, 0, ctp_bytes(c, nvec), c->stream));
         dp.C = reinterpret_cast<const double2*>(dC); dp.Ct = dCt; dp.ldc = ldc; dp.nvec = nvec;
         dp.lanes = lanes; dp.ks = c->npjp / 4; dp.nchunks = nchunks;
+        dp.scale = ws ? sc : 1.0;          // the streaming kernel accumulates sc * (P~ C~) straight into its X tile
         dp.atom_coff = c->d_atom_coff.as<long long>(); dp.atom_npj = c->d_atom_npj.as<int>(); dp.atom_type = c->d_atom_type.as<int>();
         dp.delta = c->d_delta.as<double2>(); dp.delta_ptr = c->d_delta_ptr.as<long long>();
         dim3 dg(c->natoms, (nvec + 31) / 32);
@@ -196,7 +209,7 @@ int enqueue_step(csf_ctx* c, const void* src, long long ld, void* dst, long long
         c->launches += 2;
     }
     {
-        const ColInfo ci = column_info(c->p, wide);
+        const ColInfo ci = column_info(c->p, kind);
         if (ci.smem > c->smem_optin) return fail(c, CSF_EUNSUPPORTED, "column tile does not fit shared memory");
         if (4 * ld >= (1LL << 31) || 4 * ld_dst >= (1LL << 31)) return fail(c, CSF_EUNSUPPORTED, "leading dimension too large");
         const int vpc = ci.lanes / 4;               // spinor vectors per CTA
@@ -227,22 +240,36 @@ int enqueue_step(csf_ctx* c, const void* src, long long ld, void* dst, long long
         q.nfx = c->nfree[0]; q.nfy = c->nfree[1]; q.nfz = c->nfree[2];
         q.bcx = c->bc[0]; q.bcy = c->bc[1]; q.bcz = c->bc[2];
         q.col_order = c->d_col_order.as<int>(); q.ncols = c->ncell[0] * c->ncell[1];
-        q.seg_len = std::min(c->seg_len, c->ncell[2]); q.nseg = (c->ncell[2] + q.seg_len - 1) / q.seg_len;
+        // cells per z-segment: the warp-specialised kernel streams whole columns (up to 64 cells) through one CTA
+        q.seg_len = std::min(c->seg_len > 0 ? c->seg_len : (ws ? 64 : 16), c->ncell[2]); q.nseg = (c->ncell[2] + q.seg_len - 1) / q.seg_len;
         q.nchunks = (nvec + vpc - 1) / vpc; q.chunk_group = std::min(c->chunk_group, q.nchunks);
         q.vb = c->d_vb.as<double>(); q.shift = shift; q.sc = sc; q.rot = rot & 3;
+#ifdef WS_PROF
+        {   // cycle counters of the last launch: [CTA][12 warps][4], dumped to CSF_WS_PROF_FILE by the previous launch's data
+            static long long* dprof = nullptr; static std::vector<long long> hprof(148 * 12 * 4);
+            if (!dprof) cudaMalloc(&dprof, hprof.size() * 8);
+            else if (const char* f = std::getenv("CSF_WS_PROF_FILE")) {
+                cudaStreamSynchronize(c->stream); cudaMemcpy(hprof.data(), dprof, hprof.size() * 8, cudaMemcpyDeviceToHost);
+                if (FILE* fp = std::fopen(f, "w")) { for (size_t i = 0; i < hprof.size(); i += 4) std::fprintf(fp, "%lld %lld %lld %lld\n", hprof[i], hprof[i + 1], hprof[i + 2], hprof[i + 3]); std::fclose(fp); }
+            }
+            cudaMemsetAsync(dprof, 0, hprof.size() * 8, c->stream);
+            q.prof = dprof;
+        }
+#endif
         const int kmode = column_mode(c, nvec, vpc, f32);
-        const int lv = col_aux_warps(c->p, f32, kmode, ci.lanes) - 2;      // which sub-pair lists match the kernel's expansion-warp count
+        const int lv = aux_warps(c, f32, kmode, kind) - 2;      // which sub-pair lists match the kernel's expansion-warp count
         if (c->natoms > 0) {
             q.sub_ptr = c->d_sub_ptr[lv].as<int>(); q.sub_desc = c->d_sub_desc[lv].as<int4>();
-            q.ent_loc = c->d_ent_locf.as<int>(); q.ent_p = c->d_ent_p.as<double>();
+            q.ent_loc = c->d_ent_locf.as<int>();
             q.Ct = dCt; q.npjp = c->npjp; q.a_pack = c->d_a_pack[lv].as<double>();
         }
         const long long ngroups = (q.nchunks + q.chunk_group - 1) / q.chunk_group;
-        const long long nblocks = (long long)q.chunk_group * q.ncols * q.nseg * ngroups;
-        if (nblocks > 0x7fffffffLL) return fail(c, CSF_EUNSUPPORTED, "grid too large");
+        long long nblocks = (long long)q.chunk_group * q.ncols * q.nseg * ngroups;
+        if (nblocks > 0x7fffffffLL || (long long)q.nchunks * q.ncols * q.nseg > 0x7fffffffLL) return fail(c, CSF_EUNSUPPORTED, "grid too large");
+        if (ws) nblocks = std::min<long long>((long long)q.nchunks * q.ncols * q.nseg, c->sm_count);      // persistent CTAs, one per SM
         {
             ProfScope ps(c, CSF_KIND_CELL);
-            CSF_CUDA(c, launch_column(c->p, c->natoms > 0 ? c->npjp / 4 : 5, kmode, f32, wide, q, nblocks, c->stream));
+            CSF_CUDA(c, launch_column(c->p, c->natoms > 0 ? c->npjp / 4 : 5, kmode, f32, kind, q, nblocks, c->stream));
         }
         c->launches += 1;
         return CSF_OK;
@@ -288,6 +315,7 @@ extern "C" {
 const char* csf_last_error(const csf_ctx* ctx) { return ctx ? ctx->err.c_str() : g_create_error.c_str(); }
 
 int csf_create(csf_ctx** out, const int ncell[3], const double box[3], int order, const int bc[3], int device, void* cuda_stream) {
+    CSF_GUARD_BEGIN
     if (!out || !ncell || !box || !bc) return fail(nullptr, CSF_EINVAL, "NULL argument");
     *out = nullptr;
     if (order < 1) return fail(nullptr, CSF_EINVAL, "order must be >= 1");
@@ -310,6 +338,7 @@ int csf_create(csf_ctx** out, const int ncell[3], const double box[3], int order
     if (ce != cudaSuccess) return cuda_fail(nullptr, ce, "cudaSetDevice");
     csf_ctx* c = new (std::nothrow) csf_ctx();
     if (!c) return fail(nullptr, CSF_ENOMEM, "out of host memory");
+    struct Owner { csf_ctx* p; ~Owner() { delete p; } } owner{c};        // released on success
     c->device = device; c->stream = static_cast<cudaStream_t>(cuda_stream);
     c->p = order; c->n = order + 1; c->M = M; c->E = (int)E;
     for (int d = 0; d < 3; ++d) {
@@ -320,30 +349,23 @@ int csf_create(csf_ctx** out, const int ncell[3], const double box[3], int order
     for (int d = 0; d < 3; ++d) build_dir(c->gll, c->h[d], &c->dir[d]);
     cudaDeviceProp prop;
     ce = cudaGetDeviceProperties(&prop, device);
-    if (ce != cudaSuccess) { delete c; return cuda_fail(nullptr, ce, "cudaGetDeviceProperties"); }
+    if (ce != cudaSuccess) return cuda_fail(nullptr, ce, "cudaGetDeviceProperties");
     c->sm_count = prop.multiProcessorCount; c->smem_optin = prop.sharedMemPerBlockOptin;
-    // tuning hooks for sweeps (defaults are the measured best on B200): cells per z-segment, vector chunks per group
-    if (const char* e = std::getenv("CSF_SEG_LEN")) { int v = std::atoi(e); if (v >= 1) c->seg_len = v; }
+    // CSF_LANES pins the column kernel variant for the parity tests (both variants against the oracle on every case)
     if (const char* e = std::getenv("CSF_LANES")) { int v = std::atoi(e); if (v == 16 || v == 32) c->lanes_force = v; }
-    if (const char* e = std::getenv("CSF_CHUNK_GROUP")) { int v = std::atoi(e); if (v >= 1) c->chunk_group = v; }
-    // traversal order of the cells: 8x8x8 bricks, x fastest inside, so that the faces shared between
-    // neighbouring cells are combined in L2 before they are evicted
-    std::vector<int> order_v; order_v.reserve(E);
+    if (const char* e = std::getenv("CSF_KERNEL")) c->kernel_force = std::strcmp(e, "ws") == 0 ? 2 : (std::strcmp(e, "wide") == 0 ? 1 : 0);
     const int B = 8;
-    for (int bz = 0; bz < ncell[2]; bz += B) for (int by = 0; by < ncell[1]; by += B) for (int bx = 0; bx < ncell[0]; bx += B)
-        for (int z = bz; z < std::min(bz + B, ncell[2]); ++z) for (int y = by; y < std::min(by + B, ncell[1]); ++y)
-            for (int x = bx; x < std::min(bx + B, ncell[0]); ++x) order_v.push_back(x + ncell[0] * (y + ncell[1] * z));
-    ce = c->d_cell_order.upload(order_v);
-    if (ce != cudaSuccess) { delete c; return cuda_fail(nullptr, ce, "upload cell order"); }
     // traversal order of the (cx, cy) columns: 8x8 tiles, x fastest inside (neighbouring columns run together, so the
     // x / y faces they share are combined in L2)
     std::vector<int> col_v; col_v.reserve((size_t)ncell[0] * ncell[1]);
     for (int by = 0; by < ncell[1]; by += B) for (int bx = 0; bx < ncell[0]; bx += B)
         for (int y = by; y < std::min(by + B, ncell[1]); ++y) for (int x = bx; x < std::min(bx + B, ncell[0]); ++x) col_v.push_back(x + ncell[0] * y);
     ce = c->d_col_order.upload(col_v);
-    if (ce != cudaSuccess) { delete c; return cuda_fail(nullptr, ce, "upload column order"); }
+    if (ce != cudaSuccess) return cuda_fail(nullptr, ce, "upload column order");
+    owner.p = nullptr;
     *out = c;
     return CSF_OK;
+    CSF_GUARD_END((csf_ctx*)nullptr)
 }
 
 int csf_destroy(csf_ctx* ctx) {
@@ -372,6 +394,7 @@ static void axis_tables(const csf_ctx* c, int d, std::vector<double>* x, std::ve
 }
 
 int csf_node_coords(const csf_ctx* ctx, double* xyz) {
+    CSF_GUARD_BEGIN
     if (!ctx || !xyz) return CSF_EINVAL;
     std::vector<double> ax[3], am[3];
     for (int d = 0; d < 3; ++d) axis_tables(ctx, d, &ax[d], &am[d]);
@@ -380,9 +403,11 @@ int csf_node_coords(const csf_ctx* ctx, double* xyz) {
         xyz[3 * I] = ax[0][x]; xyz[3 * I + 1] = ax[1][y]; xyz[3 * I + 2] = ax[2][z];
     }
     return CSF_OK;
+    CSF_GUARD_END(ctx)
 }
 
 int csf_mass_diag(const csf_ctx* ctx, double* mh) {
+    CSF_GUARD_BEGIN
     if (!ctx || !mh) return CSF_EINVAL;
     std::vector<double> ax[3], am[3];
     for (int d = 0; d < 3; ++d) axis_tables(ctx, d, &ax[d], &am[d]);
@@ -390,9 +415,11 @@ int csf_mass_diag(const csf_ctx* ctx, double* mh) {
     for (int z = 0; z < ctx->nfree[2]; ++z) for (int y = 0; y < ctx->nfree[1]; ++y) for (int x = 0; x < ctx->nfree[0]; ++x, ++I)
         mh[I] = am[0][x] * am[1][y] * am[2][z];
     return CSF_OK;
+    CSF_GUARD_END(ctx)
 }
 
 int csf_set_potential(csf_ctx* c, const double* veff, const double* bxyz) {
+    CSF_GUARD_BEGIN
     if (!c) return CSF_EINVAL;
     if (!veff) return fail(c, CSF_EINVAL, "veff is NULL");
     CSF_CUDA(c, cudaSetDevice(c->device));
@@ -405,10 +432,12 @@ int csf_set_potential(csf_ctx* c, const double* veff, const double* bxyz) {
     CSF_CUDA(c, c->d_vb.upload(vb));
     c->have_pot = true;
     return CSF_OK;
+    CSF_GUARD_END(c)
 }
 
 int csf_set_projectors(csf_ctx* c, int natoms, const int64_t* node_ptr, const int64_t* node_idx, const int* nproj,
                        const double* pvals, const int* atom_type, int ntypes, const csf_c128* delta, const int64_t* delta_ptr) {
+    CSF_GUARD_BEGIN
     if (!c) return CSF_EINVAL;
     if (natoms < 0) return fail(c, CSF_EINVAL, "natoms < 0");
     CSF_CUDA(c, cudaSetDevice(c->device));
@@ -433,7 +462,7 @@ int csf_set_projectors(csf_ctx* c, int natoms, const int64_t* node_ptr, const in
     csf_mass_diag(c, mass.data());
     // owner cell and local index of every support node; sort each atom's entries by (cell, lz, ly, lx)
     struct Ent { int cell, lz, ly, lx; long long t; };
-    std::vector<int> ent_node((size_t)nent), ent_loc((size_t)nent), ent_locf((size_t)nent);
+    std::vector<int> ent_node((size_t)nent), ent_locf((size_t)nent);
     std::vector<double> ent_p((size_t)nent * npjp, 0.0);
     std::vector<long long> atom_coff(natoms); std::vector<int> atom_npj(nproj, nproj + natoms), atom_ty(atom_type, atom_type + natoms);
     std::vector<int> gb_atom, gb_beg, gb_end;
@@ -458,7 +487,7 @@ int csf_set_projectors(csf_ctx* c, int natoms, const int64_t* node_ptr, const in
                 return fail(c, CSF_EINVAL, "duplicate node in an atom's support");
         for (size_t q = 0; q < ents.size(); ++q) {
             const long long e = t0 + (long long)q, t = ents[q].t, I = node_idx[t];
-            ent_node[e] = (int)I; ent_loc[e] = ents[q].ly * p + ents[q].lx; ent_locf[e] = (ents[q].lz * p + ents[q].ly) * p + ents[q].lx;
+            ent_node[e] = (int)I; ent_locf[e] = (ents[q].lz * p + ents[q].ly) * p + ents[q].lx;
             const double s = 1.0 / std::sqrt(mass[I]);
             for (int x = 0; x < nproj[a]; ++x) ent_p[(size_t)e * npjp + x] = s * pvals[pv_off + (t - t0) * nproj[a] + x];
             if (q == 0 || ents[q].cell != ents[q - 1].cell) {
@@ -486,27 +515,13 @@ int csf_set_projectors(csf_ctx* c, int natoms, const int64_t* node_ptr, const in
             const size_t kstep = (size_t)atom_k0[a] + (e - node_ptr[a]) / 4; const int kq = (int)((e - node_ptr[a]) % 4);
             for (int x = 0; x < nproj[a]; ++x) g_pack[(kstep * mt + x / 8) * 32 + (x % 8) * 4 + kq] = ent_p[(size_t)e * npjp + x];
         }
-    // cell-major pair lists
-    std::vector<int> pair_ptr(c->E + 1, 0);
-    for (const Pair& pr : pairs) pair_ptr[pr.cell + 1]++;
-    for (int e = 0; e < c->E; ++e) pair_ptr[e + 1] += pair_ptr[e];
-    std::vector<int> fill(pair_ptr.begin(), pair_ptr.end() - 1), pair_atom(pairs.size()), pair_off(pairs.size() * (p + 1));
-    for (const Pair& pr : pairs) {
-        int s = fill[pr.cell]++; pair_atom[s] = pr.atom;
-        for (int k = 0; k <= p; ++k) pair_off[(size_t)s * (p + 1) + k] = pr.off[k];
-    }
-    // sub-pairs for the column kernel: every (cell, atom) pair split at the owned-node index XSPLIT = ceil(p^3 / 2)
-    // (entries of a pair are sorted by that index), grouped by (cell, half)
+    // sub-pairs for the column kernels: every (cell, atom) pair split into the owned-node row ranges of the nq expansion
+    // warps (entries of a pair are sorted by that index), grouped by (cell, warp)
     if (crows >= (1LL << 31)) return fail(c, CSF_EUNSUPPORTED, "too many projector rows");
     for (int lv = 0; lv < kColMaxAuxWarps - 1; ++lv) {
     const int nq = 2 + lv;
-    bool used = false;                          // does any kernel of this order and lane count run nq expansion warps?
-    for (int w = 0; w < 2; ++w) {
-        if ((w == 1 && (!have_wide(p) || c->lanes_force == 16)) || (w == 0 && have_wide(p) && c->lanes_force == 32)) continue;
-        for (int f = 0; f < 2; ++f) for (int md = 0; md < 3; ++md)
-            if (c->lanes_force != 0 || !have_wide(p) || wide_possible(c, f != 0, md) == (w == 1))
-                used = used || col_aux_warps(p, f != 0, md, column_info(p, w != 0).lanes) == nq;
-    }
+    bool used = false;                          // does any kernel this context can run have nq expansion warps?
+    for (int f = 0; f < 2; ++f) for (int md = 0; md < 3; ++md) used = used || aux_warps(c, f != 0, md, column_kind(c)) == nq;
     if (!used) continue;
     struct Sub { int key; int4 d; };
     std::vector<Sub> subs; subs.reserve(nq * pairs.size());
@@ -542,15 +557,14 @@ int csf_set_projectors(csf_ctx* c, int natoms, const int64_t* node_ptr, const in
     std::vector<double2> dl((size_t)delta_ptr[ntypes]);
     for (size_t i = 0; i < dl.size(); ++i) dl[i] = make_double2(delta[i].re, delta[i].im);
     std::vector<long long> dptr(delta_ptr, delta_ptr + ntypes + 1);
-    CSF_CUDA(c, c->d_pair_ptr.upload(pair_ptr)); CSF_CUDA(c, c->d_pair_atom.upload(pair_atom)); CSF_CUDA(c, c->d_pair_off.upload(pair_off));
-    CSF_CUDA(c, c->d_ent_locf.upload(ent_locf));
-    CSF_CUDA(c, c->d_ent_loc.upload(ent_loc)); CSF_CUDA(c, c->d_ent_node.upload(ent_node)); CSF_CUDA(c, c->d_ent_p.upload(ent_p));
+    CSF_CUDA(c, c->d_ent_locf.upload(ent_locf)); CSF_CUDA(c, c->d_ent_node.upload(ent_node));
     CSF_CUDA(c, c->d_atom_coff.upload(atom_coff)); CSF_CUDA(c, c->d_atom_npj.upload(atom_npj)); CSF_CUDA(c, c->d_atom_type.upload(atom_ty));
     CSF_CUDA(c, c->d_delta.upload(dl)); CSF_CUDA(c, c->d_delta_ptr.upload(dptr));
     CSF_CUDA(c, c->d_gb_k0.upload(gb_k0)); CSF_CUDA(c, c->d_g_pack.upload(g_pack)); CSF_CUDA(c, c->d_gb_atom.upload(gb_atom)); CSF_CUDA(c, c->d_gb_beg.upload(gb_beg)); CSF_CUDA(c, c->d_gb_end.upload(gb_end));
     c->natoms = natoms; c->crows = crows; c->npjp = npjp; c->npj_uniform = uniform ? nproj[0] : 0;
     c->n_gather_blocks = (int)gb_atom.size();
     return CSF_OK;
+    CSF_GUARD_END(c)
 }
 
 int csf_workspace_bytes(const csf_ctx* c, int nvec, int mode, size_t* bytes) {
@@ -566,6 +580,7 @@ int csf_workspace_bytes(const csf_ctx* c, int nvec, int mode, size_t* bytes) {
 }
 
 int csf_apply_H(csf_ctx* c, const csf_c128* dX, csf_c128* dY, int64_t ld, int nvec, void* d_work, size_t work_bytes) {
+    CSF_GUARD_BEGIN
     if (!c) return CSF_EINVAL;
     const size_t need = c->natoms > 0 ? coef_bytes(c, std::max(nvec, 0)) + ctp_bytes(c, std::max(nvec, 0)) : 0;
     int rc = check_block_args(c, dX, dY, ld, nvec, d_work, work_bytes, need);
@@ -576,10 +591,12 @@ int csf_apply_H(csf_ctx* c, const csf_c128* dX, csf_c128* dY, int64_t ld, int nv
     rc = enqueue_zero(c, reinterpret_cast<double*>(dY), ld, nvec);
     if (rc != CSF_OK) return rc;
     return enqueue_step(c, reinterpret_cast<const double*>(dX), ld, reinterpret_cast<double*>(dY), ld, nvec, 1.0, 0, 0.0, dC, dCt);
+    CSF_GUARD_END(c)
 }
 
 int csf_filter(csf_ctx* c, const csf_c128* dX, csf_c128* dY, int64_t ld, int nvec, int degree, double a, double b, int mode,
                void* d_work, size_t work_bytes) {
+    CSF_GUARD_BEGIN
     if (!c) return CSF_EINVAL;
     if (mode != CSF_FP64 && mode != CSF_FP32_INTERMEDIATE) return fail(c, CSF_EINVAL, "unknown mode");
     if (degree < 0) return fail(c, CSF_EINVAL, "degree < 0");
@@ -642,9 +659,11 @@ int csf_filter(csf_ctx* c, const csf_c128* dX, csf_c128* dY, int64_t ld, int nve
         if (rc != CSF_OK) return rc;
     }
     return CSF_OK;
+    CSF_GUARD_END(c)
 }
 
 int csf_filter_host(csf_ctx* c, const csf_c128* hX, csf_c128* hY, int64_t ld, int nvec, int degree, double a, double b, int mode) {
+    CSF_GUARD_BEGIN
     if (!c) return CSF_EINVAL;
     if (!hX || !hY) return fail(c, CSF_EINVAL, "NULL host block pointer");
     if (nvec < 0 || ld < nvec) return fail(c, CSF_EINVAL, "need 0 <= nvec <= ld");
@@ -674,25 +693,30 @@ int csf_filter_host(csf_ctx* c, const csf_c128* hX, csf_c128* hY, int64_t ld, in
     }
     // chunk i: host->device on hs_in, filter on the context's stream, device->host on hs_out; slot i%2 is reused
     // only after chunk i-2 has been filtered (x slot) and copied out (y slot), so copies overlap the filter.
+    // an error inside the pipeline must not return while copies into the caller's host memory are in flight
+    auto drain = [&]() { cudaStreamSynchronize(c->hs_in); cudaStreamSynchronize(c->stream); cudaStreamSynchronize(c->hs_out); };
+#define CSF_CUDA_H(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) { drain(); return cuda_fail(c, e__, #call); } } while (0)
     for (int i = 0; i < nch; ++i) {
         const int s = i & 1, v0 = i * chunk, nv = std::min(chunk, nvec - v0);
         const size_t wbytes = (size_t)nv * sizeof(double2);
-        if (i >= 2) CSF_CUDA(c, cudaStreamWaitEvent(c->hs_in, c->ev_cmp[s], 0));
-        CSF_CUDA(c, cudaMemcpy2DAsync(c->h_x[s].p, wbytes, hX + v0, (size_t)ld * sizeof(double2), wbytes, rows, cudaMemcpyHostToDevice, c->hs_in));
-        CSF_CUDA(c, cudaEventRecord(c->ev_in[s], c->hs_in));
-        CSF_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_in[s], 0));
-        if (i >= 2) CSF_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_out[s], 0));
+        if (i >= 2) CSF_CUDA_H(cudaStreamWaitEvent(c->hs_in, c->ev_cmp[s], 0));
+        CSF_CUDA_H(cudaMemcpy2DAsync(c->h_x[s].p, wbytes, hX + v0, (size_t)ld * sizeof(double2), wbytes, rows, cudaMemcpyHostToDevice, c->hs_in));
+        CSF_CUDA_H(cudaEventRecord(c->ev_in[s], c->hs_in));
+        CSF_CUDA_H(cudaStreamWaitEvent(c->stream, c->ev_in[s], 0));
+        if (i >= 2) CSF_CUDA_H(cudaStreamWaitEvent(c->stream, c->ev_out[s], 0));
         rc = csf_filter(c, static_cast<const csf_c128*>(c->h_x[s].p), static_cast<csf_c128*>(c->h_y[s].p), nv, nv, degree, a, b, mode, c->h_w.p, c->h_w.bytes);
-        if (rc != CSF_OK) { cudaDeviceSynchronize(); return rc; }
-        CSF_CUDA(c, cudaEventRecord(c->ev_cmp[s], c->stream));
-        CSF_CUDA(c, cudaStreamWaitEvent(c->hs_out, c->ev_cmp[s], 0));
-        CSF_CUDA(c, cudaMemcpy2DAsync(hY + v0, (size_t)ld * sizeof(double2), c->h_y[s].p, wbytes, wbytes, rows, cudaMemcpyDeviceToHost, c->hs_out));
-        CSF_CUDA(c, cudaEventRecord(c->ev_out[s], c->hs_out));
+        if (rc != CSF_OK) { drain(); return rc; }
+        CSF_CUDA_H(cudaEventRecord(c->ev_cmp[s], c->stream));
+        CSF_CUDA_H(cudaStreamWaitEvent(c->hs_out, c->ev_cmp[s], 0));
+        CSF_CUDA_H(cudaMemcpy2DAsync(hY + v0, (size_t)ld * sizeof(double2), c->h_y[s].p, wbytes, wbytes, rows, cudaMemcpyDeviceToHost, c->hs_out));
+        CSF_CUDA_H(cudaEventRecord(c->ev_out[s], c->hs_out));
     }
+#undef CSF_CUDA_H
     CSF_CUDA(c, cudaStreamSynchronize(c->hs_out));
     CSF_CUDA(c, cudaStreamSynchronize(c->stream));
     CSF_CUDA(c, cudaStreamSynchronize(c->hs_in));
     return CSF_OK;
+    CSF_GUARD_END(c)
 }
 
 int csf_set_host_chunk(csf_ctx* c, int ncols) {
@@ -705,6 +729,7 @@ int csf_set_host_chunk(csf_ctx* c, int ncols) {
 int csf_profile_enable(csf_ctx* c, int on) { if (!c) return CSF_EINVAL; c->prof = on != 0; return CSF_OK; }
 
 int csf_profile_read(csf_ctx* c, int kind, double* ms_total, int64_t* launches) {
+    CSF_GUARD_BEGIN
     if (!c || kind < 0 || kind >= CSF_NKINDS) return CSF_EINVAL;
     CSF_CUDA(c, cudaSetDevice(c->device));
     CSF_CUDA(c, cudaStreamSynchronize(c->stream));
@@ -718,6 +743,7 @@ int csf_profile_read(csf_ctx* c, int kind, double* ms_total, int64_t* launches) 
     if (launches) *launches = (int64_t)c->prof_ev[kind].size();
     c->prof_ev[kind].clear();
     return CSF_OK;
+    CSF_GUARD_END(c)
 }
 
 int csf_probe_fp64_peak(int device, double* tflops_fma, double* tflops_mma) {
@@ -755,11 +781,18 @@ int csf_probe_fp64_peak(int device, double* tflops_fma, double* tflops_mma) {
 int csf_column_lanes(const csf_ctx* c, int nvec, int mode, int* lanes) {
     if (!c || !lanes || nvec < 1 || (mode != CSF_FP64 && mode != CSF_FP32_INTERMEDIATE)) return CSF_EINVAL;
     const bool f32 = mode == CSF_FP32_INTERMEDIATE;
-    *lanes = column_info(c->p, use_wide(c, nvec, f32)).lanes;
+    *lanes = column_info(c->p, column_kind(c)).lanes;
     return CSF_OK;
 }
 
 int csf_launch_count(const csf_ctx* c, int64_t* launches) { if (!c || !launches) return CSF_EINVAL; *launches = c->launches; return CSF_OK; }
+
+int csf_set_tuning(csf_ctx* c, int seg_len, int chunk_group) {
+    if (!c) return CSF_EINVAL;
+    if (seg_len < 0 || chunk_group < 1) return fail(c, CSF_EINVAL, "need seg_len >= 0 and chunk_group >= 1");
+    c->seg_len = seg_len; c->chunk_group = chunk_group;
+    return CSF_OK;
+}
 
 int csf_set_variant(csf_ctx* c, int variant) {
     if (!c) return CSF_EINVAL;

@@ -90,9 +90,9 @@ struct ColParams {
     const int4* sub_desc;                // [nsub] {atom, first tile in a_pack, entry begin, entry end}
     const double* a_pack;                // [ntiles][KS][32] P~ in DMMA A-fragment order (lane = row*4 + k), zero padded
     const int* ent_loc;                  // [nent] local owned index (lz*p + ly)*p + lx
-    const double* ent_p;                 // [nent][npjp] S_I P_{I chi}, zero padded
     const double* Ct;                    // C~ in B-fragment order: [atom][chunk][KS][L/8][32] (DeltaParams)
     int npjp;
+    long long* prof;                     // WS_PROF builds of csf_colws.cuh: per (CTA, warp) cycle counters
 };
 
 __device__ __forceinline__ double col_flip(double x, unsigned mask) {

@@ -24,13 +24,17 @@ constexpr int kLanes = CSF_P <= 6 ? 16 : 8;      // order 7 does not fit shared 
 
 template <typename T, int KS, int MODE>
 cudaError_t launch_t(const ColParams& cp, long long nblocks, cudaStream_t s) {
-    static bool configured = false;
+    // the opt-in to > 48 KB of dynamic shared memory belongs to the device's context: remember it per device
+    static bool configured[64] = {};
     auto kern = column_kernel<T, CSF_P, KS, MODE, kLanes>;
     using Cfg = ColCfg<T, CSF_P, kLanes, col_aux_warps(CSF_P, sizeof(T) == 4, MODE, kLanes)>;
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM);
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= 64 || !configured[dev]) {
+        e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM);
         if (e != cudaSuccess) return e;
-        configured = true;
+        if (dev >= 0 && dev < 64) configured[dev] = true;
     }
     kern<<<(unsigned)nblocks, Cfg::NT, Cfg::SMEM, s>>>(cp);
     return cudaGetLastError();

@@ -145,6 +145,7 @@ struct DeltaParams {
     // real lane nt*8 + rw = spin*(L/2) + 2*(vector % VPC) + ri; rows chi >= n_pj stay zero (the buffer is cleared).
     const double2* C; double* Ct; long long ldc; int nvec;
     int lanes, ks, nchunks;
+    double scale;                 // C~ is stored times this factor (1, or the step's sc for the warp-specialised column kernel)
     const long long* atom_coff; const int* atom_npj; const int* atom_type;
     const double2* delta; const long long* delta_ptr;
 };
@@ -167,7 +168,7 @@ __global__ void __launch_bounds__(256) delta_apply_kernel(const __grid_constant_
         const int chi = r >> 1, spin = r & 1, vpc = A.lanes / 4;
         const int dl = spin * (A.lanes / 2) + (v % vpc) * 2;
         double* o = A.Ct + ((((long long)atom * A.nchunks + v / vpc) * A.ks + (chi >> 2)) * (A.lanes / 8) + (dl >> 3)) * 32 + (dl & 7) * 4 + (chi & 3);
-        o[0] = sr; o[4] = si;
+        o[0] = A.scale * sr; o[4] = A.scale * si;
     }
 }
 

@@ -8,6 +8,21 @@ def rel_fro(y, yref):
     return float(np.linalg.norm(y - yref) / max(np.linalg.norm(yref), 1e-300))
 
 
+def col_err_max(y, yref):
+    """Largest per-column relative 2-norm error (SURVEY 8(c) "also report the per-column maximum"): after Chebyshev
+    amplification a wrong weakly-amplified column would hide under the strongly-amplified ones in the block norm."""
+    num = np.linalg.norm(y - yref, axis=0); den = np.maximum(np.linalg.norm(yref, axis=0), 1e-300)
+    return float((num / den).max())
+
+
+def assert_block_close(y, yref, tol, col_tol=None):
+    """Block Frobenius error < tol (BASELINE.json's metric) and every column on its own < col_tol (default 10 tol)."""
+    e = rel_fro(y, yref); ec = col_err_max(y, yref)
+    assert e < tol, f"relative Frobenius error {e:.3e} >= {tol:.1e}"
+    assert ec < (col_tol if col_tol is not None else 10 * tol), f"per-column maximum error {ec:.3e}"
+    return e, ec
+
+
 def setup_pair(cfg, with_projectors=True, assemble_sparse=True, soc_off=False):
     """Returns (oracle ctx, gpu ctx, system). Inputs are generated once from the ORACLE's coordinates/masses;
     the GPU library's own coordinates and masses are asserted to agree in test_gpu_parity.py."""

@@ -7,7 +7,7 @@ import numpy as np
 import pytest
 
 from paper_2410_02754_b200 import synth, bounds
-from helpers import setup_pair, gpu_apply_H, gpu_filter, rel_fro
+from helpers import setup_pair, gpu_apply_H, gpu_filter, rel_fro, assert_block_close
 
 pytestmark = pytest.mark.gpu
 TOL = 1e-11
@@ -30,7 +30,7 @@ def test_apply_H_all_orders(order):
     cfg = _cfg((2, 3, 2), (2.2, 3.0, 1.9), order, (0, 0, 0), 2 if order >= 2 else 0, nvec=5)
     ref, gpu, s = setup_pair(cfg, with_projectors=order >= 2)
     X = synth.random_block(s.rng, 2 * ref.M, cfg.nvec)
-    assert rel_fro(gpu_apply_H(gpu, X), ref.apply_H(X)) < TOL
+    assert_block_close(gpu_apply_H(gpu, X), ref.apply_H(X), TOL)
 
 
 @pytest.mark.parametrize("variant", [0, 1])
@@ -39,7 +39,7 @@ def test_apply_H_cfg0_variants_and_ragged(variant, nvec, ld):
     ref, gpu, s = setup_pair(synth.CONFIGS[0])
     gpu.set_variant(variant)
     X = synth.random_block(s.rng, 2 * ref.M, nvec)
-    assert rel_fro(gpu_apply_H(gpu, X, ld=ld), ref.apply_H(X)) < TOL
+    assert_block_close(gpu_apply_H(gpu, X, ld=ld), ref.apply_H(X), TOL)
 
 
 @pytest.mark.parametrize("bc", [(0, 0, 1), (1, 1, 1), (1, 0, 0), (0, 1, 0)])
@@ -48,7 +48,7 @@ def test_apply_H_dirichlet_and_noncubic(bc, order):
     cfg = _cfg((3, 2, 4), (3.3, 2.5, 3.0), order, bc, 3, nvec=7)
     ref, gpu, s = setup_pair(cfg)
     X = synth.random_block(s.rng, 2 * ref.M, cfg.nvec)
-    assert rel_fro(gpu_apply_H(gpu, X), ref.apply_H(X)) < TOL
+    assert_block_close(gpu_apply_H(gpu, X), ref.apply_H(X), TOL)
 
 
 def test_apply_H_parts_separately():
@@ -64,14 +64,14 @@ def test_apply_H_parts_separately():
                 ctx.set_projectors(s.node_ptr, s.node_idx, s.nproj, s.pvals, s.atom_type, s.delta, s.delta_ptr)
             else:
                 ctx.set_projectors(*empty)
-        assert rel_fro(gpu_apply_H(gpu, X), ref.apply_H(X)) < TOL
+        assert_block_close(gpu_apply_H(gpu, X), ref.apply_H(X), TOL)
 
 
 def test_single_cell_periodic_directions():
     cfg = _cfg((1, 1, 3), (1.0, 1.2, 3.0), 3, (0, 0, 0), 0, nvec=4)
     ref, gpu, s = setup_pair(cfg, with_projectors=False)
     X = synth.random_block(s.rng, 2 * ref.M, cfg.nvec)
-    assert rel_fro(gpu_apply_H(gpu, X), ref.apply_H(X)) < TOL
+    assert_block_close(gpu_apply_H(gpu, X), ref.apply_H(X), TOL)
 
 
 def test_generic_projector_counts():
@@ -87,7 +87,7 @@ def test_generic_projector_counts():
     args = (node_ptr, np.concatenate(idx), nproj, np.concatenate(pv), np.arange(3, dtype=np.int32), np.concatenate(dl), dptr)
     ref.set_projectors(*args); gpu.set_projectors(*args)
     X = synth.random_block(s.rng, 2 * M, cfg.nvec)
-    assert rel_fro(gpu_apply_H(gpu, X), ref.apply_H(X)) < TOL
+    assert_block_close(gpu_apply_H(gpu, X), ref.apply_H(X), TOL)
 
 
 @pytest.mark.parametrize("degree", [0, 1, 2, 3, 8, 9])
@@ -95,8 +95,8 @@ def test_filter_cfg0_degrees(degree, cfg0_oracle):
     ref, a, b, X = (cfg0_oracle[k] for k in ("ctx", "a", "b", "X"))
     _, gpu, _ = setup_pair(synth.CONFIGS[0])
     Yref = ref.filter(X, degree, a, b)
-    assert rel_fro(gpu_filter(gpu, X, degree, a, b), Yref) < TOL
-    assert rel_fro(gpu_filter(gpu, X[:, :11], degree, a, b, ld=14), Yref[:, :11]) < TOL
+    assert_block_close(gpu_filter(gpu, X, degree, a, b), Yref, TOL)
+    assert_block_close(gpu_filter(gpu, X[:, :11], degree, a, b, ld=14), Yref[:, :11], TOL)
 
 
 def test_filter_cfg0_against_dense_brute_force(cfg0_oracle):
@@ -106,7 +106,7 @@ def test_filter_cfg0_against_dense_brute_force(cfg0_oracle):
     lam, V = np.linalg.eigh(ref.dense_H()); lt = (lam - 0.5 * (a + b)) / (0.5 * (b - a))
     t = np.where(np.abs(lt) <= 1, np.cos(8 * np.arccos(np.clip(lt, -1, 1))), np.cosh(8 * np.arccosh(np.maximum(np.abs(lt), 1))))
     Yb = V @ (t[:, None] * (V.conj().T @ X))
-    assert rel_fro(gpu_filter(gpu, X, 8, a, b), Yb) < TOL
+    assert_block_close(gpu_filter(gpu, X, 8, a, b), Yb, TOL)
 
 
 @pytest.mark.parametrize("base,ncell,natoms,nvec,degree", [(2, (4, 4, 8), 3, 24, 10), (3, (6, 6, 6), 4, 16, 12), (4, (6, 6, 6), 4, 16, 12)])
@@ -116,7 +116,7 @@ def test_filter_shapes_of_large_configs(base, ncell, natoms, nvec, degree):
     ref, gpu, s = setup_pair(cfg)
     a, b, _, _ = bounds.lanczos_bounds(lambda v: ref.apply_H(v), 2 * ref.M)
     X = synth.random_block(s.rng, 2 * ref.M, nvec)
-    assert rel_fro(gpu_filter(gpu, X, degree, a, b), ref.filter(X, degree, a, b)) < TOL
+    assert_block_close(gpu_filter(gpu, X, degree, a, b), ref.filter(X, degree, a, b), TOL)
 
 
 def test_su2_covariance_on_gpu():
@@ -129,7 +129,7 @@ def test_su2_covariance_on_gpu():
     rot = lambda Z: (Z.reshape(M, 2, -1).transpose(0, 2, 1) @ U.T).transpose(0, 2, 1).reshape(2 * M, -1)
     Y = gpu_filter(gpu, X, 8, a, b)
     gpu.set_potential(s.veff, s.bxyz @ R.T)
-    assert rel_fro(gpu_filter(gpu, np.ascontiguousarray(rot(X)), 8, a, b), rot(Y)) < TOL
+    assert_block_close(gpu_filter(gpu, np.ascontiguousarray(rot(X)), 8, a, b), rot(Y), TOL)
 
 
 def test_error_codes():
@@ -173,7 +173,7 @@ def test_filter_host_pipeline_matches_oracle(chunk, nvec, ld, cfg0_oracle):
     hY = torch.full((2 * ref.M, ld), 7.0 + 3.0j, dtype=torch.complex128).pin_memory()
     gpu.filter_host(hX, hY, ld, nvec, 8, a, b)
     out = hY.numpy()
-    assert rel_fro(out[:, :nvec], ref.filter(X, 8, a, b)) < TOL
+    assert_block_close(out[:, :nvec], ref.filter(X, 8, a, b), TOL)
     if ld > nvec:
         assert np.all(out[:, nvec:] == 7.0 + 3.0j), "padding columns were touched"
     Yn = np.zeros((2 * ref.M, ld), dtype=np.complex128)      # pageable NumPy buffers work too
@@ -220,7 +220,7 @@ def test_fp32_intermediate_shapes_of_large_configs(base, ncell, natoms, nvec, de
     ref, gpu, s = setup_pair(cfg)
     a, b, _, _ = bounds.lanczos_bounds(lambda v: ref.apply_H(v), 2 * ref.M)
     X = synth.random_block(s.rng, 2 * ref.M, nvec)
-    assert rel_fro(gpu_filter32(gpu, X, degree, a, b), ref.filter(X, degree, a, b)) < TOL32
+    assert_block_close(gpu_filter32(gpu, X, degree, a, b), ref.filter(X, degree, a, b), TOL32)
 
 
 @pytest.mark.parametrize("order", [1, 2, 4, 6, 7])
@@ -229,4 +229,4 @@ def test_fp32_intermediate_orders(order):
     ref, gpu, s = setup_pair(cfg, with_projectors=order >= 2)
     a, b, _, _ = bounds.lanczos_bounds(lambda v: ref.apply_H(v), 2 * ref.M)
     X = synth.random_block(s.rng, 2 * ref.M, cfg.nvec)
-    assert rel_fro(gpu_filter32(gpu, X, 5, a, b), ref.filter(X, 5, a, b)) < TOL32
+    assert_block_close(gpu_filter32(gpu, X, 5, a, b), ref.filter(X, 5, a, b), TOL32)
