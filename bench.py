@@ -124,9 +124,21 @@ def build_system(cfg, ctx, with_projectors=True):
     return sysm
 
 
+def roofline_model(p, c_ov, fp32):
+    """Algorithmic bytes and flops per unit and the time floors they imply.
+    FP64 mode: 48 B/unit through the column kernel + 16 c_ov B/unit re-read by the projector gather; all flops FP64.
+    FP32-intermediate mode: 24 B/unit + 8 c_ov; the cell arithmetic (kinetic, potential, recurrence) runs on the FP32 FMA pipe,
+    the projector contractions (gather + expansion, 144 c_ov flops/unit) stay FP64."""
+    f_cell, f_gather, f_total = algorithmic_flops(p, c_ov)
+    f_proj = 144.0 * c_ov
+    return {"bytes_column": 24.0 if fp32 else 48.0, "bytes_gather": (8.0 if fp32 else 16.0) * c_ov,
+            "flops_fp64": f_proj if fp32 else f_total, "flops_fp32": (f_total - f_proj) if fp32 else 0.0,
+            "flops_column": f_cell, "flops_total": f_total}
+
+
 def cpu_sample_config(cfg):
-    """Bounded sample of the workload for the oracle: same cell size, order, boundary conditions, atom density and
-    degree on an 8x8x8-cell sub-mesh (config 0/1: the whole mesh), 16 columns."""
+    """Fallback sample when the host cannot hold the config's CSR: same cell size, order, boundary conditions, atom density
+    and degree on an 8x8x8-cell sub-mesh (config 0/1: the whole mesh), 16 columns."""
     if cfg.index <= 1:
         return synth.Config(cfg.index, cfg.name, cfg.ncell, cfg.box, cfg.order, cfg.bc, cfg.natoms, cfg.placement, min(cfg.nvec, 16), cfg.degree, 0, cfg.seed)
     nc = tuple(min(8, c) for c in cfg.ncell)
@@ -134,25 +146,50 @@ def cpu_sample_config(cfg):
     return synth.scaled_config(cfg, nc, max(1, int(round(cfg.natoms * frac))), nvec=16, degree=cfg.degree)
 
 
-def run_oracle_sample(cfg, steps=1, warmup=0):
-    """Times the oracle as it stands (oracle/, OpenMP) on the bounded sample; returns (units/s, description, cores, ms/step)."""
-    from oracle import oracle as O
-    from paper_2410_02754_b200 import bounds
-    sc = cpu_sample_config(cfg)
-    ref = O.RefCtx(sc.ncell, sc.box, sc.order, sc.bc)
-    sysm = build_system(sc, ref)
-    a, b, _, _ = bounds.lanczos_bounds(lambda v: ref.apply_H(v), 2 * ref.M, k=10)
-    X = synth.random_block(sysm.rng, 2 * ref.M, sc.nvec)
+class OracleSample:
+    """The oracle as it stands (oracle/, OpenMP on all host cores) on a bounded sample of the benchmarked workload:
+    the ACTUAL config (mesh, atoms, potential: the global CSR is assembled once, outside the timed region, like the GPU
+    side's set-up) with 8 columns and as many Chebyshev degrees as fit `budget_s` seconds (SURVEY 8(d) "CPU baseline").
+    If the host cannot hold the CSR it falls back to an 8x8x8-cell sub-mesh and says so."""
+
+    def __init__(self, cfg, budget_s=20.0, est_units_per_s=4.5e7):
+        import psutil
+        from oracle import oracle as O
+        from paper_2410_02754_b200 import bounds
+        self.O = O
+        need = cfg.M * ((cfg.order + 2) ** 3 * 12.0 + 200.0) + 5 * 2 * cfg.M * 8 * 16.0          # CSR + conn + vectors
+        self.full = psutil.virtual_memory().available > 1.5 * need
+        self.cfg = cfg
+        sc = cfg if self.full else cpu_sample_config(cfg)
+        self.ncols = 8 if self.full else sc.nvec
+        per_degree = 2.0 * sc.M * self.ncols
+        self.degree = int(min(sc.degree, max(2, round(budget_s * est_units_per_s / per_degree)))) if self.full else sc.degree
+        self.ref = O.RefCtx(sc.ncell, sc.box, sc.order, sc.bc)
+        self.sysm = build_system(sc, self.ref)
+        self.a, self.b, _, _ = bounds.lanczos_bounds(lambda v: self.ref.apply_H(v), 2 * self.ref.M, k=6)
+        self.X = synth.random_block(self.sysm.rng, 2 * self.ref.M, self.ncols)
+        self.units = 2.0 * self.ref.M * self.ncols * self.degree
+        if self.full:
+            self.desc = (f"the config's own operator ({sc.ncell[0]}x{sc.ncell[1]}x{sc.ncell[2]} cells, {sc.natoms} atoms; CSR assembled outside the timed region), "
+                         f"8 columns, degree {self.degree} of {cfg.degree}: {self.units:.3g} of the block's {2.0 * cfg.M * cfg.nvec * cfg.degree:.3g} units; "
+                         f"a full block would take {cfg.nvec / 8.0 * cfg.degree / self.degree:.0f}x as long (linear extrapolation)")
+        else:
+            self.desc = (f"host memory too small for the config's CSR: {sc.ncell[0]}x{sc.ncell[1]}x{sc.ncell[2]} cells of order {sc.order} (same cell size, bc, atom density: "
+                         f"{sc.natoms} atoms), {sc.nvec} columns, degree {sc.degree}: {self.units:.3g} of the workload's {2.0 * cfg.M * cfg.nvec * cfg.degree:.3g} units")
+
+    def step(self):
+        t0 = time.perf_counter()
+        self.ref.filter(self.X, self.degree, self.a, self.b)
+        return time.perf_counter() - t0
+
+
+def run_oracle_sample(cfg, steps=1, warmup=0, budget_s=20.0):
+    """Returns (units/s, description, cores, ms/step)."""
+    smp = OracleSample(cfg, budget_s=budget_s)
     for _ in range(warmup):
-        ref.filter(X[:, :2], 2, a, b)
-    t0 = time.perf_counter()
-    for _ in range(steps):
-        ref.filter(X, sc.degree, a, b)
-    dt = (time.perf_counter() - t0) / steps
-    units = 2.0 * ref.M * sc.nvec * sc.degree
-    desc = f"{sc.ncell[0]}x{sc.ncell[1]}x{sc.ncell[2]} cells of order {sc.order} (same cell size, bc, atom density: {sc.natoms} atoms), " \
-           f"{sc.nvec} columns, degree {sc.degree}: {units:.3g} of the workload's {2.0 * cfg.M * cfg.nvec * cfg.degree:.3g} units"
-    return units / dt, desc, O.num_threads(), dt * 1e3
+        smp.ref.filter(smp.X[:, :2], 1, smp.a, smp.b)
+    dt = sum(smp.step() for _ in range(steps)) / steps
+    return smp.units / dt, smp.desc, smp.O.num_threads(), dt * 1e3
 
 
 def workload_dict(cfg, sysm=None):
@@ -171,7 +208,8 @@ def main_reference(args):
     if rank != 0:
         return 0
     cfg = synth.CONFIGS[args.config]
-    val, desc, cores, ms = run_oracle_sample(cfg, steps=max(1, args.steps), warmup=min(args.warmup, 1))
+    nsteps = max(1, args.steps)
+    val, desc, cores, ms = run_oracle_sample(cfg, steps=nsteps, warmup=min(args.warmup, 1), budget_s=max(2.0, min(20.0, 150.0 / (nsteps + 1))))
     out = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
            "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
            "config": workload_dict(cfg),
@@ -182,18 +220,14 @@ def main_reference(args):
 
 
 # ----------------------------------------------------------------------------------------------- our arm
-def main_ours(args):
+def measure(cfg_index, mode_name, steps, warmup, args, ctxs):
+    """One benchmark leg: `steps` timed csf_filter calls of one block of config `cfg_index` in `mode_name` on this rank's GPU.
+    Returns the result dict and the live objects the end-to-end leg reuses (ctx, X, bounds)."""
     import torch
     import torch.distributed as dist
     from paper_2410_02754_b200 import binding, bounds
-
-    world = int(os.environ.get("WORLD_SIZE", "1")); rank = int(os.environ.get("RANK", "0")); local = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise RuntimeError("bench.py needs a CUDA device: the product path has no CPU fallback")
-    torch.cuda.set_device(local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    cfg = synth.CONFIGS[args.config]
+    world, rank, local = ctxs["world"], ctxs["rank"], ctxs["local"]
+    cfg = synth.CONFIGS[cfg_index]
     nvec = args.nvec or cfg.nvec
     degree = args.degree or cfg.degree
     stream = torch.cuda.current_stream()
@@ -203,7 +237,8 @@ def main_ours(args):
     t_setup = time.perf_counter()
     sysm = build_system(cfg, ctx, with_projectors=not args.no_projectors)
     M = ctx.M; rows = 2 * M
-    mode = binding.CSF_FP32_INTERMEDIATE if args.mode == "fp32" else binding.CSF_FP64
+    fp32 = mode_name == "fp32"
+    mode = binding.CSF_FP32_INTERMEDIATE if fp32 else binding.CSF_FP64
     wb = max(ctx.workspace_bytes(nvec, mode), ctx.workspace_bytes(nvec))
     work = torch.empty(max(wb, 16), dtype=torch.uint8, device="cuda")
 
@@ -231,7 +266,7 @@ def main_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    for _ in range(args.warmup):
+    for _ in range(warmup):
         ctx.filter(X, Y, nvec, nvec, degree, a, b, mode, work)
     barrier()
     for k in range(binding.KIND_AUX + 1):
@@ -244,7 +279,7 @@ def main_ours(args):
     barrier()
     e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
     e0.record(stream)
-    for _ in range(args.steps):
+    for _ in range(steps):
         ctx.filter(X, Y, nvec, nvec, degree, a, b, mode, work)
     e1.record(stream)
     barrier()
@@ -254,53 +289,99 @@ def main_ours(args):
     launches = ctx.launch_count() - l0
     kinds = {binding.KIND_NAMES[k]: ctx.profile_read(k) for k in range(binding.KIND_AUX + 1)}
     ctx.profile_enable(False)
-    ms_per_step = ms / args.steps
+    ms_per_step = ms / steps
     units_step = float(rows) * nvec * degree
     value = world * units_step / (ms_per_step * 1e-3)
     finite = bool(torch.isfinite(torch.view_as_real(Y)).all().item())
 
-    # ---- roofline of the dominant kernel (cell kernel) and of the whole step
-    f_cell, f_gather, f_total = algorithmic_flops(cfg.order, sysm.coverage)
-    peaks = {}
+    # ---- roofline of the dominant kernel (column kernel) and of the whole step
+    rm = roofline_model(cfg.order, sysm.coverage, fp32)
+    peaks = ctxs["peaks"]
+    sm_max = float(peaks.get("sm_max_mhz", 1965.0))
+    peak64 = SM_COUNT * FP64_FMA_PER_CLK_PER_SM * 2 * sm_max * 1e6 / 1e12
+    peak32 = 2.0 * peak64                                   # 128 FP32 lanes per clock and SM
+    hbm = float(peaks.get("hbm_gbs", 6650.0))
+    cell_ms, cell_n = kinds["cell"]
+    launch_units = float(rows) * nvec
+    # time floors of one H apply (all kernels of a step): HBM, and the ALU pipes (FP32 part at the FP32 peak + FP64 part at the FP64 peak)
+    t_hbm = (rm["bytes_column"] + rm["bytes_gather"]) * launch_units / (hbm * 1e9)
+    t_alu = launch_units * (rm["flops_fp32"] / (peak32 * 1e12) + rm["flops_fp64"] / (peak64 * 1e12))
+    roof = None
+    if cell_n > 0:
+        t_cell = cell_ms / cell_n * 1e-3
+        if fp32:
+            # the column kernel's own floors: 24 B/unit, its FP32 cell flops + the FP64 expansion (72 c_ov flops/unit)
+            f32c = rm["flops_column"] - 72.0 * sysm.coverage
+            t_floor = max(rm["bytes_column"] * launch_units / (hbm * 1e9), launch_units * (f32c / (peak32 * 1e12) + 72.0 * sysm.coverage / (peak64 * 1e12)))
+            ach = rm["flops_column"] * launch_units / t_cell / 1e12
+            roof = {"kernel": "column_kernel<float> (a1-a4, a7, a8)", "bound": "alu", "achieved": ach, "peak": rm["flops_column"] * launch_units / t_floor / 1e12,
+                    "unit": "TFLOP/s", "frac": t_floor / t_cell,
+                    "peak_source": "mixed-pipe floor: FP32 cell flops at 148 SMs x 128 FMA/clk x 2 x %.0f MHz + FP64 expansion flops at half that, or 24 B/unit at the measured HBM copy rate, whichever is slower (DESIGN.md section 5)" % sm_max}
+        else:
+            ach = rm["flops_column"] * launch_units / t_cell / 1e12
+            roof = {"kernel": "column_kernel (a1-a4, a7, a8)", "bound": "alu", "achieved": ach, "peak": peak64, "unit": "TFLOP/s", "frac": ach / peak64,
+                    "peak_source": "148 SMs x 64 FP64 FMA/clk x 2 x %.0f MHz (DESIGN.md; DFMA and DMMA share these units: 36.4 TF/s measured together)" % sm_max}
+        tr = ctxs["traffic"].get("cfg%d_%s" % (cfg.index, mode_name))
+        roof.update({"traffic": (float(tr["dram_bytes_per_unit"]) * launch_units) if tr else None,
+                     "traffic_source": tr["source"] if tr else None,
+                     "algorithmic_bytes": rm["bytes_column"] * launch_units, "flops_per_unit": rm["flops_column"],
+                     "flops_note": "algorithmic count of SURVEY 8(d) (cheapest algorithm implemented); the kernel executes fewer kinetic flops (shared z-planes are contracted once) and more projector flops (K 18 -> 20, partial row tiles)",
+                     "avg_launch_ms": t_cell * 1e3, "launches": cell_n, "share_of_step": cell_ms / ms_local,
+                     "hbm_achieved_gbs": rm["bytes_column"] * launch_units / t_cell / 1e9, "hbm_peak_gbs": hbm,
+                     "hbm_frac": rm["bytes_column"] * launch_units / t_cell / 1e9 / hbm,
+                     "hbm_peak_source": "measured (MEASURED_PEAKS.json)" if peaks else "fallback"})
+    t_apply = ms_per_step * 1e-3 / degree
+    step = {"flops_per_unit": rm["flops_total"], "bytes_per_unit": rm["bytes_column"] + rm["bytes_gather"],
+            "floor_ms_per_apply": {"hbm": t_hbm * 1e3, "alu": t_alu * 1e3}, "ms_per_apply": t_apply * 1e3,
+            "frac": max(t_hbm, t_alu) / t_apply, "frac_alu": t_alu / t_apply, "frac_hbm": t_hbm / t_apply,
+            "bound": "alu" if t_alu >= t_hbm else "hbm",
+            "kernel_ms": {k: round(v[0] / steps, 3) for k, v in kinds.items()}}
+    conf = workload_dict(cfg, sysm)
+    conf.update({"block_vectors": nvec, "degree": degree, "bounds": [a, b], "lanczos_ritz": [tmin, tmax], "parallelism": f"replicas x{world}" if world > 1 else "single GPU",
+                 "mode": mode_name, "column_kernel_lanes": ctx.column_lanes(nvec, 1 if fp32 else 0), "setup_s": round(t_setup, 2)})
+    res = {"value": value, "ms_per_step": ms_per_step, "steps": steps, "warmup": warmup, "dtype": "f32" if fp32 else "f64", "config": conf, "clocks": clocks,
+           "gpu_launches": launches, "roofline": roof, "step_roofline": step, "finite": finite}
+    if cfg.nstates > 0:
+        nblocks = math.ceil(cfg.nstates / cfg.nvec)
+        res["full_filter_extrapolated_s"] = {"blocks": nblocks, "seconds": nblocks * ms_per_step * 1e-3, "note": "per-block time x blocks of the config's state count (BASELINE.json)"}
+    live = {"ctx": ctx, "X": X, "Y": Y, "work": work, "a": a, "b": b, "rows": rows, "nvec": nvec, "degree": degree, "mode": mode, "barrier": barrier}
+    return res, live
+
+
+def main_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    world = int(os.environ.get("WORLD_SIZE", "1")); rank = int(os.environ.get("RANK", "0")); local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    peaks, traffic = {}, {}
     try:
         with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
             peaks = json.load(f)
     except OSError:
         pass
-    sm_max = float(peaks.get("sm_max_mhz", 1965.0))
-    fp32 = args.mode == "fp32"
-    # FP32-intermediate mode: the cell arithmetic runs on the FP32 FMA pipe (128 lanes/clk/SM) and moves 24 B/unit
-    peak_alu = SM_COUNT * FP64_FMA_PER_CLK_PER_SM * (2 if fp32 else 1) * 2 * sm_max * 1e6 / 1e12
-    bytes_unit = 24.0 if fp32 else 48.0
-    hbm = float(peaks.get("hbm_gbs", 6650.0))
-    cell_ms, cell_n = kinds["cell"]
-    roof = None
-    if cell_n > 0:
-        t_cell = cell_ms / cell_n * 1e-3
-        ach = f_cell * rows * nvec / t_cell / 1e12
-        traffic = None
-        try:
-            with open(os.path.join(ROOT, "profiles", "r1_traffic.json")) as f:
-                traffic = None if fp32 else float(json.load(f)["dram_bytes_per_unit"]) * rows * nvec    # ncu --set full capture (FP64 kernel), scaled to this launch
-        except (OSError, KeyError, ValueError):
-            pass
-        roof = {"kernel": "column_kernel (a1-a4, a7, a8)", "bound": "alu", "achieved": ach, "peak": peak_alu, "unit": "TFLOP/s", "frac": ach / peak_alu,
-                "peak_source": ("148 SMs x 128 FP32 FMA/clk x 2 x %.0f MHz (DESIGN.md)" if fp32 else "148 SMs x 64 FP64 FMA/clk x 2 x %.0f MHz (DESIGN.md)") % sm_max, "traffic": traffic,
-                "algorithmic_bytes": bytes_unit * rows * nvec,
-                "flops_per_unit": f_cell, "avg_launch_ms": t_cell * 1e3, "launches": cell_n,
-                "share_of_step": cell_ms / ms_local,
-                "hbm_achieved_gbs": bytes_unit * rows * nvec / t_cell / 1e9, "hbm_peak_gbs": hbm, "hbm_frac": bytes_unit * rows * nvec / t_cell / 1e9 / hbm,
-                "hbm_peak_source": "measured (MEASURED_PEAKS.json)" if peaks else "fallback"}
-        if not args.no_probe:
-            pf, pm = binding.probe_fp64_peak(local)
-            roof["peak_measured_dfma"] = pf; roof["peak_measured_dmma"] = pm; roof["frac_of_measured_dfma"] = ach / pf
-    step = {"flops_per_unit": f_total, "tflops": f_total * units_step / (ms_per_step * 1e-3) / 1e12,
-            "frac_alu": f_total * units_step / (ms_per_step * 1e-3) / 1e12 / peak_alu,
-            "hbm_gbs": bytes_unit * units_step / (ms_per_step * 1e-3) / 1e9, "frac_hbm": bytes_unit * units_step / (ms_per_step * 1e-3) / 1e9 / hbm,
-            "kernel_ms": {k: round(v[0] / args.steps, 3) for k, v in kinds.items()}}
+    try:
+        with open(os.path.join(ROOT, "profiles", "r2_traffic.json")) as f:       # DRAM bytes per unit from one `ncu --set full` capture per (config, mode)
+            traffic = json.load(f)
+    except (OSError, ValueError):
+        pass
+    ctxs = {"world": world, "rank": rank, "local": local, "peaks": peaks, "traffic": traffic}
+
+    head, live = measure(args.config, args.mode, args.steps, args.warmup, args, ctxs)
+    if head["roofline"] is not None and not args.no_probe:
+        from paper_2410_02754_b200 import binding
+        pf, pm = binding.probe_fp64_peak(local)
+        head["roofline"]["peak_measured_dfma"] = pf; head["roofline"]["peak_measured_dmma"] = pm
+        if args.mode == "fp64":
+            head["roofline"]["frac_of_measured_dfma"] = head["roofline"]["achieved"] / pf
 
     # ---- end to end: host buffers through csf_filter_host (H2D + filter + D2H inside the timed region)
     e2e = None
+    ctx, X, rows, nvec, degree, a, b, mode, barrier = (live[k] for k in ("ctx", "X", "rows", "nvec", "degree", "a", "b", "mode", "barrier"))
     if not args.no_e2e:
         import psutil
         e2e_nvec = nvec
@@ -310,7 +391,8 @@ def main_ours(args):
             e2e_nvec //= 2
         hX = torch.empty((rows, e2e_nvec), dtype=torch.complex128, pin_memory=True)
         hX.copy_(X[:, :e2e_nvec])
-        del X, Y, work
+        live["X"] = live["Y"] = live["work"] = None
+        del X
         torch.cuda.empty_cache()
         hY = torch.empty((rows, e2e_nvec), dtype=torch.complex128, pin_memory=True)
         ctx.set_host_chunk(args.host_chunk)
@@ -330,20 +412,33 @@ def main_ours(args):
                "api": "csf_filter_host (pinned host X, Y; column chunks staged H2D / filtered / D2H on three streams)",
                "finite": bool(torch.isfinite(torch.view_as_real(hY[::4097])).all().item())}
         del hX, hY
+    live.clear()
+    del ctx
+    torch.cuda.empty_cache()
+
+    # ---- the other roofline-target legs (BASELINE.json: configs 2-4 in complex128, config 4 also FP32-intermediate)
+    others = []
+    if world == 1 and not args.no_others and not (args.nvec or args.degree):
+        for k, m in [(2, "fp64"), (3, "fp64"), (4, "fp64"), (4, "fp32")]:
+            if (k, m) == (args.config, args.mode):
+                continue
+            r, lv = measure(k, m, args.other_steps, max(3, min(args.warmup, 3)), args, ctxs)
+            lv.clear()
+            torch.cuda.empty_cache()
+            others.append({"workload": r["config"]["workload"], "mode": m, "value": r["value"], "unit": UNIT, "ms_per_step": r["ms_per_step"], "steps": r["steps"],
+                           "warmup": r["warmup"], "roofline": r["roofline"], "step_roofline": r["step_roofline"], "clocks": r["clocks"], "finite": r["finite"],
+                           "full_filter_extrapolated_s": r.get("full_filter_extrapolated_s"), "c_ov": r["config"].get("c_ov")})
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        v, desc, cores, _ = run_oracle_sample(cfg)
+        v, desc, cores, _ = run_oracle_sample(synth.CONFIGS[args.config])
         cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
 
     if rank == 0:
-        conf = workload_dict(cfg, sysm)
-        conf.update({"block_vectors": nvec, "degree": degree, "bounds": [a, b], "lanczos_ritz": [tmin, tmax], "parallelism": f"replicas x{world}" if world > 1 else "single GPU", "mode": args.mode,
-                     "column_kernel_lanes": ctx.column_lanes(nvec, 1 if args.mode == "fp32" else 0),
-                     "setup_s": round(t_setup, 2)})
-        out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step,
-               "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32" if args.mode == "fp32" else "f64", "data": "synthetic", "config": conf,
-               "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roof, "step_roofline": step, "cpu_baseline": cpu, "finite": finite}
+        out = {"metric": METRIC, "value": head["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": head["ms_per_step"],
+               "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": head["dtype"], "data": "synthetic", "config": head["config"],
+               "clocks": head["clocks"], "e2e": e2e, "gpu_launches": head["gpu_launches"], "roofline": head["roofline"], "step_roofline": head["step_roofline"],
+               "cpu_baseline": cpu, "finite": head["finite"], "full_filter_extrapolated_s": head.get("full_filter_extrapolated_s"), "other_configs": others}
         print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()
@@ -368,6 +463,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-profile", action="store_true")
     ap.add_argument("--no-probe", action="store_true")
+    ap.add_argument("--no-others", action="store_true", help="skip the other roofline-target legs (configs 2, 4 in FP64, config 4 in FP32-intermediate)")
+    ap.add_argument("--other-steps", type=int, default=2, help="timed steps of each other leg")
     args = ap.parse_args()
     return main_reference(args) if args.impl == "reference" else main_ours(args)
 
