@@ -160,6 +160,46 @@ int csf_set_variant(csf_ctx* ctx, int variant);
  * flush and multi-group grids on small meshes. CSF_EINVAL on seg_len < 0 or chunk_group < 1. */
 int csf_set_tuning(csf_ctx* ctx, int seg_len, int chunk_group);
 
+/* ---- Subspace steps around the filter -----------------------------------------------
+ * X is a block in the same layout and basis as for csf_filter (Loewdin-scaled: X = M_D^{1/2} U), so the generalized problem
+ * of PAPER.md:473-477 eq.71, X_s^dagger H X_s Q = X_s^dagger M X_s Q Lambda, reads Hs Q = Ss Q Lambda with the two matrices below. */
+
+/* Device workspace of csf_rr_project / csf_rr_rotate for a block of nvec vectors. */
+int csf_rr_workspace_bytes(const csf_ctx* ctx, int nvec, size_t* bytes);
+
+/* Rayleigh-Ritz projection (eq.71): dHs = X^dagger Hhat X, dSs = X^dagger X, both DEVICE complex128 [nvec][nvec] row-major,
+ * exactly Hermitian (the upper triangle is computed, the lower mirrored). FP64 tensor-core GEMMs over all 2M rows.
+ * Enqueues on the context's stream; X is not modified. Errors as csf_apply_H. */
+int csf_rr_project(csf_ctx* ctx, const csf_c128* dX, int64_t ld, int nvec, csf_c128* dHs, csf_c128* dSs,
+                   void* d_work, size_t work_bytes);
+
+/* Solve the projected problem Hs Q = Ss Q Lambda (eq.71; n x n, dense: cuSOLVER's zhegvd, loaded at first use). dQ: DEVICE
+ * [n][n] row-major, column j = eigenvector j with Q^dagger Ss Q = I; lambda_host: HOST [n], ascending. SYNCHRONISES.
+ * CSF_EINVAL if Ss is not positive definite (linearly dependent block), CSF_EUNSUPPORTED if libcusolver is missing. */
+int csf_rr_solve(csf_ctx* ctx, const csf_c128* dHs, const csf_c128* dSs, int n, csf_c128* dQ, double* lambda_host);
+
+/* Subspace rotation (eq.72): dU = X Q, dU [2M][ldu] must not alias dX; Q as returned by csf_rr_solve (any
+ * complex [nvec][nvec] row-major matrix is accepted). Needs csf_rr_workspace_bytes. Enqueues on the stream. */
+int csf_rr_rotate(csf_ctx* ctx, const csf_c128* dX, int64_t ld, int nvec, const csf_c128* dQ, csf_c128* dU, int64_t ldu,
+                  void* d_work, size_t work_bytes);
+
+/* Electron density and magnetisation at the nodes (eq.4-5) from a block of states with occupations
+ * occ_host[nvec] (HOST): psi^alpha_n(r_I) = X[2I+alpha][n] / sqrt(m_I), d_rho_m (DEVICE) [M][4] = rho, m_x, m_y, m_z.
+ * accumulate != 0 adds to d_rho_m (blocks of states are summed), else overwrites. Copies occ, then enqueues on the stream. */
+int csf_density(csf_ctx* ctx, const csf_c128* dX, int64_t ld, int nvec, const double* occ_host, double* d_rho_m, int accumulate);
+
+/* k steps of the Lanczos recurrence on Hhat on the device (lambda_min, lambda_max from Lanczos), start vector
+ * d_v0 (DEVICE complex128 [2M], any non-zero norm; not modified): alpha_host[k], beta_host[k] (HOST) receive the tridiagonal
+ * coefficients, beta_host[j] = |w| after step j (beta_host[k-1] is the residual norm), *steps_done <= k the steps taken (an
+ * invariant subspace ends the recurrence early). SYNCHRONISES (two scalars come back per step). */
+int csf_lanczos_workspace_bytes(const csf_ctx* ctx, size_t* bytes);
+int csf_lanczos(csf_ctx* ctx, const csf_c128* d_v0, int k, double* alpha_host, double* beta_host, int* steps_done,
+                void* d_work, size_t work_bytes);
+
+/* Smallest and largest eigenvalue of the symmetric tridiagonal matrix (alpha[k], beta[0..k-2]) by Sturm bisection: the Ritz
+ * values theta_min, theta_max of a csf_lanczos run; theta_max + beta[k-1] is the customary upper bound b of the filter. Host only. */
+int csf_tridiag_extremes(const double* alpha, const double* beta, int k, double* theta_min, double* theta_max);
+
 /* Text of the last error recorded on ctx (never NULL; "" if none). With ctx = NULL: last csf_create failure. */
 const char* csf_last_error(const csf_ctx* ctx);
 

@@ -17,7 +17,9 @@ CSF_FP64, CSF_FP32_INTERMEDIATE = 0, 1
 
 EXPORTS = ["csf_create", "csf_destroy", "csf_set_stream", "csf_num_nodes", "csf_node_coords", "csf_mass_diag", "csf_set_potential",
            "csf_set_projectors", "csf_workspace_bytes", "csf_apply_H", "csf_filter", "csf_filter_host", "csf_set_host_chunk",
-           "csf_profile_enable", "csf_profile_read", "csf_probe_fp64_peak", "csf_launch_count", "csf_column_lanes", "csf_set_variant", "csf_set_tuning", "csf_last_error"]
+           "csf_profile_enable", "csf_profile_read", "csf_probe_fp64_peak", "csf_launch_count", "csf_column_lanes", "csf_set_variant", "csf_set_tuning", "csf_last_error",
+           "csf_rr_workspace_bytes", "csf_rr_project", "csf_rr_solve", "csf_rr_rotate", "csf_density", "csf_lanczos_workspace_bytes", "csf_lanczos",
+           "csf_tridiag_extremes"]
 KIND_CELL, KIND_PGATHER, KIND_DELTA, KIND_AUX = 0, 1, 2, 3
 KIND_NAMES = ("cell", "proj_gather", "delta", "aux")
 
@@ -152,11 +154,52 @@ class Csf:
     def launch_count(self):
         n = C.c_int64(); self._chk(self._L.csf_launch_count(self._h, C.byref(n))); return int(n.value)
 
+    # ---- subspace steps
+    def rr_workspace_bytes(self, nvec):
+        b = C.c_size_t(); self._chk(self._L.csf_rr_workspace_bytes(self._h, C.c_int(int(nvec)), C.byref(b))); return int(b.value)
+
+    def rr_project(self, dX, ld, nvec, dHs, dSs, d_work, work_bytes=0):
+        self._chk(self._L.csf_rr_project(self._h, self._ptr(dX), C.c_int64(int(ld)), C.c_int(int(nvec)), self._ptr(dHs), self._ptr(dSs), self._ptr(d_work), self._nbytes(d_work, work_bytes)))
+
+    def rr_solve(self, dHs, dSs, n, dQ):
+        """Returns the Ritz values (host NumPy array, ascending); dQ receives the eigenvectors on the device."""
+        lam = np.zeros(int(n))
+        self._chk(self._L.csf_rr_solve(self._h, self._ptr(dHs), self._ptr(dSs), C.c_int(int(n)), self._ptr(dQ), _dp(lam, C.c_double)))
+        return lam
+
+    def rr_rotate(self, dX, ld, nvec, dQ, dU, ldu, d_work, work_bytes=0):
+        self._chk(self._L.csf_rr_rotate(self._h, self._ptr(dX), C.c_int64(int(ld)), C.c_int(int(nvec)), self._ptr(dQ), self._ptr(dU), C.c_int64(int(ldu)), self._ptr(d_work), self._nbytes(d_work, work_bytes)))
+
+    def density(self, dX, ld, nvec, occ, d_rho_m, accumulate=False):
+        occ = np.ascontiguousarray(occ, dtype=np.float64)
+        if occ.shape != (int(nvec),):
+            raise ValueError("occ must have shape [nvec]")
+        self._chk(self._L.csf_density(self._h, self._ptr(dX), C.c_int64(int(ld)), C.c_int(int(nvec)), _dp(occ, C.c_double), self._ptr(d_rho_m), C.c_int(1 if accumulate else 0)))
+
+    def lanczos_workspace_bytes(self):
+        b = C.c_size_t(); self._chk(self._L.csf_lanczos_workspace_bytes(self._h, C.byref(b))); return int(b.value)
+
+    def lanczos(self, d_v0, k, d_work, work_bytes=0):
+        """(alpha, beta) of k Lanczos steps on Hhat from the device vector d_v0 (host NumPy arrays, truncated to the steps taken)."""
+        al = np.zeros(int(k)); be = np.zeros(int(k)); done = C.c_int()
+        self._chk(self._L.csf_lanczos(self._h, self._ptr(d_v0), C.c_int(int(k)), _dp(al, C.c_double), _dp(be, C.c_double), C.byref(done), self._ptr(d_work), self._nbytes(d_work, work_bytes)))
+        return al[:done.value], be[:done.value]
+
     def set_tuning(self, seg_len=0, chunk_group=16):
         self._chk(self._L.csf_set_tuning(self._h, C.c_int(int(seg_len)), C.c_int(int(chunk_group))))
 
     def set_variant(self, variant):
         self._chk(self._L.csf_set_variant(self._h, C.c_int(int(variant))))
+
+
+def tridiag_extremes(alpha, beta):
+    """(theta_min, theta_max) of the Lanczos tridiagonal matrix (csf_tridiag_extremes: Sturm bisection in the library)."""
+    alpha = np.ascontiguousarray(alpha, dtype=np.float64); beta = np.ascontiguousarray(beta, dtype=np.float64)
+    lo = C.c_double(); hi = C.c_double()
+    rc = lib().csf_tridiag_extremes(_dp(alpha, C.c_double), _dp(beta, C.c_double), C.c_int(len(alpha)), C.byref(lo), C.byref(hi))
+    if rc != CSF_OK:
+        raise CsfError(rc, "csf_tridiag_extremes")
+    return float(lo.value), float(hi.value)
 
 
 def probe_fp64_peak(device=0):

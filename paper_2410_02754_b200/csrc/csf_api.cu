@@ -3,10 +3,13 @@
 #include "csf_kernels.cuh"
 #include "csf_column.cuh"
 #include "csf_colws.cuh"
+#include "csf_subspace.cuh"
 #include "csf_column_launch.h"
 #include "csf_tables.h"
 
 #include <cuda.h>
+#include <cusolverDn.h>
+#include <dlfcn.h>
 
 #include <algorithm>
 #include <cmath>
@@ -46,6 +49,7 @@ struct csf_ctx {
     Gll1D gll; Dir1D dir[3];
     bool have_pot = false;
     DevBuf d_col_order, d_vb;
+    DevBuf d_inv_mass, d_occ;               // 1 / m_I (csf_density), occupation numbers of the last csf_density call
     DevBuf d_sub_ptr[kColMaxAuxWarps - 1], d_sub_desc[kColMaxAuxWarps - 1], d_a_pack[kColMaxAuxWarps - 1], d_ent_locf;     // [nq - 2]: nq expansion warps per CTA
     int seg_len = 0, chunk_group = 16;      // cells per z-segment (0 = the kernel's default), vector chunks scheduled back to back (csf_set_tuning)
     int lanes_force = 0;                    // CSF_LANES=16|32 pins the column kernel variant (tests, sweeps); 0 = measured policy
@@ -798,6 +802,278 @@ int csf_set_variant(csf_ctx* c, int variant) {
     if (!c) return CSF_EINVAL;
     if (variant < 0 || variant > 1) return fail(c, CSF_EINVAL, "unknown variant");
     c->variant = variant;
+    return CSF_OK;
+}
+
+}  // extern "C"
+
+// ------------------------------------------------------------------------------------------------------------------
+// Subspace steps around the filter: Rayleigh-Ritz, density / magnetisation, Lanczos
+// ------------------------------------------------------------------------------------------------------------------
+namespace {
+
+size_t rr_gram_bytes(int nvec) { return ((size_t)4 * nvec * nvec * sizeof(double) + 255) / 256 * 256; }      // real [2N][2N]
+
+// G = A^T B as real matrices, then the complex nvec x nvec result into dOut (row-major)
+int enqueue_gram(csf_ctx* c, const double* A, long long lda, const double* B, long long ldb, int nvec, double* dG, double2* dOut, int sym) {
+    static bool configured[64] = {};
+    int dev = 0; CSF_CUDA(c, cudaGetDevice(&dev));
+    if (dev < 0 || dev >= 64 || !configured[dev]) {
+        CSF_CUDA(c, cudaFuncSetAttribute(gram_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kGramSmem));
+        CSF_CUDA(c, cudaFuncSetAttribute(rotate_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRotSmem));
+        if (dev >= 0 && dev < 64) configured[dev] = true;
+    }
+    const long long rows = 2 * c->M; const int nc = 2 * nvec, nt = (nc + kGT - 1) / kGT;
+    CSF_CUDA(c, cudaMemsetAsync(dG, 0, (size_t)nc * nc * sizeof(double), c->stream));
+    // row ranges: enough CTAs for ~4 waves of 2 CTAs per SM over the (upper-triangle) tiles
+    const int tiles = sym ? nt * (nt + 1) / 2 : nt * nt;
+    long long nsplit = std::max<long long>(1, std::min<long long>((8LL * c->sm_count + tiles - 1) / tiles, (rows + 4 * kGK - 1) / (4 * kGK)));
+    nsplit = std::min<long long>(nsplit, 65535);
+    const long long rpc = ((rows + nsplit - 1) / nsplit + kGK - 1) / kGK * kGK;
+    dim3 grid(nt * nt, (unsigned)((rows + rpc - 1) / rpc));
+    { ProfScope ps(c, CSF_KIND_AUX); gram_kernel<<<grid, 256, kGramSmem, c->stream>>>(A, lda, B, ldb, nc, rows, rpc, dG, nc, sym); }
+    CSF_CUDA(c, cudaGetLastError());
+    gram_finish_kernel<<<(nvec * nvec + 255) / 256, 256, 0, c->stream>>>(dG, nc, nvec, dOut, nvec, sym);
+    CSF_CUDA(c, cudaGetLastError());
+    c->launches += 2;
+    return CSF_OK;
+}
+
+// cuSOLVER's dense Hermitian-definite eigensolver, resolved at first use (no link-time dependency)
+struct CuSolver {
+    void* lib = nullptr;
+    cusolverStatus_t (*create)(cusolverDnHandle_t*) = nullptr;
+    cusolverStatus_t (*destroy)(cusolverDnHandle_t) = nullptr;
+    cusolverStatus_t (*set_stream)(cusolverDnHandle_t, cudaStream_t) = nullptr;
+    cusolverStatus_t (*bufsize)(cusolverDnHandle_t, cusolverEigType_t, cusolverEigMode_t, cublasFillMode_t, int, const cuDoubleComplex*, int, const cuDoubleComplex*, int, const double*, int*) = nullptr;
+    cusolverStatus_t (*hegvd)(cusolverDnHandle_t, cusolverEigType_t, cusolverEigMode_t, cublasFillMode_t, int, cuDoubleComplex*, int, cuDoubleComplex*, int, double*, cuDoubleComplex*, int, int*) = nullptr;
+    bool load() {
+        if (hegvd) return true;
+        for (const char* name : {"libcusolver.so.11", "libcusolver.so", "/usr/local/cuda/lib64/libcusolver.so.11"}) { lib = dlopen(name, RTLD_NOW | RTLD_GLOBAL); if (lib) break; }
+        if (!lib) return false;
+        create = reinterpret_cast<decltype(create)>(dlsym(lib, "cusolverDnCreate"));
+        destroy = reinterpret_cast<decltype(destroy)>(dlsym(lib, "cusolverDnDestroy"));
+        set_stream = reinterpret_cast<decltype(set_stream)>(dlsym(lib, "cusolverDnSetStream"));
+        bufsize = reinterpret_cast<decltype(bufsize)>(dlsym(lib, "cusolverDnZhegvd_bufferSize"));
+        hegvd = reinterpret_cast<decltype(hegvd)>(dlsym(lib, "cusolverDnZhegvd"));
+        return create && destroy && set_stream && bufsize && hegvd;
+    }
+} g_cusolver;
+
+// dst[i][j] = conj(src[j][i]) (n x n)
+__global__ void __launch_bounds__(256) conj_transpose_kernel(const double2* __restrict__ src, double2* __restrict__ dst, int n) {
+    const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= n * n) return;
+    const int i = idx / n, j = idx % n; const double2 z = src[(long long)j * n + i];
+    dst[idx] = make_double2(z.x, -z.y);
+}
+__global__ void __launch_bounds__(256) recip_kernel(const double* __restrict__ a, double* __restrict__ o, long long n) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) o[i] = 1.0 / a[i];
+}
+
+}  // namespace
+
+extern "C" {
+
+int csf_rr_workspace_bytes(const csf_ctx* c, int nvec, size_t* bytes) {
+    if (!c || !bytes || nvec < 0) return CSF_EINVAL;
+    *bytes = block_bytes(c, nvec) + coef_bytes(c, nvec) + ctp_bytes(c, nvec) + rr_gram_bytes(nvec) + 256;
+    return CSF_OK;
+}
+
+int csf_rr_project(csf_ctx* c, const csf_c128* dX, int64_t ld, int nvec, csf_c128* dHs, csf_c128* dSs, void* d_work, size_t work_bytes) {
+    if (!c) return CSF_EINVAL;
+    CSF_GUARD_BEGIN
+    if (!dHs || !dSs) return fail(c, CSF_EINVAL, "NULL output pointer");
+    size_t need = 0; csf_rr_workspace_bytes(c, std::max(nvec, 0), &need);
+    int rc = check_block_args(c, dX, dHs, ld, nvec, d_work, work_bytes, need);
+    if (rc != CSF_OK || nvec == 0) return rc;
+    CSF_CUDA(c, cudaSetDevice(c->device));
+    char* w = static_cast<char*>(d_work);
+    double* HX = reinterpret_cast<double*>(w);                                        // [2M][nvec] complex128
+    double* dC = reinterpret_cast<double*>(w + block_bytes(c, nvec));
+    double* dCt = reinterpret_cast<double*>(w + block_bytes(c, nvec) + coef_bytes(c, nvec));
+    double* dG = reinterpret_cast<double*>(w + block_bytes(c, nvec) + coef_bytes(c, nvec) + ctp_bytes(c, nvec));
+    rc = enqueue_zero(c, HX, nvec, nvec); if (rc != CSF_OK) return rc;
+    rc = enqueue_step(c, reinterpret_cast<const double*>(dX), ld, HX, nvec, nvec, 1.0, 0, 0.0, dC, dCt); if (rc != CSF_OK) return rc;
+    const double* Xr = reinterpret_cast<const double*>(dX);
+    rc = enqueue_gram(c, Xr, 2 * ld, HX, 2LL * nvec, nvec, dG, reinterpret_cast<double2*>(dHs), 1); if (rc != CSF_OK) return rc;      // Hs = X^dagger (Hhat X)
+    return enqueue_gram(c, Xr, 2 * ld, Xr, 2 * ld, nvec, dG, reinterpret_cast<double2*>(dSs), 1);                                   // Ss = X^dagger X
+    CSF_GUARD_END(c)
+}
+
+int csf_rr_solve(csf_ctx* c, const csf_c128* dHs, const csf_c128* dSs, int n, csf_c128* dQ, double* lambda_host) {
+    if (!c) return CSF_EINVAL;
+    CSF_GUARD_BEGIN
+    if (!dHs || !dSs || !dQ || !lambda_host || n < 1) return fail(c, CSF_EINVAL, "bad argument");
+    CSF_CUDA(c, cudaSetDevice(c->device));
+    if (!g_cusolver.load()) return fail(c, CSF_EUNSUPPORTED, "libcusolver not found");
+    cusolverDnHandle_t h = nullptr;
+    if (g_cusolver.create(&h) != CUSOLVER_STATUS_SUCCESS) return fail(c, CSF_ECUDA, "cusolverDnCreate failed");
+    g_cusolver.set_stream(h, c->stream);
+    // The row-major Hermitian matrices are the conjugates of the column-major ones cuSOLVER sees: conj(Hs) y = lambda conj(Ss) y,
+    // so the wanted eigenvectors are q = conj(y), and Q[i][j] = q_j[i] = conj(V_colmajor(i, j)): a conjugate transpose of the buffer.
+    DevBuf a, b, wv, work, info;
+    const size_t nn = (size_t)n * n * sizeof(double2);
+    int rc = CSF_OK;
+    cudaError_t e = a.alloc(nn); if (e == cudaSuccess) e = b.alloc(nn); if (e == cudaSuccess) e = wv.alloc((size_t)n * sizeof(double)); if (e == cudaSuccess) e = info.alloc(sizeof(int));
+    if (e != cudaSuccess) { g_cusolver.destroy(h); return cuda_fail(c, e, "cudaMalloc"); }
+    cudaMemcpyAsync(a.p, dHs, nn, cudaMemcpyDeviceToDevice, c->stream); cudaMemcpyAsync(b.p, dSs, nn, cudaMemcpyDeviceToDevice, c->stream);
+    int lwork = 0;
+    if (g_cusolver.bufsize(h, CUSOLVER_EIG_TYPE_1, CUSOLVER_EIG_MODE_VECTOR, CUBLAS_FILL_MODE_LOWER, n, a.as<cuDoubleComplex>(), n, b.as<cuDoubleComplex>(), n, wv.as<double>(), &lwork) != CUSOLVER_STATUS_SUCCESS)
+        rc = fail(c, CSF_ECUDA, "cusolverDnZhegvd_bufferSize failed");
+    if (rc == CSF_OK && work.alloc((size_t)std::max(lwork, 1) * sizeof(double2)) != cudaSuccess) rc = fail(c, CSF_ENOMEM, "cudaMalloc failed");
+    if (rc == CSF_OK && g_cusolver.hegvd(h, CUSOLVER_EIG_TYPE_1, CUSOLVER_EIG_MODE_VECTOR, CUBLAS_FILL_MODE_LOWER, n, a.as<cuDoubleComplex>(), n, b.as<cuDoubleComplex>(), n,
+                                         wv.as<double>(), work.as<cuDoubleComplex>(), lwork, info.as<int>()) != CUSOLVER_STATUS_SUCCESS)
+        rc = fail(c, CSF_ECUDA, "cusolverDnZhegvd failed");
+    int hinfo = 0;
+    if (rc == CSF_OK) {
+        conj_transpose_kernel<<<(n * n + 255) / 256, 256, 0, c->stream>>>(a.as<double2>(), reinterpret_cast<double2*>(dQ), n);
+        cudaMemcpyAsync(lambda_host, wv.p, (size_t)n * sizeof(double), cudaMemcpyDeviceToHost, c->stream);
+        cudaMemcpyAsync(&hinfo, info.p, sizeof(int), cudaMemcpyDeviceToHost, c->stream);
+        e = cudaStreamSynchronize(c->stream);
+        if (e != cudaSuccess) rc = cuda_fail(c, e, "csf_rr_solve");
+        else if (hinfo != 0) rc = fail(c, CSF_EINVAL, hinfo > n ? "X^dagger X is not positive definite (linearly dependent block)" : "eigensolver did not converge");
+    } else cudaStreamSynchronize(c->stream);
+    g_cusolver.destroy(h);
+    return rc;
+    CSF_GUARD_END(c)
+}
+
+int csf_rr_rotate(csf_ctx* c, const csf_c128* dX, int64_t ld, int nvec, const csf_c128* dQ, csf_c128* dU, int64_t ldu, void* d_work, size_t work_bytes) {
+    if (!c) return CSF_EINVAL;
+    CSF_GUARD_BEGIN
+    if (!dQ) return fail(c, CSF_EINVAL, "Q is NULL");
+    if (ldu < nvec) return fail(c, CSF_EINVAL, "need ldu >= nvec");
+    int rc = check_block_args(c, dX, dU, ld, nvec, d_work, work_bytes, rr_gram_bytes(std::max(nvec, 0)));
+    if (rc != CSF_OK || nvec == 0) return rc;
+    CSF_CUDA(c, cudaSetDevice(c->device));
+    double* Qt = static_cast<double*>(d_work);
+    const int k2 = 2 * nvec; const long long rows = 2 * c->M;
+    qtilde_kernel<<<(nvec * nvec + 255) / 256, 256, 0, c->stream>>>(reinterpret_cast<const double2*>(dQ), nvec, nvec, Qt, k2);
+    CSF_CUDA(c, cudaGetLastError());
+    static bool configured[64] = {};
+    int dev = 0; CSF_CUDA(c, cudaGetDevice(&dev));
+    if (dev < 0 || dev >= 64 || !configured[dev]) {
+        CSF_CUDA(c, cudaFuncSetAttribute(rotate_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRotSmem));
+        if (dev >= 0 && dev < 64) configured[dev] = true;
+    }
+    const long long rt = (rows + kGT - 1) / kGT, nct = (k2 + kGT - 1) / kGT;
+    if (rt * nct > 0x7fffffffLL) return fail(c, CSF_EUNSUPPORTED, "grid too large");
+    { ProfScope ps(c, CSF_KIND_AUX); rotate_kernel<<<(unsigned)(rt * nct), 256, kRotSmem, c->stream>>>(reinterpret_cast<const double*>(dX), 2 * ld, Qt, k2, k2, reinterpret_cast<double*>(dU), 2 * ldu, rows); }
+    CSF_CUDA(c, cudaGetLastError());
+    c->launches += 2;
+    return CSF_OK;
+    CSF_GUARD_END(c)
+}
+
+int csf_density(csf_ctx* c, const csf_c128* dX, int64_t ld, int nvec, const double* occ_host, double* d_rho_m, int accumulate) {
+    if (!c) return CSF_EINVAL;
+    CSF_GUARD_BEGIN
+    if (!dX || !occ_host || !d_rho_m) return fail(c, CSF_EINVAL, "NULL argument");
+    if (nvec < 0 || ld < nvec) return fail(c, CSF_EINVAL, "need 0 <= nvec <= ld");
+    CSF_CUDA(c, cudaSetDevice(c->device));
+    if (!c->d_inv_mass.p) {
+        std::vector<double> mass((size_t)c->M);
+        csf_mass_diag(c, mass.data());
+        DevBuf tmp; CSF_CUDA(c, tmp.upload(mass));
+        CSF_CUDA(c, c->d_inv_mass.alloc((size_t)c->M * sizeof(double)));
+        recip_kernel<<<(unsigned)((c->M + 255) / 256), 256, 0, c->stream>>>(tmp.as<double>(), c->d_inv_mass.as<double>(), c->M);
+        CSF_CUDA(c, cudaStreamSynchronize(c->stream));
+    }
+    if (nvec == 0) { if (!accumulate) CSF_CUDA(c, cudaMemsetAsync(d_rho_m, 0, (size_t)c->M * 4 * sizeof(double), c->stream)); return CSF_OK; }
+    if (c->d_occ.bytes < (size_t)nvec * sizeof(double)) CSF_CUDA(c, c->d_occ.alloc((size_t)nvec * sizeof(double)));
+    CSF_CUDA(c, cudaMemcpyAsync(c->d_occ.p, occ_host, (size_t)nvec * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+    CSF_CUDA(c, cudaStreamSynchronize(c->stream));                  // occ_host may be pageable and go out of scope
+    { ProfScope ps(c, CSF_KIND_AUX); density_kernel<<<(unsigned)((c->M + 7) / 8), 256, 0, c->stream>>>(reinterpret_cast<const double2*>(dX), ld, nvec, c->d_occ.as<double>(), c->d_inv_mass.as<double>(), c->M, d_rho_m, accumulate); }
+    CSF_CUDA(c, cudaGetLastError());
+    c->launches += 1;
+    return CSF_OK;
+    CSF_GUARD_END(c)
+}
+
+int csf_lanczos_workspace_bytes(const csf_ctx* c, size_t* bytes) {
+    if (!c || !bytes) return CSF_EINVAL;
+    *bytes = 3 * block_bytes(c, 1) + coef_bytes(c, 1) + ctp_bytes(c, 1) + 512;
+    return CSF_OK;
+}
+
+int csf_lanczos(csf_ctx* c, const csf_c128* d_v0, int k, double* alpha_host, double* beta_host, int* steps_done, void* d_work, size_t work_bytes) {
+    if (!c) return CSF_EINVAL;
+    CSF_GUARD_BEGIN
+    if (!d_v0 || !alpha_host || !beta_host || k < 1) return fail(c, CSF_EINVAL, "bad argument");
+    if (!c->have_pot) return fail(c, CSF_ESTATE, "csf_set_potential has not been called");
+    size_t need = 0; csf_lanczos_workspace_bytes(c, &need);
+    if (!d_work || work_bytes < need) return fail(c, CSF_EINVAL, "workspace too small");
+    CSF_CUDA(c, cudaSetDevice(c->device));
+    const long long n = 2 * c->M; const size_t vb = block_bytes(c, 1);
+    char* w8 = static_cast<char*>(d_work);
+    double2* v = reinterpret_cast<double2*>(w8); double2* vprev = reinterpret_cast<double2*>(w8 + vb); double2* w = reinterpret_cast<double2*>(w8 + 2 * vb);
+    double* dC = reinterpret_cast<double*>(w8 + 3 * vb); double* dCt = reinterpret_cast<double*>(w8 + 3 * vb + coef_bytes(c, 1));
+    double* scratch = reinterpret_cast<double*>(w8 + 3 * vb + coef_bytes(c, 1) + ctp_bytes(c, 1));
+    const int grid = c->sm_count * 8;
+    double hs[2] = {0.0, 0.0};
+    // v = v0 / |v0|, vprev = 0
+    CSF_CUDA(c, cudaMemsetAsync(scratch, 0, 2 * sizeof(double), c->stream));
+    CSF_CUDA(c, cudaMemsetAsync(v, 0, vb, c->stream));
+    CSF_CUDA(c, cudaMemcpyAsync(w, d_v0, vb, cudaMemcpyDeviceToDevice, c->stream));
+    lanczos_b_kernel<<<grid, 256, 0, c->stream>>>(w, v, 0.0, n, scratch);
+    CSF_CUDA(c, cudaMemcpyAsync(hs, scratch, 2 * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    CSF_CUDA(c, cudaStreamSynchronize(c->stream));
+    if (!(hs[1] > 0.0)) return fail(c, CSF_EINVAL, "start vector is zero");
+    lanczos_c_kernel<<<grid, 256, 0, c->stream>>>(vprev, v, w, 1.0 / std::sqrt(hs[1]), n);        // vprev = 0, v = v0 / |v0|
+    double beta = 0.0; int done = 0;
+    for (int j = 0; j < k; ++j) {
+        int rc = enqueue_zero(c, reinterpret_cast<double*>(w), 1, 1); if (rc != CSF_OK) return rc;
+        rc = enqueue_step(c, reinterpret_cast<const double*>(v), 1, reinterpret_cast<double*>(w), 1, 1, 1.0, 0, 0.0, dC, dCt); if (rc != CSF_OK) return rc;
+        CSF_CUDA(c, cudaMemsetAsync(scratch, 0, 2 * sizeof(double), c->stream));
+        lanczos_a_kernel<<<grid, 256, 0, c->stream>>>(w, vprev, v, beta, n, scratch);
+        CSF_CUDA(c, cudaMemcpyAsync(hs, scratch, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+        CSF_CUDA(c, cudaStreamSynchronize(c->stream));
+        const double alpha = hs[0];
+        lanczos_b_kernel<<<grid, 256, 0, c->stream>>>(w, v, alpha, n, scratch);
+        CSF_CUDA(c, cudaMemcpyAsync(hs, scratch, 2 * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+        CSF_CUDA(c, cudaStreamSynchronize(c->stream));
+        beta = std::sqrt(hs[1]);
+        alpha_host[j] = alpha; beta_host[j] = beta; done = j + 1;
+        c->launches += 3;
+        if (!(beta > 1e-300)) break;
+        lanczos_c_kernel<<<grid, 256, 0, c->stream>>>(vprev, v, w, 1.0 / beta, n);
+    }
+    CSF_CUDA(c, cudaGetLastError());
+    if (steps_done) *steps_done = done;
+    return CSF_OK;
+    CSF_GUARD_END(c)
+}
+
+int csf_tridiag_extremes(const double* alpha, const double* beta, int k, double* theta_min, double* theta_max) {
+    if (!alpha || !beta || k < 1 || !theta_min || !theta_max) return CSF_EINVAL;
+    // Sturm-sequence bisection on the symmetric tridiagonal matrix (alpha, beta[0..k-2]); Gershgorin interval first
+    double lo = alpha[0], hi = alpha[0];
+    for (int i = 0; i < k; ++i) {
+        const double r = (i > 0 ? std::fabs(beta[i - 1]) : 0.0) + (i + 1 < k ? std::fabs(beta[i]) : 0.0);
+        lo = std::min(lo, alpha[i] - r); hi = std::max(hi, alpha[i] + r);
+    }
+    auto count_below = [&](double x) {                 // number of eigenvalues < x
+        int cnt = 0; double d = 1.0;
+        for (int i = 0; i < k; ++i) {
+            const double b2 = i > 0 ? beta[i - 1] * beta[i - 1] : 0.0;
+            d = alpha[i] - x - (i > 0 ? b2 / d : 0.0);
+            if (d == 0.0) d = -1e-300;
+            if (d < 0.0) ++cnt;
+        }
+        return cnt;
+    };
+    auto kth = [&](int idx) {                          // eigenvalue number idx (0-based, ascending)
+        double a = lo, b = hi;
+        for (int it = 0; it < 200 && b - a > 4e-16 * std::max(std::fabs(a), std::fabs(b)); ++it) {
+            const double m = 0.5 * (a + b);
+            if (count_below(m) > idx) b = m; else a = m;
+        }
+        return 0.5 * (a + b);
+    };
+    *theta_min = kth(0); *theta_max = kth(k - 1);
     return CSF_OK;
 }
 
