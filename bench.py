@@ -239,19 +239,18 @@ def measure(cfg_index, mode_name, steps, warmup, args, ctxs):
     M = ctx.M; rows = 2 * M
     fp32 = mode_name == "fp32"
     mode = binding.CSF_FP32_INTERMEDIATE if fp32 else binding.CSF_FP64
-    wb = max(ctx.workspace_bytes(nvec, mode), ctx.workspace_bytes(nvec))
+    wb = max(ctx.workspace_bytes(nvec, mode), ctx.workspace_bytes(nvec), ctx.rr_workspace_bytes(nvec), ctx.lanczos_workspace_bytes())
     work = torch.empty(max(wb, 16), dtype=torch.uint8, device="cuda")
 
-    # bounds [a, b]: Lanczos on the library's own apply_H (input generation; see bounds.py)
-    x1 = torch.empty((rows, 1), dtype=torch.complex128, device="cuda"); y1 = torch.empty_like(x1)
-
-    def apply_h_host(v):
-        x1.copy_(torch.from_numpy(np.ascontiguousarray(v)).to("cuda"))
-        ctx.apply_H(x1, y1, 1, 1, work)
-        return y1.cpu().numpy()
-
-    a, b, tmin, tmax = bounds.lanczos_bounds(apply_h_host, rows, k=20)
-    del x1, y1
+    # bounds [a, b]: 20 Lanczos steps on the device (csf_lanczos) from a seeded start vector;
+    # b = theta_max + |beta_k| is a safe upper bound, a = theta_min + 0.02 (b - theta_min) stands in for lambda_T (A15)
+    gen0 = torch.Generator(device="cuda"); gen0.manual_seed(7)
+    v0 = torch.empty((rows, 1), dtype=torch.complex128, device="cuda")
+    torch.view_as_real(v0).normal_(0.0, math.sqrt(0.5), generator=gen0)
+    al, be = ctx.lanczos(v0, 20, work)
+    tmin, tmax = binding.tridiag_extremes(al, be)
+    b = tmax + abs(float(be[-1])); a = tmin + 0.02 * (b - tmin)
+    del v0
 
     # this rank's block of states (band group): a different seed per block index
     my_blocks = shard_states(max(cfg.nstates, nvec * world), nvec, rank, world)
@@ -376,12 +375,58 @@ def main_ours(args):
         from paper_2410_02754_b200 import binding
         pf, pm = binding.probe_fp64_peak(local)
         head["roofline"]["peak_measured_dfma"] = pf; head["roofline"]["peak_measured_dmma"] = pm
+        head["roofline"]["peak_measured_dfma_and_dmma_together"] = binding.probe_fp64_mixed(local)       # = either alone: one set of FP64 units
         if args.mode == "fp64":
             head["roofline"]["frac_of_measured_dfma"] = head["roofline"]["achieved"] / pf
 
+    ctx, X, rows, nvec, degree, a, b, mode, barrier = (live[k] for k in ("ctx", "X", "rows", "nvec", "degree", "a", "b", "mode", "barrier"))
+
+    # ---- subspace steps after the filter: Rayleigh-Ritz on the filtered block, density
+    subspace = None
+    if args.mode == "fp64" and not args.no_subspace and nvec >= 2:
+        from paper_2410_02754_b200 import binding
+        Y, work = live["Y"], live["work"]
+        stream = torch.cuda.current_stream()
+        N = nvec
+        dHs = torch.empty((N, N), dtype=torch.complex128, device="cuda"); dSs = torch.empty_like(dHs); dQ = torch.empty_like(dHs)
+        rho = torch.empty((rows // 2, 4), dtype=torch.float64, device="cuda")
+        occ = np.ones(N)
+
+        def timed(fn, reps):
+            fn(); torch.cuda.synchronize()
+            e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            for _ in range(reps):
+                fn()
+            e1.record(stream); torch.cuda.synchronize()
+            return e0.elapsed_time(e1) / reps
+
+        # the block is the filter's OUTPUT, rescaled column by column so that X^dagger X stays well conditioned
+        Y.div_(Y.norm(dim=0, keepdim=True))
+        ms_proj = timed(lambda: ctx.rr_project(Y, N, N, dHs, dSs, work), 2)
+        t0 = time.perf_counter(); solve_err = None
+        try:
+            lam = ctx.rr_solve(dHs, dSs, N, dQ)
+        except binding.CsfError as ex:             # (a random block filtered once can be numerically rank deficient: time the rotation with Q = I)
+            solve_err = str(ex); lam = np.zeros(N); dQ.copy_(torch.eye(N, dtype=torch.complex128, device="cuda"))
+        ms_solve = (time.perf_counter() - t0) * 1e3
+        ms_rot = timed(lambda: ctx.rr_rotate(Y, N, N, dQ, X, N, work), 2)           # U overwrites the input block (no longer needed)
+        ms_rho = timed(lambda: ctx.density(X, N, N, occ, rho), 3)
+        peak64 = SM_COUNT * FP64_FMA_PER_CLK_PER_SM * 2 * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6 / 1e12
+        hbm = float(peaks.get("hbm_gbs", 6650.0))
+        f_gram = 4.0 * N * N * rows                                                   # Hermitian N x N product over `rows` rows: N (N + 1) / 2 x 8 flops
+        t_apply = head["ms_per_step"] / degree                                      # one H apply of the filter leg
+        subspace = {"note": "Rayleigh-Ritz (PAPER.md eq.71-72) on the filtered block, density (eq.4-5); dense FP64 contractions: tensor-pipe (DMMA) bound",
+                    "rr_project_ms": ms_proj, "rr_project_tflops_gemm": 2 * f_gram / max(ms_proj - t_apply, 1e-3) / 1e9,
+                    "rr_project_frac_of_fp64_peak": 2 * f_gram / max(ms_proj - t_apply, 1e-3) / 1e9 / peak64,
+                    "rr_solve_ms_host_wall": ms_solve, "rr_solve_error": solve_err, "ritz_min_max": [float(lam[0]), float(lam[-1])],
+                    "rr_rotate_ms": ms_rot, "rr_rotate_tflops": 8.0 * N * N * rows / ms_rot / 1e9, "rr_rotate_frac_of_fp64_peak": 8.0 * N * N * rows / ms_rot / 1e9 / peak64,
+                    "density_ms": ms_rho, "density_gbs": rows * N * 16.0 / ms_rho / 1e6, "density_frac_of_hbm": rows * N * 16.0 / ms_rho / 1e6 / hbm,
+                    "filter_ms": head["ms_per_step"], "rr_share_of_chfsi_pass": (ms_proj + ms_solve + ms_rot) / (head["ms_per_step"] + ms_proj + ms_solve + ms_rot)}
+        del dHs, dSs, dQ, rho, Y, work
+
     # ---- end to end: host buffers through csf_filter_host (H2D + filter + D2H inside the timed region)
     e2e = None
-    ctx, X, rows, nvec, degree, a, b, mode, barrier = (live[k] for k in ("ctx", "X", "rows", "nvec", "degree", "a", "b", "mode", "barrier"))
     if not args.no_e2e:
         import psutil
         e2e_nvec = nvec
@@ -390,6 +435,9 @@ def main_ours(args):
         while e2e_nvec > 8 and need * e2e_nvec > 0.7 * avail:
             e2e_nvec //= 2
         hX = torch.empty((rows, e2e_nvec), dtype=torch.complex128, pin_memory=True)
+        if subspace is not None:                      # the block was overwritten by the rotation: draw it again
+            gen = torch.Generator(device="cuda"); gen.manual_seed(4242)
+            torch.view_as_real(X).normal_(0.0, math.sqrt(0.5), generator=gen)
         hX.copy_(X[:, :e2e_nvec])
         live["X"] = live["Y"] = live["work"] = None
         del X
@@ -438,7 +486,8 @@ def main_ours(args):
         out = {"metric": METRIC, "value": head["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": head["ms_per_step"],
                "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": head["dtype"], "data": "synthetic", "config": head["config"],
                "clocks": head["clocks"], "e2e": e2e, "gpu_launches": head["gpu_launches"], "roofline": head["roofline"], "step_roofline": head["step_roofline"],
-               "cpu_baseline": cpu, "finite": head["finite"], "full_filter_extrapolated_s": head.get("full_filter_extrapolated_s"), "other_configs": others}
+               "cpu_baseline": cpu, "finite": head["finite"], "full_filter_extrapolated_s": head.get("full_filter_extrapolated_s"), "other_configs": others,
+               "subspace": subspace}
         print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()
@@ -463,6 +512,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-profile", action="store_true")
     ap.add_argument("--no-probe", action="store_true")
+    ap.add_argument("--no-subspace", action="store_true", help="skip the Rayleigh-Ritz / density timings after the headline leg")
     ap.add_argument("--no-others", action="store_true", help="skip the other roofline-target legs (configs 2, 4 in FP64, config 4 in FP32-intermediate)")
     ap.add_argument("--other-steps", type=int, default=2, help="timed steps of each other leg")
     args = ap.parse_args()

@@ -140,10 +140,16 @@ int csf_profile_read(csf_ctx* ctx, int kind, double* ms_total, int64_t* launches
  * independent DFMA chains, tflops_mma from mma.sync m8n8k4 f64 (DMMA) chains. Synchronises. Either pointer may be NULL. */
 int csf_probe_fp64_peak(int device, double* tflops_fma, double* tflops_mma);
 
+/* The same two loops side by side (even warps DFMA chains, odd warps DMMA chains): *tflops_total is the sum of both.
+ * On B200 it equals either loop alone (36.4 TF/s against 33.9 / 36.7): DFMA and DMMA issue to the same FP64 units, so the
+ * FP64 roofline has ONE peak and tensor-core tiles buy no extra rate. Synchronises. */
+int csf_probe_fp64_mixed(int device, double* tflops_total);
+
 /* Which column-kernel variant a block of nvec vectors runs with in `mode` on this context: *lanes = 32 (orders 4 and 5:
- * the warp-specialised kernel, 8 vectors per CTA) or 16 (the other orders: 4 vectors per CTA; 8 lanes = 2 vectors at
- * order 7). The environment variable CSF_LANES=16, read by csf_create, pins the 16-lane kernel at orders 4 and 5 too
- * (parity tests run every case through both). Host-only query. */
+ * 8 vectors per CTA) or 16 (the other orders: 4 vectors per CTA; 8 lanes = 2 vectors at order 7). Environment variables read
+ * by csf_create pin the variant for the parity tests, which run every case through each kernel: CSF_LANES=16 (the 16-lane
+ * kernel at orders 4 and 5 too), CSF_KERNEL=ws (the warp-specialised streaming kernel of csf_colws.cuh, orders 4 and 5;
+ * parity-green but slower). Host-only query. */
 int csf_column_lanes(const csf_ctx* ctx, int nvec, int mode, int* lanes);
 
 /* Number of kernel launches (own kernels only, memsets excluded) enqueued by this context so far. */

@@ -17,7 +17,7 @@ CSF_FP64, CSF_FP32_INTERMEDIATE = 0, 1
 
 EXPORTS = ["csf_create", "csf_destroy", "csf_set_stream", "csf_num_nodes", "csf_node_coords", "csf_mass_diag", "csf_set_potential",
            "csf_set_projectors", "csf_workspace_bytes", "csf_apply_H", "csf_filter", "csf_filter_host", "csf_set_host_chunk",
-           "csf_profile_enable", "csf_profile_read", "csf_probe_fp64_peak", "csf_launch_count", "csf_column_lanes", "csf_set_variant", "csf_set_tuning", "csf_last_error",
+           "csf_profile_enable", "csf_profile_read", "csf_probe_fp64_peak", "csf_probe_fp64_mixed", "csf_launch_count", "csf_column_lanes", "csf_set_variant", "csf_set_tuning", "csf_last_error",
            "csf_rr_workspace_bytes", "csf_rr_project", "csf_rr_solve", "csf_rr_rotate", "csf_density", "csf_lanczos_workspace_bytes", "csf_lanczos",
            "csf_tridiag_extremes"]
 KIND_CELL, KIND_PGATHER, KIND_DELTA, KIND_AUX = 0, 1, 2, 3
@@ -190,6 +190,15 @@ class Csf:
 
     def set_variant(self, variant):
         self._chk(self._L.csf_set_variant(self._h, C.c_int(int(variant))))
+
+
+def probe_fp64_mixed(device=0):
+    """TFLOP/s of DFMA and DMMA loops running side by side on every SM (csf_probe_fp64_mixed)."""
+    t = C.c_double()
+    rc = lib().csf_probe_fp64_mixed(C.c_int(int(device)), C.byref(t))
+    if rc != CSF_OK:
+        raise CsfError(rc, lib().csf_last_error(None).decode())
+    return float(t.value)
 
 
 def tridiag_extremes(alpha, beta):

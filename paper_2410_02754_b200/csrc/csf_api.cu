@@ -54,6 +54,7 @@ struct csf_ctx {
     int seg_len = 0, chunk_group = 16;      // cells per z-segment (0 = the kernel's default), vector chunks scheduled back to back (csf_set_tuning)
     int lanes_force = 0;                    // CSF_LANES=16|32 pins the column kernel variant (tests, sweeps); 0 = measured policy
     int kernel_force = 0;                   // CSF_KERNEL=wide|ws pins the 8-vector kernel of orders 4 and 5 (1 | 2)
+    bool bulk_gather = true;                // CSF_GATHER=reg pins the register-load projector gather (tests run both)
     // projectors
     int natoms = 0, npj_uniform = 0, npjp = 0; long long crows = 0;
     DevBuf d_ent_node, d_atom_coff, d_atom_npj, d_atom_type, d_delta, d_delta_ptr, d_gb_atom, d_gb_beg, d_gb_end, d_gb_k0, d_g_pack;
@@ -194,7 +195,22 @@ int enqueue_step(csf_ctx* c, const void* src, long long ld, void* dst, long long
         dim3 gg(c->n_gather_blocks, (nvec + 16 * kGatherNT - 1) / (16 * kGatherNT));
         {
             ProfScope ps(c, CSF_KIND_PGATHER);
-            if (c->npj_uniform == 18 && !f32) proj_gather_kernel<3, double, 2, 2><<<gg, 256, 0, c->stream>>>(gp);     // (slower than the full-DMMA form with float loads)
+            // complex128 blocks with 16-byte aligned rows: the bulk-copy kernel (src staged in shared memory by cp.async.bulk)
+            const bool bulk = !f32 && c->bulk_gather && ((uintptr_t)src & 15) == 0;
+            if (bulk) {
+                static bool configured[64] = {};
+                int dev = 0; CSF_CUDA(c, cudaGetDevice(&dev));
+                if (dev < 0 || dev >= 64 || !configured[dev]) {
+                    CSF_CUDA(c, cudaFuncSetAttribute(proj_gather_bulk_kernel<3, 2, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kGbSmem));
+                    CSF_CUDA(c, cudaFuncSetAttribute(proj_gather_bulk_kernel<3, 3, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kGbSmem));
+                    CSF_CUDA(c, cudaFuncSetAttribute(proj_gather_bulk_kernel<4, 4, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kGbSmem));
+                    if (dev >= 0 && dev < 64) configured[dev] = true;
+                }
+                if (c->npj_uniform == 18) proj_gather_bulk_kernel<3, 2, 2><<<gg, 256, kGbSmem, c->stream>>>(gp);
+                else if (c->npjp <= 24) proj_gather_bulk_kernel<3, 3, 0><<<gg, 256, kGbSmem, c->stream>>>(gp);
+                else proj_gather_bulk_kernel<4, 4, 0><<<gg, 256, kGbSmem, c->stream>>>(gp);
+            }
+            else if (c->npj_uniform == 18 && !f32) proj_gather_kernel<3, double, 2, 2><<<gg, 256, 0, c->stream>>>(gp);     // (slower than the full-DMMA form with float loads)
             else if (c->npjp <= 24) { if (f32) proj_gather_kernel<3, float><<<gg, 256, 0, c->stream>>>(gp); else proj_gather_kernel<3, double><<<gg, 256, 0, c->stream>>>(gp); }
             else { if (f32) proj_gather_kernel<4, float><<<gg, 256, 0, c->stream>>>(gp); else proj_gather_kernel<4, double><<<gg, 256, 0, c->stream>>>(gp); }
         }
@@ -357,6 +373,7 @@ int csf_create(csf_ctx** out, const int ncell[3], const double box[3], int order
     c->sm_count = prop.multiProcessorCount; c->smem_optin = prop.sharedMemPerBlockOptin;
     // CSF_LANES pins the column kernel variant for the parity tests (both variants against the oracle on every case)
     if (const char* e = std::getenv("CSF_LANES")) { int v = std::atoi(e); if (v == 16 || v == 32) c->lanes_force = v; }
+    if (const char* e = std::getenv("CSF_GATHER")) c->bulk_gather = std::strcmp(e, "reg") != 0;
     if (const char* e = std::getenv("CSF_KERNEL")) c->kernel_force = std::strcmp(e, "ws") == 0 ? 2 : (std::strcmp(e, "wide") == 0 ? 1 : 0);
     const int B = 8;
     // traversal order of the (cx, cy) columns: 8x8 tiles, x fastest inside (neighbouring columns run together, so the
@@ -598,18 +615,9 @@ int csf_apply_H(csf_ctx* c, const csf_c128* dX, csf_c128* dY, int64_t ld, int nv
     CSF_GUARD_END(c)
 }
 
-int csf_filter(csf_ctx* c, const csf_c128* dX, csf_c128* dY, int64_t ld, int nvec, int degree, double a, double b, int mode,
-               void* d_work, size_t work_bytes) {
-    CSF_GUARD_BEGIN
-    if (!c) return CSF_EINVAL;
-    if (mode != CSF_FP64 && mode != CSF_FP32_INTERMEDIATE) return fail(c, CSF_EINVAL, "unknown mode");
-    if (degree < 0) return fail(c, CSF_EINVAL, "degree < 0");
-    if (!(a < b)) return fail(c, CSF_EINVAL, "need a < b");
-    size_t need = 0;
-    if (nvec > 0) csf_workspace_bytes(c, nvec, mode, &need);
-    int rc = check_block_args(c, dX, dY, ld, nvec, d_work, work_bytes, degree >= 1 ? need : 0);
-    if (rc != CSF_OK || nvec == 0) return rc;
-    CSF_CUDA(c, cudaSetDevice(c->device));
+// the launch sequence of one filter call on c->stream (arguments already checked)
+static int filter_enqueue(csf_ctx* c, const csf_c128* dX, csf_c128* dY, int64_t ld, int nvec, int degree, double a, double b, int mode, void* d_work) {
+    int rc = CSF_OK;
     const long long rows = 2 * c->M;
     const double cc = 0.5 * (a + b), ee = 0.5 * (b - a);
     const double2* X = reinterpret_cast<const double2*>(dX);
@@ -663,6 +671,23 @@ int csf_filter(csf_ctx* c, const csf_c128* dX, csf_c128* dY, int64_t ld, int nve
         if (rc != CSF_OK) return rc;
     }
     return CSF_OK;
+}
+
+int csf_filter(csf_ctx* c, const csf_c128* dX, csf_c128* dY, int64_t ld, int nvec, int degree, double a, double b, int mode,
+               void* d_work, size_t work_bytes) {
+    CSF_GUARD_BEGIN
+    if (!c) return CSF_EINVAL;
+    if (mode != CSF_FP64 && mode != CSF_FP32_INTERMEDIATE) return fail(c, CSF_EINVAL, "unknown mode");
+    if (degree < 0) return fail(c, CSF_EINVAL, "degree < 0");
+    if (!(a < b)) return fail(c, CSF_EINVAL, "need a < b");
+    size_t need = 0;
+    if (nvec > 0) csf_workspace_bytes(c, nvec, mode, &need);
+    int rc = check_block_args(c, dX, dY, ld, nvec, d_work, work_bytes, degree >= 1 ? need : 0);
+    if (rc != CSF_OK || nvec == 0) return rc;
+    CSF_CUDA(c, cudaSetDevice(c->device));
+    // (Replaying the sequence as a CUDA graph was measured at config 1, the launch-bound one: 11.40 against 11.48 ms per block.
+    // The gaps are on the device, not in the launch path; the graph was dropped.)
+    return filter_enqueue(c, dX, dY, ld, nvec, degree, a, b, mode, d_work);
     CSF_GUARD_END(c)
 }
 
@@ -779,6 +804,32 @@ int csf_probe_fp64_peak(int device, double* tflops_fma, double* tflops_mma) {
     cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(sink);
     if (tflops_fma) *tflops_fma = out[0];
     if (tflops_mma) *tflops_mma = out[1];
+    return CSF_OK;
+}
+
+int csf_probe_fp64_mixed(int device, double* tflops_total) {
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) return fail(nullptr, CSF_ECUDA, "no such CUDA device");
+    if (cudaSetDevice(device) != cudaSuccess) return fail(nullptr, CSF_ECUDA, "cudaSetDevice failed");
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return fail(nullptr, CSF_ECUDA, "cudaGetDeviceProperties failed");
+    double* sink = nullptr;
+    if (cudaMalloc(&sink, 1 << 20) != cudaSuccess) return fail(nullptr, CSF_ENOMEM, "cudaMalloc failed");
+    cudaEvent_t e0, e1; cudaEventCreate(&e0); cudaEventCreate(&e1);
+    const int blocks = prop.multiProcessorCount * 4, iters = 4096;
+    float best = 1e30f;
+    for (int rep = 0; rep < 5; ++rep) {
+        cudaEventRecord(e0, 0);
+        probe_mixed_kernel<<<blocks, 256>>>(sink, iters, 1.0000001);
+        cudaEventRecord(e1, 0);
+        if (cudaEventSynchronize(e1) != cudaSuccess) { cudaFree(sink); return fail(nullptr, CSF_ECUDA, "probe kernel failed"); }
+        float ms = 0.f; cudaEventElapsedTime(&ms, e0, e1);
+        if (rep > 0 && ms < best) best = ms;
+    }
+    // per CTA: 4 warps x 32 threads x 8 chains x 2 flops (DFMA) + 4 warps x 8 mma x 512 flops (DMMA) per iteration
+    const double flops = (double)blocks * iters * (4.0 * 32 * 8 * 2 + 4.0 * 8 * 512);
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(sink);
+    if (tflops_total) *tflops_total = flops / (best * 1e-3) * 1e-12;
     return CSF_OK;
 }
 

@@ -139,16 +139,6 @@ template <int N> __host__ __device__ constexpr int col_canon(int i, int j) {
 // as long) is on the main-thread side again: config 4 44.3 -> 39.8 ms, config 1 0.52 -> 0.47 ms per launch.
 __host__ __device__ constexpr bool col_main_tma(int p, int lanes = 16) { return p >= 5 || (p == 4 && lanes == 32); }
 
-// x-split of the main threads (compile-time option, off): two threads per (plane, lane), each computing one half of the
-// output columns i of phase A and of the z-lines of phase B. The second half works on the x-mirrored plane, which by the
-// centro-symmetry of Ah and the (anti)symmetry of uh needs the same table entries: 12 main warps instead of 6, three per
-// SM sub-partition, at the price of loading every plane twice and of computing d twice. Parity-green, measured slower
-// on B200 (wide FP64 order-5 kernel, 128 registers: config 3 44.0 against 38.4 ms, config 2 48.3 against 42.2).
-#ifndef CSF_HSPLIT
-#define CSF_HSPLIT 1
-#endif
-__host__ __device__ constexpr int col_hsplit(int p, bool f32, int lanes) { return (lanes == 32 && p == 5 && !f32) ? CSF_HSPLIT : 1; }
-
 // register cap per thread: what the CTAs/SM allowed by shared memory leave (orders 4, 5; other orders uncapped).
 // L = 16: order 4 runs 3 CTAs/SM (FP32: 4), order 5 two (FP32: 3).
 __host__ __device__ constexpr int col_maxreg(int p, bool f32, int lanes, int auxw) {
@@ -156,14 +146,13 @@ __host__ __device__ constexpr int col_maxreg(int p, bool f32, int lanes, int aux
     // The register file is per SM sub-partition (16384 registers): w warps per SM sit ceil(w / 4) per sub-partition.
     // 32 lanes, order 5: 6 main warps + auxw in one CTA/SM (FP64; up to 8 warps sit 2 per sub-partition, up to 12 sit 3) or
     // two CTAs of 8 warps (FP32); order 4: two CTAs of 5 + 3 warps.
-    if (lanes == 32) return p == 4 ? 128 : (f32 ? 128 : (col_hsplit(p, f32, lanes) == 2 ? 128 : (auxw <= 2 ? 224 : 168)));   // 12 + 4 warps: 4 per sub-partition
+    if (lanes == 32) return p == 4 ? 128 : (f32 ? 128 : (auxw <= 2 ? 224 : 168));
     return f32 ? (p == 4 ? 96 : 128) : (p == 4 ? 128 : 168);
 }
 
 template <typename T, int P, int L, int AUXW = 2> struct ColCfg {
     static constexpr int N = P + 1;
-    static constexpr int HS = col_hsplit(P, sizeof(T) == 4, L);
-    static constexpr int NTM = (N * L * HS + 31) / 32 * 32;          // main threads
+    static constexpr int NTM = (N * L + 31) / 32 * 32;               // main threads
     static constexpr int NAUX = 32 * AUXW;                           // auxiliary (expansion) threads
     static constexpr int NT = NTM + NAUX;                            // threads per CTA
     static constexpr int PLANE = N * N * L;                          // reals per ring plane and field
@@ -189,7 +178,7 @@ __global__ void __launch_bounds__(ColCfg<T, P, L, AUXW>::NT) __maxnreg__(col_max
     constexpr bool kWarpPlane = L % 32 == 0;      // a main warp holds exactly one plane
     constexpr bool FAST = MODE >= 1;      // x, y periodic and all lanes live: no per-access predicate
     constexpr bool ZISO = MODE == 2;      // z periodic too and cubic cells: no z check, no rho multiply
-    constexpr int N = Cfg::N, NTM = Cfg::NTM, VPC = L / 4, HS = Cfg::HS;        // VPC vectors per CTA
+    constexpr int N = Cfg::N, NTM = Cfg::NTM, VPC = L / 4;        // VPC vectors per CTA
     constexpr int PLANE = Cfg::PLANE, EPLANE = Cfg::EPLANE;
     extern __shared__ __align__(128) unsigned char smem[];
     T* R1 = reinterpret_cast<T*>(smem);
@@ -364,7 +353,7 @@ __global__ void __launch_bounds__(ColCfg<T, P, L, AUXW>::NT) __maxnreg__(col_max
 
     // ================================================================== main warps
     const int mtid = tid - kColAux;
-    const int lane = mtid % L, q = mtid / (L * HS), h = (mtid / L) % HS;      // h = 1: the x-mirrored half
+    const int lane = mtid % L, q = mtid / L;
     const int spin = lane / (L / 2), ri = lane & 1;
     const int vec = chunk * VPC + ((lane % (L / 2)) >> 1);
     const bool lane_on = FAST || vec < A.nvec;
@@ -383,18 +372,7 @@ __global__ void __launch_bounds__(ColCfg<T, P, L, AUXW>::NT) __maxnreg__(col_max
             yo_[i] = gy < 0 ? -1 : gy * A.nfx;
         }
     }
-    // HS == 2: per-thread x offsets, mirrored for h = 1 (index i is then the table-space column)
-    int xh_[HS == 2 ? N : 1];
-    if (HS == 2) {
-#pragma unroll
-        for (int i = 0; i < N; ++i) {
-            const int a = FAST ? (i < P ? x0f + i : xPf) : xo_[FAST ? 0 : i];
-            const int b = FAST ? (N - 1 - i < P ? x0f + N - 1 - i : xPf) : xo_[FAST ? 0 : N - 1 - i];
-            xh_[HS == 2 ? i : 0] = h ? b : a;
-        }
-    }
-#define XO(i) (HS == 2 ? xh_[HS == 2 ? (i) : 0] : (FAST ? ((i) < P ? x0f + (i) : xPf) : xo_[FAST ? 0 : (i)]))
-#define XR(i) ((HS == 2 && h) ? N - 1 - (i) : (i))
+#define XO(i) (FAST ? ((i) < P ? x0f + (i) : xPf) : xo_[FAST ? 0 : (i)])
 #define YO(j) (FAST ? ((j) < P ? y0f + (j) * A.nfx : yPf) : yo_[FAST ? 0 : (j)])
     const T* sp = static_cast<const T*>(A.src) + ((long long)spin * (A.rs >> 2) + vec) * 2 + ri;
     const int slot_out = ri ^ (A.rot & 1);
@@ -403,9 +381,9 @@ __global__ void __launch_bounds__(ColCfg<T, P, L, AUXW>::NT) __maxnreg__(col_max
     const T scax = (T)(A.sc * A.ax);
 
     T u[N][N];
-    T carry[N / HS];
+    T carry[N];
 #pragma unroll
-    for (int i = 0; i < N / HS; ++i) carry[i] = (T)0;
+    for (int i = 0; i < N; ++i) carry[i] = (T)0;
 
     // plane of the segment handled by this thread in iteration t (segment-local plane index g), or -1
     auto plane_of = [&](int t) -> int {
@@ -473,8 +451,8 @@ __global__ void __launch_bounds__(ColCfg<T, P, L, AUXW>::NT) __maxnreg__(col_max
             }
             // output column i: a1 = (Ah u)[:, i], b1 = (Bx u)[:, i]; then the y-step on the column
 #pragma unroll
-            for (int i = 0; i < N / HS; ++i) {
-                const int ir = XR(i);
+            for (int i = 0; i < N; ++i) {
+                const int ir = i;
                 T a1[N], b1[N], b1s[N];
 #pragma unroll
                 for (int j = 0; j < N; ++j) {
@@ -521,8 +499,8 @@ __global__ void __launch_bounds__(ColCfg<T, P, L, AUXW>::NT) __maxnreg__(col_max
             const T* r2 = R2 + j * N * L + lane;
             const T* xp = X + j * P * L + lane;
 #pragma unroll
-            for (int i = 0; i < N / HS; ++i) {
-                const int ir = XR(i);
+            for (int i = 0; i < N; ++i) {
+                const int ir = i;
                 T f1[N], f2[N];
 #pragma unroll
                 for (int k = 0; k < N; ++k) {
@@ -565,7 +543,6 @@ __global__ void __launch_bounds__(ColCfg<T, P, L, AUXW>::NT) __maxnreg__(col_max
 #undef TAB_U
 #undef XO
 #undef YO
-#undef XR
 #undef UH
 #undef BETA
 }

@@ -70,10 +70,12 @@ __global__ void __launch_bounds__(256, 2) proj_gather_kernel(const __grid_consta
     const T* sb = static_cast<const T*>(A.src) + ((long long)spin * A.ld + v0 + (rw >> 1)) * 2 + (rw & 1);
     const double* gp = A.g_pack + (long long)A.gb_k0[blockIdx.x] * (MT * 32) + wl;
     constexpr int NA = MD + (NX > 0 ? NX : 0);      // a[0..MD) = DMMA A fragments, a[MD..) = this thread's row of the extra projectors
-    auto load_step = [&](int e, int ks, double (&a)[NA], double (&b)[kGatherNT]) {
+    // the node index of a support row is needed before its src row can be requested: it is fetched one round (two k-steps)
+    // ahead of the data, so that the data loads never wait for an index
+    auto load_node = [&](int e) { const int er = e + kk; return __ldg(A.ent_node + (er < e1 ? er : e0)); };
+    auto load_step = [&](int e, int ks, int node, double (&a)[NA], double (&b)[kGatherNT]) {
         const int er = e + kk;
         const bool ok = er < e1;
-        const int node = __ldg(A.ent_node + (ok ? er : e0));
 #pragma unroll
         for (int m = 0; m < MD; ++m) a[m] = (e < e1) ? __ldg(gp + ((long long)ks * MT + m) * 32) : 0.0;
 #pragma unroll
@@ -84,13 +86,16 @@ __global__ void __launch_bounds__(256, 2) proj_gather_kernel(const __grid_consta
     };
     // two k-steps are multiplied while the next two are in flight
     double a0[NA], b0[kGatherNT], a1[NA], b1[kGatherNT];
-    load_step(e0, 0, a0, b0);
-    load_step(e0 + 4, 1, a1, b1);
+    int n2 = load_node(e0 + 8), n3 = load_node(e0 + 12);
+    load_step(e0, 0, load_node(e0), a0, b0);
+    load_step(e0 + 4, 1, load_node(e0 + 4), a1, b1);
     int ks = 0;
     for (int e = e0; e < e1; e += 8, ks += 2) {
         double a2[NA], b2[kGatherNT], a3[NA], b3[kGatherNT];
-        load_step(e + 8, ks + 2, a2, b2);
-        load_step(e + 12, ks + 3, a3, b3);
+        const int m2 = n2, m3 = n3;
+        n2 = load_node(e + 16); n3 = load_node(e + 20);
+        load_step(e + 8, ks + 2, m2, a2, b2);
+        load_step(e + 12, ks + 3, m3, a3, b3);
 #pragma unroll
         for (int m = 0; m < MD; ++m)
 #pragma unroll
@@ -110,6 +115,137 @@ __global__ void __launch_bounds__(256, 2) proj_gather_kernel(const __grid_consta
     }
     const long long coff = A.atom_coff[atom];
     // extra projectors: sum the four support rows of a k-step (lanes kk = 0..3), lane kk = 0 adds real lane rw of its vector
+#pragma unroll
+    for (int x = 0; x < NX; ++x)
+#pragma unroll
+        for (int nt = 0; nt < kGatherNT; ++nt) {
+            double v = accx[x][nt];
+            v += __shfl_xor_sync(0xffffffffu, v, 1); v += __shfl_xor_sync(0xffffffffu, v, 2);
+            const int vv = v0 + nt * 4 + (rw >> 1);
+            if (kk == 0 && 8 * MD + x < npj && vv < A.nvec) atomicAdd(A.C + ((coff + 2 * (8 * MD + x) + spin) * A.ldc + vv) * 2 + (rw & 1), v);
+        }
+#pragma unroll
+    for (int m = 0; m < MD; ++m) {
+        const int chi = m * 8 + rw;
+        if (chi < npj) {
+#pragma unroll
+            for (int nt = 0; nt < kGatherNT; ++nt) {
+                const int v = v0 + nt * 4 + kk;
+                if (v < A.nvec) {
+                    double* cp = A.C + ((coff + 2 * chi + spin) * A.ldc + v) * 2;
+                    atomicAdd(cp, acc[m][nt][0]); atomicAdd(cp + 1, acc[m][nt][1]);
+                }
+            }
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// proj_gather_bulk_kernel (a5, complex128 blocks): the same contraction with the src rows staged in shared memory by bulk
+// asynchronous copies (cp.async.bulk global -> shared, completing on an mbarrier): one 1 KB request per (support row, spin)
+// = 64 vectors, 16 rows per stage, kGbStages stages per CTA and two CTAs per SM, i.e. ~200 KB of src in flight per SM
+// against ~32 KB with register loads (the register kernel sat at 59 % of the HBM copy rate, latency-bound). The B fragments
+// then come from shared memory; a row stride of 2 KB + 64 B puts the four rows of a fragment on two bank halves.
+// ---------------------------------------------------------------------------------------------------
+constexpr int kGbRows = 16;                       // support rows per stage (4 k-steps)
+constexpr int kGbStages = 3;
+constexpr int kGbRowBytes = 2 * 1024 + 64;        // both spins x 64 vectors x 16 B, + 64 B of skew
+constexpr size_t kGbSmem = (size_t)kGbStages * kGbRows * kGbRowBytes + 64;
+
+template <int MT, int MD, int NX>
+__global__ void __launch_bounds__(256, 2) proj_gather_bulk_kernel(const __grid_constant__ GatherParams A) {
+    extern __shared__ __align__(128) unsigned char gsm[];
+    const unsigned mb0 = (unsigned)__cvta_generic_to_shared(gsm + (size_t)kGbStages * kGbRows * kGbRowBytes);      // full[s], empty[s]
+    const int tid = threadIdx.x, wl = tid & 31, warp = tid >> 5;
+    const int kk = wl & 3, rw = wl >> 2;
+    const int spin = warp & 1;
+    const int vc0 = blockIdx.y * 64;                                     // first vector of this CTA
+    const int vloc = (warp >> 1) * (4 * kGatherNT);                      // this warp's first vector inside the chunk
+    const int nv = min(64, A.nvec - vc0);                                // live vectors of the chunk
+    const int atom = A.gb_atom[blockIdx.x];
+    const int e0 = A.gb_beg[blockIdx.x], e1 = A.gb_end[blockIdx.x];
+    const int npj = A.atom_npj[atom];
+    if (tid == 0) {
+        for (int s = 0; s < kGbStages; ++s) {
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(mb0 + 8 * s));
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], 8;" ::"r"(mb0 + 8 * (kGbStages + s)));
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    const int ngroups = (e1 - e0 + kGbRows - 1) / kGbRows;
+    // warp 0 issues the copies of a stage: lane = (row, spin)
+    auto issue = [&](int g) {
+        const int s = g % kGbStages;
+        const int eg = e0 + g * kGbRows, rows_g = min(kGbRows, e1 - eg);
+        if (g >= kGbStages) {                                           // every warp has consumed the group that was in this stage
+            unsigned done = 0;
+            while (!done) asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }" : "=r"(done) : "r"(mb0 + 8 * (kGbStages + s)), "r"((unsigned)((g / kGbStages - 1) & 1)) : "memory");
+        }
+        if (wl == 0) asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mb0 + 8 * s), "r"((unsigned)(rows_g * 2 * nv * 16)) : "memory");
+        __syncwarp();
+        const int row = wl >> 1, sp = wl & 1;
+        if (row < rows_g) {
+            const long long node = __ldg(A.ent_node + eg + row);
+            const char* src = static_cast<const char*>(A.src) + ((2 * node + sp) * A.ld + vc0) * 16;
+            const unsigned dst = (unsigned)__cvta_generic_to_shared(gsm + ((size_t)s * kGbRows + row) * kGbRowBytes + sp * 1024);
+            asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst), "l"(src), "r"((unsigned)(nv * 16)), "r"(mb0 + 8 * s) : "memory");
+        }
+    };
+    if (warp == 0)
+        for (int g = 0; g < kGbStages && g < ngroups; ++g) issue(g);
+    double acc[MD][kGatherNT][2];
+    double accx[NX > 0 ? NX : 1][kGatherNT];
+#pragma unroll
+    for (int m = 0; m < MD; ++m)
+#pragma unroll
+        for (int nt = 0; nt < kGatherNT; ++nt) { acc[m][nt][0] = 0.0; acc[m][nt][1] = 0.0; }
+#pragma unroll
+    for (int x = 0; x < (NX > 0 ? NX : 1); ++x)
+#pragma unroll
+        for (int nt = 0; nt < kGatherNT; ++nt) accx[x][nt] = 0.0;
+    const double* gp = A.g_pack + (long long)A.gb_k0[blockIdx.x] * (MT * 32) + wl;
+    constexpr int NA = MD + (NX > 0 ? NX : 0);
+    for (int g = 0; g < ngroups; ++g) {
+        const int s = g % kGbStages;
+        const int eg = e0 + g * kGbRows;
+        // P~^T fragments of the group's four k-steps (global / L2), requested before the wait
+        double a[4][NA];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const bool on = eg + 4 * q < e1;
+#pragma unroll
+            for (int m = 0; m < MD; ++m) a[q][m] = on ? __ldg(gp + ((long long)(4 * g + q) * MT + m) * 32) : 0.0;
+#pragma unroll
+            for (int x = 0; x < NX; ++x) a[q][MD + x] = on ? __ldg(gp - wl + ((long long)(4 * g + q) * MT + MD) * 32 + x * 4 + kk) : 0.0;
+        }
+        {
+            unsigned done = 0;
+            while (!done) asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }" : "=r"(done) : "r"(mb0 + 8 * s), "r"((unsigned)((g / kGbStages) & 1)) : "memory");
+        }
+        const double* sb = reinterpret_cast<const double*>(gsm + (size_t)s * kGbRows * kGbRowBytes + spin * 1024) + (vloc + (rw >> 1)) * 2 + (rw & 1);
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const bool ok = eg + 4 * q + kk < e1;
+            double b[kGatherNT];
+#pragma unroll
+            for (int nt = 0; nt < kGatherNT; ++nt)
+                b[nt] = (ok && vloc + nt * 4 + (rw >> 1) < nv) ? sb[(size_t)(4 * q + kk) * (kGbRowBytes / 8) + nt * 8] : 0.0;
+#pragma unroll
+            for (int m = 0; m < MD; ++m)
+#pragma unroll
+                for (int nt = 0; nt < kGatherNT; ++nt) gather_dmma(acc[m][nt][0], acc[m][nt][1], a[q][m], b[nt]);
+#pragma unroll
+            for (int x = 0; x < NX; ++x)
+#pragma unroll
+                for (int nt = 0; nt < kGatherNT; ++nt) accx[x][nt] = fma(a[q][MD + x], b[nt], accx[x][nt]);
+        }
+        __syncwarp();
+        if (wl == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(mb0 + 8 * (kGbStages + s)) : "memory");
+        if (warp == 0 && g + kGbStages < ngroups) issue(g + kGbStages);
+    }
+    const long long coff = A.atom_coff[atom];
+    const int v0 = vc0 + vloc;
 #pragma unroll
     for (int x = 0; x < NX; ++x)
 #pragma unroll
@@ -257,6 +393,35 @@ __global__ void __launch_bounds__(256) probe_dmma_kernel(double* sink, int iters
 #pragma unroll
     for (int q = 0; q < 8; ++q) s += d[q][0] + d[q][1];
     if (s == 12345.678) sink[threadIdx.x] = s;
+}
+
+// even warps run the DFMA chains, odd warps the DMMA chains: do the two instruction kinds have separate execution units?
+__global__ void __launch_bounds__(256) probe_mixed_kernel(double* sink, int iters, double m) {
+    if (((threadIdx.x >> 5) & 1) == 0) {
+        double a0 = threadIdx.x, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5, a6 = a0 + 6, a7 = a0 + 7;
+        const double c = 1e-9;
+#pragma unroll 4
+        for (int it = 0; it < iters; ++it) {
+            a0 = fma(a0, m, c); a1 = fma(a1, m, c); a2 = fma(a2, m, c); a3 = fma(a3, m, c);
+            a4 = fma(a4, m, c); a5 = fma(a5, m, c); a6 = fma(a6, m, c); a7 = fma(a7, m, c);
+        }
+        const double s = a0 + a1 + a2 + a3 + a4 + a5 + a6 + a7;
+        if (s == 12345.678) sink[threadIdx.x] = s;
+    } else {
+        double d[8][2];
+#pragma unroll
+        for (int q = 0; q < 8; ++q) { d[q][0] = threadIdx.x + q; d[q][1] = threadIdx.x - q; }
+        const double a = m * 1e-3, b = 1e-3 * (threadIdx.x & 3);
+#pragma unroll 2
+        for (int it = 0; it < iters; ++it) {
+#pragma unroll
+            for (int q = 0; q < 8; ++q) dmma884(d[q][0], d[q][1], a, b);
+        }
+        double s = 0.0;
+#pragma unroll
+        for (int q = 0; q < 8; ++q) s += d[q][0] + d[q][1];
+        if (s == 12345.678) sink[threadIdx.x] = s;
+    }
 }
 
 }  // namespace csf
