@@ -3,11 +3,14 @@
 
 A "step" is one pass of the whole hot path over one block: Y = T_m(H~) X for B spinor vectors, i.e. m
 applications of [projector gather -> Delta -> gather/cell apply/assembly/recurrence].
-metric = spinor DoF x vectors x degree per second (BASELINE.json). Default workload: BASELINE.json configs[3]
+metric = spinor DoF x vectors x degree per second (BASELINE.json). Headline workload: BASELINE.json configs[3]
 (periodic bulk, 32^3 cells of order 5, 8.19 M spinor DoF, 500 atoms, block of 256, degree 40), the largest
-single-GPU configuration of the roofline target set; `--config k` selects another.
+single-GPU configuration of the roofline target set; `--config k` selects another. The same JSON line carries the other
+roofline-target legs (`other_configs`: configs 2 and 4 in complex128, config 4 FP32-intermediate), the Rayleigh-Ritz /
+density timings on the filtered block (`subspace`), the end-to-end leg through host buffers (`e2e`) and the CPU oracle
+on the config's own operator (`cpu_baseline`). DESIGN.md section 6 describes every field.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config k] [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config k] [--mode fp64|fp32] [--impl ours|reference]
 
 N > 1 (under torchrun): the path does not shard (BASELINE.json north_star), so every rank filters its own block
 of states on its own replica of the operator ("replicas only"; the paper's band groups). No
