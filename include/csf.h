@@ -110,6 +110,18 @@ int csf_workspace_bytes(const csf_ctx* ctx, int nvec, int mode, size_t* bytes);
 int csf_apply_H(csf_ctx* ctx, const csf_c128* dX, csf_c128* dY, int64_t ld, int nvec,
                 void* d_work, size_t work_bytes);
 
+/* csf_apply_H for callers that may not allocate (CUDA graph capture, tight serving loops): the same launch sequence,
+ * with the projector-coefficient scratch (C = P~^T X and C~ = Delta C of P:551-561 steps 3-4) in an array of
+ * CSF_STATIC_SCRATCH_BYTES that is part of the library image: every GPU that loads libcsf.so holds it until the process
+ * exits. The call takes no workspace and calls no cudaMalloc / cudaFree / allocating library routine; the scratch is
+ * cleared by the call itself (it keeps the previous call's contents otherwise). ALL contexts and calls on one device
+ * share the array: two calls that overlap on the GPU (different streams, no dependency) race; order them.
+ * Errors: as csf_apply_H, plus CSF_EUNSUPPORTED with a text naming both sizes when the scratch for (this context's
+ * projectors, nvec) exceeds CSF_STATIC_SCRATCH_BYTES, CSF_ESTATE while per-kernel profiling is enabled (it creates
+ * events), CSF_ECUDA if the array's device address cannot be resolved. Without projectors no scratch is used. */
+#define CSF_STATIC_SCRATCH_BYTES (8u << 20)
+int csf_apply_H_static(csf_ctx* ctx, const csf_c128* dX, csf_c128* dY, int64_t ld, int nvec);
+
 /* Y = T_degree((Hhat - c)/e) X with c = (a+b)/2, e = (b-a)/2 (eq.70). degree = 0 copies X to Y.
  * Same pointer rules as csf_apply_H; X is not modified. mode: CSF_FP64, or CSF_FP32_INTERMEDIATE (complex128
  * in and out; both recurrence buffers complex64 and the cell-level arithmetic FP32 in between, projector coefficients

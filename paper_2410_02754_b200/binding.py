@@ -14,9 +14,10 @@ LIB_PATH = os.path.join(HERE, "libcsf.so")
 CSF_OK, CSF_EINVAL, CSF_ENOMEM, CSF_ECUDA, CSF_ESTATE, CSF_EUNSUPPORTED = 0, -1, -2, -3, -4, -5
 CSF_BC_PERIODIC, CSF_BC_DIRICHLET, CSF_BC_FREE = 0, 1, 2
 CSF_FP64, CSF_FP32_INTERMEDIATE = 0, 1
+STATIC_SCRATCH_BYTES = 8 << 20          # CSF_STATIC_SCRATCH_BYTES of include/csf.h
 
 EXPORTS = ["csf_create", "csf_destroy", "csf_set_stream", "csf_num_nodes", "csf_node_coords", "csf_mass_diag", "csf_set_potential",
-           "csf_set_projectors", "csf_workspace_bytes", "csf_apply_H", "csf_filter", "csf_filter_host", "csf_set_host_chunk",
+           "csf_set_projectors", "csf_workspace_bytes", "csf_apply_H", "csf_apply_H_static", "csf_filter", "csf_filter_host", "csf_set_host_chunk",
            "csf_profile_enable", "csf_profile_read", "csf_probe_fp64_peak", "csf_probe_fp64_mixed", "csf_launch_count", "csf_column_lanes", "csf_set_variant", "csf_set_tuning", "csf_last_error",
            "csf_rr_workspace_bytes", "csf_rr_project", "csf_rr_solve", "csf_rr_rotate", "csf_density", "csf_lanczos_workspace_bytes", "csf_lanczos",
            "csf_tridiag_extremes"]
@@ -120,6 +121,11 @@ class Csf:
 
     def apply_H(self, dX, dY, ld, nvec, d_work, work_bytes=0):
         self._chk(self._L.csf_apply_H(self._h, self._ptr(dX), self._ptr(dY), C.c_int64(int(ld)), C.c_int(int(nvec)), self._ptr(d_work), self._nbytes(d_work, work_bytes)))
+
+    def apply_H_static(self, dX, dY, ld, nvec):
+        """csf_apply_H without a workspace and without any allocation: the scratch is a static array inside the library
+        (STATIC_SCRATCH_BYTES); calls on one device share it and must not overlap on the GPU."""
+        self._chk(self._L.csf_apply_H_static(self._h, self._ptr(dX), self._ptr(dY), C.c_int64(int(ld)), C.c_int(int(nvec))))
 
     def filter(self, dX, dY, ld, nvec, degree, a, b, mode=CSF_FP64, d_work=0, work_bytes=0):
         self._chk(self._L.csf_filter(self._h, self._ptr(dX), self._ptr(dY), C.c_int64(int(ld)), C.c_int(int(nvec)), C.c_int(int(degree)),

@@ -16,6 +16,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <numeric>
 #include <string>
@@ -609,6 +610,55 @@ int csf_apply_H(csf_ctx* c, const csf_c128* dX, csf_c128* dY, int64_t ld, int nv
     CSF_CUDA(c, cudaSetDevice(c->device));
     double* dC = static_cast<double*>(d_work);
     double* dCt = reinterpret_cast<double*>(static_cast<char*>(d_work) + coef_bytes(c, nvec));
+    rc = enqueue_zero(c, reinterpret_cast<double*>(dY), ld, nvec);
+    if (rc != CSF_OK) return rc;
+    return enqueue_step(c, reinterpret_cast<const double*>(dX), ld, reinterpret_cast<double*>(dY), ld, nvec, 1.0, 0, 0.0, dC, dCt);
+    CSF_GUARD_END(c)
+}
+
+}  // extern "C"
+
+// Scratch of csf_apply_H_static: part of the library image, resident on every GPU that loads it, never freed.
+// In host code the name is only a handle for cudaGetSymbolAddress: it is NOT a device address and is never passed to a kernel.
+static __device__ __align__(256) unsigned char g_static_scratch[CSF_STATIC_SCRATCH_BYTES];
+
+namespace {
+// device address of g_static_scratch on the context's device (which must be current), resolved once per device
+int static_scratch_address(csf_ctx* c, unsigned char** out) {
+    static unsigned char* addr[64] = {};
+    static std::mutex mu;
+    if (c->device < 0 || c->device >= 64) return fail(c, CSF_EUNSUPPORTED, "device ordinal >= 64");
+    std::lock_guard<std::mutex> lk(mu);
+    if (!addr[c->device]) {
+        void* p = nullptr;
+        cudaError_t e = cudaGetSymbolAddress(&p, g_static_scratch);
+        if (e != cudaSuccess) return cuda_fail(c, e, "cudaGetSymbolAddress(g_static_scratch)");
+        if (!p || ((uintptr_t)p & 255) != 0) return fail(c, CSF_ECUDA, "static scratch has no usable device address");
+        addr[c->device] = static_cast<unsigned char*>(p);
+    }
+    *out = addr[c->device];
+    return CSF_OK;
+}
+}  // namespace
+
+extern "C" {
+
+int csf_apply_H_static(csf_ctx* c, const csf_c128* dX, csf_c128* dY, int64_t ld, int nvec) {
+    CSF_GUARD_BEGIN
+    if (!c) return CSF_EINVAL;
+    int rc = check_block_args(c, dX, dY, ld, nvec, nullptr, 0, 0);
+    if (rc != CSF_OK || nvec == 0) return rc;
+    if (c->prof) return fail(c, CSF_ESTATE, "csf_apply_H_static: switch per-kernel profiling off first (it creates events)");
+    const size_t cb = c->natoms > 0 ? coef_bytes(c, nvec) : 0, need = c->natoms > 0 ? cb + ctp_bytes(c, nvec) : 0;
+    if (need > (size_t)CSF_STATIC_SCRATCH_BYTES)
+        return fail(c, CSF_EUNSUPPORTED, "csf_apply_H_static: projector scratch of " + std::to_string(need) + " bytes for nvec = " + std::to_string(nvec) +
+                    " exceeds the static limit of " + std::to_string((size_t)CSF_STATIC_SCRATCH_BYTES) + " bytes; use csf_apply_H with a workspace, or fewer vectors per call");
+    CSF_CUDA(c, cudaSetDevice(c->device));
+    unsigned char* scratch = nullptr;
+    if (need > 0) { rc = static_scratch_address(c, &scratch); if (rc != CSF_OK) return rc; }
+    // enqueue_step clears C and C~ on the stream before the gather / Delta kernels add into them
+    double* dC = reinterpret_cast<double*>(scratch);
+    double* dCt = reinterpret_cast<double*>(scratch + cb);
     rc = enqueue_zero(c, reinterpret_cast<double*>(dY), ld, nvec);
     if (rc != CSF_OK) return rc;
     return enqueue_step(c, reinterpret_cast<const double*>(dX), ld, reinterpret_cast<double*>(dY), ld, nvec, 1.0, 0, 0.0, dC, dCt);
