@@ -219,6 +219,30 @@ int csf_lanczos(csf_ctx* ctx, const csf_c128* d_v0, int k, double* alpha_host, d
 int csf_tridiag_extremes(const double* alpha, const double* beta, int k, double* theta_min, double* theta_max);
 
 /* Text of the last error recorded on ctx (never NULL; "" if none). With ctx = NULL: last csf_create failure. */
+/* ---- potential on a general quadrature rule, dense cell-matrix form of H X --------------------------
+ * PAPER.md:528-547 eq.79-83: V_eff and B are given at the n_q^3 Gauss-Legendre points of every cell (eq.44);
+ * the cell-level potential matrices V^(e) = (N~ o (w J v^(e))) N~^T are dense n_p^3 x n_p^3. P:551-561 eq.84: H X is then
+ * computed cell by cell: extraction R^(e) X, product with the dense cell-level matrix (kinetic + potential, 2x2 in spin),
+ * assembly, plus the nonlocal part. This is the paper's own formulation; csf_apply_H (sum-factorised, nodal potential)
+ * is the fast path, and bench.py reports both. */
+
+/* Physical coordinates of the quadrature points, xyz_host[E][nq^3][3], cell e = cx + ncx (cy + ncy cz), point
+ * q = qx + nq (qy + nq qz): where the caller evaluates its fields for csf_set_potential_quadrature. 1 <= nq <= 16. */
+int csf_quadrature_points(const csf_ctx* ctx, int nq, double* xyz_host);
+
+/* vq_host[E][nq^3][4] = V_eff, B_x, B_y, B_z at those points (host, copied). Builds on the device, for every cell, the four
+ * real matrices 1/2 K^(e) + V^(e) +- B_z^(e), B_x^(e), B_y^(e) with the Loewdin scaling applied: 4 (n_p^3)^2 doubles per
+ * cell (1.5 MB at order 5). Synchronises. Independent of csf_set_potential; csf_set_projectors applies to both paths.
+ * Errors: CSF_EINVAL (NULL, nq out of range), CSF_ENOMEM when the matrices do not fit device memory, CSF_ECUDA. */
+int csf_set_potential_quadrature(csf_ctx* ctx, int nq, const double* vq_host);
+
+/* Bytes of device workspace csf_apply_H_dense needs for nvec vectors (projector coefficients; 0 without projectors). */
+int csf_dense_workspace_bytes(const csf_ctx* ctx, int nvec, size_t* bytes);
+
+/* Y = Hhat X through the dense cell matrices (eq.84). Pointer rules and errors as csf_apply_H; CSF_ESTATE if
+ * csf_set_potential_quadrature was never called. Enqueues only. */
+int csf_apply_H_dense(csf_ctx* ctx, const csf_c128* dX, csf_c128* dY, int64_t ld, int nvec, void* d_work, size_t work_bytes);
+
 const char* csf_last_error(const csf_ctx* ctx);
 
 #ifdef __cplusplus

@@ -20,7 +20,7 @@ EXPORTS = ["csf_create", "csf_destroy", "csf_set_stream", "csf_num_nodes", "csf_
            "csf_set_projectors", "csf_workspace_bytes", "csf_apply_H", "csf_apply_H_static", "csf_filter", "csf_filter_host", "csf_set_host_chunk",
            "csf_profile_enable", "csf_profile_read", "csf_probe_fp64_peak", "csf_probe_fp64_mixed", "csf_launch_count", "csf_column_lanes", "csf_set_variant", "csf_set_tuning", "csf_last_error",
            "csf_rr_workspace_bytes", "csf_rr_project", "csf_rr_solve", "csf_rr_rotate", "csf_density", "csf_lanczos_workspace_bytes", "csf_lanczos",
-           "csf_tridiag_extremes"]
+           "csf_tridiag_extremes", "csf_quadrature_points", "csf_set_potential_quadrature", "csf_dense_workspace_bytes", "csf_apply_H_dense"]
 KIND_CELL, KIND_PGATHER, KIND_DELTA, KIND_AUX = 0, 1, 2, 3
 KIND_NAMES = ("cell", "proj_gather", "delta", "aux")
 
@@ -61,6 +61,7 @@ class Csf:
             raise CsfError(rc, self._L.csf_last_error(None).decode())
         self.ncell, self.box, self.order, self.bc, self.device = tuple(ncell), tuple(box), int(order), tuple(bc), int(device)
         m = C.c_int64(); self._chk(self._L.csf_num_nodes(self._h, C.byref(m))); self.M = int(m.value)
+        self.E = int(self.ncell[0]) * int(self.ncell[1]) * int(self.ncell[2])
 
     def _chk(self, rc):
         if rc != CSF_OK:
@@ -126,6 +127,27 @@ class Csf:
         """csf_apply_H without a workspace and without any allocation: the scratch is a static array inside the library
         (STATIC_SCRATCH_BYTES); calls on one device share it and must not overlap on the GPU."""
         self._chk(self._L.csf_apply_H_static(self._h, self._ptr(dX), self._ptr(dY), C.c_int64(int(ld)), C.c_int(int(nvec))))
+
+    # ---- SURVEY 8(f) NEXT-3: general quadrature rule, dense cell-matrix apply
+    def quadrature_points(self, nq):
+        """[E, nq^3, 3] coordinates of the Gauss-Legendre points of every cell."""
+        out = np.empty((self.E, int(nq) ** 3, 3), dtype=np.float64)
+        self._chk(self._L.csf_quadrature_points(self._h, C.c_int(int(nq)), _dp(out, C.c_double)))
+        return out
+
+    def set_potential_quadrature(self, nq, vq):
+        """vq[E, nq^3, 4] = V_eff, B_x, B_y, B_z at the quadrature points."""
+        vq = np.ascontiguousarray(vq, dtype=np.float64)
+        assert vq.shape == (self.E, int(nq) ** 3, 4), "vq must be [E, nq^3, 4]"
+        self._chk(self._L.csf_set_potential_quadrature(self._h, C.c_int(int(nq)), _dp(vq, C.c_double)))
+
+    def dense_workspace_bytes(self, nvec):
+        b = C.c_size_t()
+        self._chk(self._L.csf_dense_workspace_bytes(self._h, C.c_int(int(nvec)), C.byref(b)))
+        return int(b.value)
+
+    def apply_H_dense(self, dX, dY, ld, nvec, d_work=0, work_bytes=0):
+        self._chk(self._L.csf_apply_H_dense(self._h, self._ptr(dX), self._ptr(dY), C.c_int64(int(ld)), C.c_int(int(nvec)), self._ptr(d_work), self._nbytes(d_work, work_bytes)))
 
     def filter(self, dX, dY, ld, nvec, degree, a, b, mode=CSF_FP64, d_work=0, work_bytes=0):
         self._chk(self._L.csf_filter(self._h, self._ptr(dX), self._ptr(dY), C.c_int64(int(ld)), C.c_int(int(nvec)), C.c_int(int(degree)),

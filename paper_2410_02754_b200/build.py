@@ -11,7 +11,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libcsf.so")
 SOURCES = ["csf_api.cu", "csf_tables.cpp", "csf_column_p.cu", "csf_colws_p.cu"]
-HEADERS = ["csf_kernels.cuh", "csf_column.cuh", "csf_colws.cuh", "csf_subspace.cuh", "csf_column_launch.h", "csf_tables.h", os.path.join("..", "..", "include", "csf.h")]
+HEADERS = ["csf_kernels.cuh", "csf_column.cuh", "csf_colws.cuh", "csf_subspace.cuh", "csf_dense.cuh", "csf_column_launch.h", "csf_tables.h", os.path.join("..", "..", "include", "csf.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "--use_fast_math=false",
               "-Xcompiler", "-fPIC", "-shared", "-Xptxas", "-v"]
 

@@ -4,6 +4,7 @@
 #include "csf_column.cuh"
 #include "csf_colws.cuh"
 #include "csf_subspace.cuh"
+#include "csf_dense.cuh"
 #include "csf_column_launch.h"
 #include "csf_tables.h"
 
@@ -50,6 +51,7 @@ struct csf_ctx {
     Gll1D gll; Dir1D dir[3];
     bool have_pot = false;
     DevBuf d_col_order, d_vb;
+    DevBuf d_cellmat; int dense_nq = 0, dense_n3p = 0;      // cell matrices of csf_set_potential_quadrature (fragment order, csf_dense.cuh)
     DevBuf d_inv_mass, d_occ;               // 1 / m_I (csf_density), occupation numbers of the last csf_density call
     DevBuf d_sub_ptr[kColMaxAuxWarps - 1], d_sub_desc[kColMaxAuxWarps - 1], d_a_pack[kColMaxAuxWarps - 1], d_ent_locf;     // [nq - 2]: nq expansion warps per CTA
     int seg_len = 0, chunk_group = 16;      // cells per z-segment (0 = the kernel's default), vector chunks scheduled back to back (csf_set_tuning)
@@ -1176,6 +1178,161 @@ int csf_tridiag_extremes(const double* alpha, const double* beta, int k, double*
     };
     *theta_min = kth(0); *theta_max = kth(k - 1);
     return CSF_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+// potential at the Gauss-Legendre points of an n_q^3 rule (eq.79-83) and the dense
+// cell-matrix form of H X (eq.84); kernels in csf_dense.cuh
+
+int csf_quadrature_points(const csf_ctx* c, int nq, double* xyz) {
+    CSF_GUARD_BEGIN
+    if (!c || !xyz) return CSF_EINVAL;
+    double x[kMaxQ], w[kMaxQ];
+    if (!build_gauss_legendre(nq, x, w)) return fail(const_cast<csf_ctx*>(c), CSF_EINVAL, "need 1 <= nq <= 16");
+    const long long nq3 = (long long)nq * nq * nq;
+    for (long long e = 0; e < c->E; ++e) {
+        const int cc[3] = {(int)(e % c->ncell[0]), (int)((e / c->ncell[0]) % c->ncell[1]), (int)(e / ((long long)c->ncell[0] * c->ncell[1]))};
+        for (int qz = 0; qz < nq; ++qz) for (int qy = 0; qy < nq; ++qy) for (int qx = 0; qx < nq; ++qx) {
+            double* o = xyz + (e * nq3 + qx + nq * (qy + (long long)nq * qz)) * 3;
+            o[0] = (cc[0] + 0.5 * (x[qx] + 1.0)) * c->h[0]; o[1] = (cc[1] + 0.5 * (x[qy] + 1.0)) * c->h[1]; o[2] = (cc[2] + 0.5 * (x[qz] + 1.0)) * c->h[2];
+        }
+    }
+    return CSF_OK;
+    CSF_GUARD_END(c)
+}
+
+int csf_set_potential_quadrature(csf_ctx* c, int nq, const double* vq) {
+    CSF_GUARD_BEGIN
+    if (!c) return CSF_EINVAL;
+    if (!vq) return fail(c, CSF_EINVAL, "vq is NULL");
+    double gx[kMaxQ], gw[kMaxQ];
+    if (!build_gauss_legendre(nq, gx, gw)) return fail(c, CSF_EINVAL, "need 1 <= nq <= 16");
+    CSF_CUDA(c, cudaSetDevice(c->device));
+    const int n = c->n, n3 = n * n * n, n3p = (n3 + 7) / 8 * 8, nq3 = nq * nq * nq;
+    const size_t mat_bytes = (size_t)c->E * 4 * n3p * n3p * sizeof(double);
+    size_t free_b = 0, total_b = 0;
+    CSF_CUDA(c, cudaMemGetInfo(&free_b, &total_b));
+    const size_t have = c->d_cellmat.bytes, reserve = (size_t)256 << 20;          // (the old matrices are released before the new ones are allocated)
+    if (mat_bytes > have && mat_bytes - have + reserve > free_b)
+        return fail(c, CSF_ENOMEM, "dense cell matrices need " + std::to_string(mat_bytes) + " bytes of device memory (4 n_p^6 doubles per cell); " + std::to_string(free_b) + " free");
+    // 1-D tables: L[i][q] = l_i(x_q), s_i = m1d_i^(-1/2) per direction
+    std::vector<double> L((size_t)n * nq);
+    lagrange_at_points(c->gll, nq, gx, L.data());
+    std::vector<double> Ns((size_t)nq3 * n3p, 0.0), wJ((size_t)nq3), kin((size_t)n3p * n3p, 0.0);
+    const double J = c->h[0] * c->h[1] * c->h[2] / 8.0;
+    for (int qz = 0; qz < nq; ++qz) for (int qy = 0; qy < nq; ++qy) for (int qx = 0; qx < nq; ++qx) {
+        const size_t q = qx + (size_t)nq * (qy + (size_t)nq * qz);
+        wJ[q] = gw[qx] * gw[qy] * gw[qz] * J;
+        for (int k = 0; k < n; ++k) for (int j = 0; j < n; ++j) for (int i = 0; i < n; ++i) {
+            const double s = 1.0 / std::sqrt(c->dir[0].m1d[i] * c->dir[1].m1d[j] * c->dir[2].m1d[k]);
+            Ns[q * n3p + i + n * (j + n * k)] = s * L[(size_t)i * nq + qx] * L[(size_t)j * nq + qy] * L[(size_t)k * nq + qz];
+        }
+    }
+    // S 1/2 K^(e) S = Bz (x) By (x) Ax + Bz (x) Ay (x) Bx + Az (x) By (x) Bx with B = diag(beta) - u u^T (csf_tables.h; eq.40 first term)
+    auto Bm = [&](int d, int i, int j) { return (i == j ? c->dir[d].beta[i] : 0.0) - c->dir[d].u[i] * c->dir[d].u[j]; };
+    for (int k = 0; k < n; ++k) for (int j = 0; j < n; ++j) for (int i = 0; i < n; ++i)
+        for (int k2 = 0; k2 < n; ++k2) for (int j2 = 0; j2 < n; ++j2) for (int i2 = 0; i2 < n; ++i2) {
+            const double bx = Bm(0, i, i2), by = Bm(1, j, j2), bz = Bm(2, k, k2);
+            kin[(size_t)(i + n * (j + n * k)) * n3p + i2 + n * (j2 + n * k2)] =
+                bz * by * c->dir[0].A[i][i2] + bz * c->dir[1].A[j][j2] * bx + c->dir[2].A[k][k2] * by * bx;
+        }
+    DevBuf dNs, dwJ, dkin, dvq;
+    CSF_CUDA(c, cudaStreamSynchronize(c->stream));
+    CSF_CUDA(c, dNs.upload(Ns)); CSF_CUDA(c, dwJ.upload(wJ)); CSF_CUDA(c, dkin.upload(kin));
+    CSF_CUDA(c, dvq.alloc((size_t)c->E * nq3 * 4 * sizeof(double)));
+    CSF_CUDA(c, cudaMemcpy(dvq.p, vq, (size_t)c->E * nq3 * 4 * sizeof(double), cudaMemcpyHostToDevice));
+    if (c->d_cellmat.bytes != mat_bytes) { if (c->d_cellmat.alloc(mat_bytes) != cudaSuccess) { cudaGetLastError(); c->dense_nq = 0; return fail(c, CSF_ENOMEM, "cudaMalloc of the dense cell matrices failed"); } }
+    CellMatParams cp{};
+    cp.Ns = dNs.as<double>(); cp.wJ = dwJ.as<double>(); cp.kin = dkin.as<double>(); cp.vq = dvq.as<double>(); cp.out = c->d_cellmat.as<double>();
+    cp.nq3 = nq3; cp.n3 = n3; cp.n3p = n3p;
+    const long long nblk = (long long)c->E * (n3p / 8);
+    if (nblk > 0x7fffffffLL) return fail(c, CSF_EUNSUPPORTED, "grid too large");
+    cellmat_build_kernel<<<(unsigned)nblk, 256, 0, c->stream>>>(cp);
+    CSF_CUDA(c, cudaGetLastError());
+    CSF_CUDA(c, cudaStreamSynchronize(c->stream));        // the staging buffers above are freed on return
+    c->dense_nq = nq; c->dense_n3p = n3p; c->launches += 1;
+    return CSF_OK;
+    CSF_GUARD_END(c)
+}
+
+int csf_dense_workspace_bytes(const csf_ctx* c, int nvec, size_t* bytes) {
+    if (!c || !bytes || nvec < 0) return CSF_EINVAL;
+    *bytes = c->natoms > 0 ? 2 * coef_bytes(c, nvec) : 0;
+    return CSF_OK;
+}
+
+int csf_apply_H_dense(csf_ctx* c, const csf_c128* dX, csf_c128* dY, int64_t ld, int nvec, void* d_work, size_t work_bytes) {
+    CSF_GUARD_BEGIN
+    if (!c) return CSF_EINVAL;
+    if (!dX || !dY) return fail(c, CSF_EINVAL, "NULL block pointer");
+    if ((const void*)dX == (const void*)dY) return fail(c, CSF_EINVAL, "Y must not alias X");
+    if (nvec < 0 || ld < nvec) return fail(c, CSF_EINVAL, "need 0 <= nvec <= ld");
+    if (c->dense_nq == 0) return fail(c, CSF_ESTATE, "csf_set_potential_quadrature has not been called");
+    size_t need = 0; csf_dense_workspace_bytes(c, nvec, &need);
+    if (nvec > 0 && need > 0 && (!d_work || work_bytes < need)) return fail(c, CSF_EINVAL, "workspace too small");
+    if (nvec == 0) return CSF_OK;
+    CSF_CUDA(c, cudaSetDevice(c->device));
+    int rc = enqueue_zero(c, reinterpret_cast<double*>(dY), ld, nvec);
+    if (rc != CSF_OK) return rc;
+    DenseParams q{};
+    q.mat = c->d_cellmat.as<double>(); q.X = reinterpret_cast<const double2*>(dX); q.ld = ld; q.Y = reinterpret_cast<double*>(dY); q.ldy = ld;
+    q.nvec = nvec; q.p = c->p; q.n3 = c->n * c->n * c->n; q.n3p = c->dense_n3p;
+    q.ncx = c->ncell[0]; q.ncy = c->ncell[1]; q.ncz = c->ncell[2]; q.nfx = c->nfree[0]; q.nfy = c->nfree[1]; q.nfz = c->nfree[2];
+    q.bcx = c->bc[0] == CSF_BC_DIRICHLET; q.bcy = c->bc[1] == CSF_BC_DIRICHLET; q.bcz = c->bc[2] == CSF_BC_DIRICHLET;
+    // 16 vectors per CTA where the X tile of the cell still leaves room for two CTAs per SM, 8 otherwise
+    const bool v16 = nvec > 8 && dense_smem<16>(q.n3p) <= 100 * 1024;
+    const int vc = v16 ? 16 : 8;
+    const size_t smem = v16 ? dense_smem<16>(q.n3p) : dense_smem<8>(q.n3p);
+    if (smem > c->smem_optin) return fail(c, CSF_EUNSUPPORTED, "cell tile does not fit shared memory");
+    const long long nblk = (long long)c->E * ((nvec + vc - 1) / vc);
+    if (nblk > 0x7fffffffLL) return fail(c, CSF_EUNSUPPORTED, "grid too large");
+    {
+        static bool configured[64] = {};
+        if (c->device >= 64 || !configured[c->device]) {
+            CSF_CUDA(c, cudaFuncSetAttribute(dense_cell_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_optin));
+            CSF_CUDA(c, cudaFuncSetAttribute(dense_cell_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_optin));
+            if (c->device < 64) configured[c->device] = true;
+        }
+        ProfScope ps(c, CSF_KIND_CELL);
+        if (v16) dense_cell_kernel<16><<<(unsigned)nblk, 256, smem, c->stream>>>(q);
+        else dense_cell_kernel<8><<<(unsigned)nblk, 256, smem, c->stream>>>(q);
+    }
+    CSF_CUDA(c, cudaGetLastError());
+    c->launches += 1;
+    if (c->natoms == 0) return CSF_OK;
+    // step 4: Y += P~ Delta P~^T X
+    double* dC = static_cast<double*>(d_work);
+    double2* dD = reinterpret_cast<double2*>(static_cast<char*>(d_work) + coef_bytes(c, nvec));
+    const long long ldc = nvec;
+    CSF_CUDA(c, cudaMemsetAsync(dC, 0, (size_t)c->crows * ldc * sizeof(double2), c->stream));
+    GatherParams gp{};
+    gp.src = dX; gp.ld = ld; gp.nvec = nvec;
+    gp.gb_atom = c->d_gb_atom.as<int>(); gp.gb_beg = c->d_gb_beg.as<int>(); gp.gb_end = c->d_gb_end.as<int>();
+    gp.ent_node = c->d_ent_node.as<int>(); gp.g_pack = c->d_g_pack.as<double>(); gp.gb_k0 = c->d_gb_k0.as<int>();
+    gp.atom_coff = c->d_atom_coff.as<long long>(); gp.atom_npj = c->d_atom_npj.as<int>();
+    gp.C = dC; gp.ldc = ldc;
+    dim3 gg(c->n_gather_blocks, (nvec + 16 * kGatherNT - 1) / (16 * kGatherNT));
+    {
+        ProfScope ps(c, CSF_KIND_PGATHER);
+        if (c->npjp <= 24) proj_gather_kernel<3, double><<<gg, 256, 0, c->stream>>>(gp);
+        else proj_gather_kernel<4, double><<<gg, 256, 0, c->stream>>>(gp);
+    }
+    CSF_CUDA(c, cudaGetLastError());
+    DeltaPlainParams dp{};
+    dp.C = reinterpret_cast<const double2*>(dC); dp.D = dD; dp.ldc = ldc; dp.nvec = nvec;
+    dp.atom_coff = c->d_atom_coff.as<long long>(); dp.atom_npj = c->d_atom_npj.as<int>(); dp.atom_type = c->d_atom_type.as<int>();
+    dp.delta = c->d_delta.as<double2>(); dp.delta_ptr = c->d_delta_ptr.as<long long>();
+    { ProfScope ps(c, CSF_KIND_DELTA); delta_plain_kernel<<<dim3(c->natoms, (nvec + 31) / 32), 256, 0, c->stream>>>(dp); }
+    CSF_CUDA(c, cudaGetLastError());
+    ExpandPlainParams ep{};
+    ep.D = dD; ep.ldc = ldc; ep.Y = reinterpret_cast<double*>(dY); ep.ldy = ld; ep.nvec = nvec; ep.mt = c->npjp <= 24 ? 3 : 4;
+    ep.gb_atom = gp.gb_atom; ep.gb_beg = gp.gb_beg; ep.gb_end = gp.gb_end; ep.gb_k0 = gp.gb_k0; ep.ent_node = gp.ent_node; ep.g_pack = gp.g_pack;
+    ep.atom_coff = gp.atom_coff; ep.atom_npj = gp.atom_npj;
+    { ProfScope ps(c, CSF_KIND_AUX); expand_plain_kernel<<<dim3(c->n_gather_blocks, (nvec + 31) / 32), 256, 0, c->stream>>>(ep); }
+    CSF_CUDA(c, cudaGetLastError());
+    c->launches += 3;
+    return CSF_OK;
+    CSF_GUARD_END(c)
 }
 
 }  // extern "C"

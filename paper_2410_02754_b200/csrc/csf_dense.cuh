@@ -1,0 +1,238 @@
+// csf_dense.cuh — the general-quadrature potential and the dense cell-matrix form of H X.
+//
+//   PAPER.md:528-547 eq.79-83: with the potential given at the n_q^3 Gauss-Legendre points of every cell, the cell-level
+//   potential matrices are V^(e) = (N~ o (w J v^(e))) N~^T, dense n_p^3 x n_p^3, N~[a][q] = N~_a(r~_q).
+//   PAPER.md:551-561 eq.84: H X cell by cell: extract X^(e) = R^(e) X, multiply by the dense cell-level matrix,
+//   assemble Y += R^(e)T Y^(e), add the nonlocal part C^T Delta C X.
+//
+// This is the paper's own formulation of the local part (one dense 2 n_p^3 x 2 n_p^3 block per cell, batched GEMM),
+// built here as the measured alternative to the sum-factorised column kernel of csf_column.cuh, and as the only path
+// that takes a non-nodal quadrature rule. Every cell matrix carries the Loewdin scaling S^(e) (.) S^(e) and the kinetic
+// block 1/2 K^(e) (the same for all cells of the uniform mesh):
+//      H^(e) = [ P   M1 - i M2 ]     P  = 1/2 K + V + Bz,   Q  = 1/2 K + V - Bz,
+//              [ M1 + i M2   Q ]     M1 = Bx,               M2 = By          (sigma of P:46; all four real, symmetric)
+// The four real matrices of a cell are stored in the order the FP64 tensor-core tile (mma.sync m8n8k4) reads its
+// A operand:  [cell][m-tile of 8 rows][k-step of 4 columns][matrix P, Q, M1, M2][lane = (row % 8) * 4 + column % 4],
+// so that a warp fetches the four fragments of one (m-tile, k-step) as 1 KB of consecutive memory.
+#pragma once
+#include <cuda_runtime.h>
+
+namespace csf {
+
+// ---------------------------------------------------------------------------------------------------------------------
+// set-up: the cell matrices from the potential at the quadrature points
+struct CellMatParams {
+    const double* Ns;        // [nq3][n3p]: s_a N~_a(r~_q), s_a = (1-D lumped masses of node a)^(-1/2); zero for a >= n3
+    const double* wJ;        // [nq3]: w_q J^(e)
+    const double* kin;       // [n3p][n3p]: S^(e) 1/2 K^(e) S^(e)
+    const double* vq;        // [E][nq3][4]: V_eff, B_x, B_y, B_z at the quadrature points
+    double* out;             // fragment order, see above
+    int nq3, n3, n3p;
+};
+
+constexpr int kCmChunk = 128;     // quadrature points staged per pass
+
+// grid = cells x m-tiles (m-tile fastest), 256 threads: thread = column b (strided), 8 rows x 4 fields in registers
+__global__ void __launch_bounds__(256) cellmat_build_kernel(const __grid_constant__ CellMatParams A) {
+    __shared__ double f[kCmChunk][4];
+    __shared__ double na[kCmChunk][8];
+    const int mtn = A.n3p / 8, ksn = A.n3p / 4;
+    const int mt = blockIdx.x % mtn; const long long e = blockIdx.x / mtn;
+    for (int b0 = 0; b0 < A.n3p; b0 += 256) {
+        const int b = b0 + threadIdx.x;
+        double acc[8][4];
+#pragma unroll
+        for (int r = 0; r < 8; ++r)
+#pragma unroll
+            for (int d = 0; d < 4; ++d) acc[r][d] = 0.0;
+        for (int q0 = 0; q0 < A.nq3; q0 += kCmChunk) {
+            const int nqc = min(kCmChunk, A.nq3 - q0);
+            __syncthreads();
+            for (int t = threadIdx.x; t < nqc * 4; t += 256) f[t >> 2][t & 3] = A.wJ[q0 + (t >> 2)] * A.vq[(e * A.nq3 + q0 + (t >> 2)) * 4 + (t & 3)];
+            for (int t = threadIdx.x; t < nqc * 8; t += 256) na[t >> 3][t & 7] = A.Ns[(long long)(q0 + (t >> 3)) * A.n3p + mt * 8 + (t & 7)];
+            __syncthreads();
+            if (b < A.n3p)
+                for (int q = 0; q < nqc; ++q) {
+                    const double nb = A.Ns[(long long)(q0 + q) * A.n3p + b];
+                    const double g0 = nb * f[q][0], g1 = nb * f[q][1], g2 = nb * f[q][2], g3 = nb * f[q][3];
+#pragma unroll
+                    for (int r = 0; r < 8; ++r) {
+                        const double a = na[q][r];
+                        acc[r][0] = fma(a, g0, acc[r][0]); acc[r][1] = fma(a, g1, acc[r][1]);
+                        acc[r][2] = fma(a, g2, acc[r][2]); acc[r][3] = fma(a, g3, acc[r][3]);
+                    }
+                }
+        }
+        if (b < A.n3p) {
+            double* o = A.out + (((e * mtn + mt) * ksn + (b >> 2)) * 4) * 32 + (b & 3);
+#pragma unroll
+            for (int r = 0; r < 8; ++r) {
+                const double k = A.kin[(long long)(mt * 8 + r) * A.n3p + b];
+                o[0 * 32 + r * 4] = k + acc[r][0] + acc[r][3];
+                o[1 * 32 + r * 4] = k + acc[r][0] - acc[r][3];
+                o[2 * 32 + r * 4] = acc[r][1];
+                o[3 * 32 + r * 4] = acc[r][2];
+            }
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+// eq.84: extraction, dense cell-level product, assembly
+struct DenseParams {
+    const double* mat;                 // cell matrices in fragment order
+    const double2* X; long long ld;    // [2M][ld] complex128
+    double* Y; long long ldy;          // [2M][ldy] complex128 as reals; Y += ...
+    int nvec, p, n3, n3p;
+    int ncx, ncy, ncz, nfx, nfy, nfz, bcx, bcy, bcz;      // bc: 0 periodic, 1 Dirichlet (boundary nodes removed)
+};
+
+__device__ __forceinline__ void dense_dmma(double& d0, double& d1, double a, double b) {
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
+}
+
+// global index of the 1-D node f = cell * p + i of a direction with nc cells, or -1 on a Dirichlet face
+__device__ __forceinline__ int dense_axis_node(int f, int nc, int p, int bc) {
+    if (bc == 0) return f == nc * p ? 0 : f;
+    return (f == 0 || f == nc * p) ? -1 : f - 1;
+}
+
+// VC spinor vectors per CTA; the X tile of the cell is kept as two real arrays [n3p][2 VC + 8] (spin up, spin down;
+// the row stride 2 VC + 8 = 8 mod 16 doubles keeps the B-fragment reads free of bank conflicts)
+template <int VC> __host__ __device__ constexpr int dense_ldw() { return 2 * VC + 8; }
+template <int VC> __host__ __device__ constexpr size_t dense_smem(int n3p) { return (size_t)2 * n3p * dense_ldw<VC>() * sizeof(double) + (size_t)n3p * sizeof(int); }
+
+// grid = cells x vector chunks (chunk fastest): the chunks of one cell run next to each other, so the cell's matrices (1.5 MB at order 5)
+// are fetched from HBM once and served from L2 to the other chunks. 8 warps, warp w takes the m-tiles w, w + 8, ...
+template <int VC>
+__global__ void __launch_bounds__(256) dense_cell_kernel(const __grid_constant__ DenseParams A) {
+    constexpr int LDW = dense_ldw<VC>(), NT = VC / 4;          // n-tiles of 8 real columns = 4 complex vectors
+    extern __shared__ __align__(16) unsigned char dense_raw[];
+    double* Xu = reinterpret_cast<double*>(dense_raw);
+    double* Xd = Xu + (size_t)A.n3p * LDW;
+    int* node = reinterpret_cast<int*>(Xd + (size_t)A.n3p * LDW);
+    const int nch = (A.nvec + VC - 1) / VC;
+    const int e = blockIdx.x / nch, v0 = (blockIdx.x % nch) * VC;
+    const int n = A.p + 1;
+    const int cx = e % A.ncx, cy = (e / A.ncx) % A.ncy, cz = e / (A.ncx * A.ncy);
+    // connectivity of the cell (eq.74), local node a = i + n (j + n k)
+    for (int a = threadIdx.x; a < A.n3p; a += 256) {
+        int g = -1;
+        if (a < A.n3) {
+            const int i = a % n, j = (a / n) % n, k = a / (n * n);
+            const int gx = dense_axis_node(cx * A.p + i, A.ncx, A.p, A.bcx), gy = dense_axis_node(cy * A.p + j, A.ncy, A.p, A.bcy),
+                      gz = dense_axis_node(cz * A.p + k, A.ncz, A.p, A.bcz);
+            if (gx >= 0 && gy >= 0 && gz >= 0) g = gx + A.nfx * (gy + A.nfy * gz);
+        }
+        node[a] = g;
+    }
+    __syncthreads();
+    // step 1, extraction: X^(e) = R^(e) X
+    for (int t = threadIdx.x; t < A.n3p * 2 * VC; t += 256) {
+        const int c = t % VC, s = (t / VC) & 1, a = t / (2 * VC);
+        const int g = node[a];
+        double2 z = make_double2(0.0, 0.0);
+        if (g >= 0 && v0 + c < A.nvec) z = A.X[(2LL * g + s) * A.ld + v0 + c];
+        double* o = (s ? Xd : Xu) + (size_t)a * LDW + 2 * c;
+        o[0] = z.x; o[1] = z.y;
+    }
+    __syncthreads();
+    // step 2, cell-level product with the dense matrix; step 3, assembly
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int kk = lane & 3, rw = lane >> 2;
+    const int mtn = A.n3p / 8, ksn = A.n3p / 4;
+    for (int mt = warp; mt < mtn; mt += 8) {
+        double au[NT][2], ad[NT][2], t1[NT][2], t2[NT][2];       // P Xu + M1 Xd,  M1 Xu + Q Xd,  M2 Xu,  M2 Xd
+#pragma unroll
+        for (int j = 0; j < NT; ++j) { au[j][0] = au[j][1] = ad[j][0] = ad[j][1] = t1[j][0] = t1[j][1] = t2[j][0] = t2[j][1] = 0.0; }
+        const double* m = A.mat + (((long long)e * mtn + mt) * ksn) * 128 + lane;
+#pragma unroll 4
+        for (int ks = 0; ks < ksn; ++ks) {
+            const double mp = __ldg(m + ks * 128), mq = __ldg(m + ks * 128 + 32), m1 = __ldg(m + ks * 128 + 64), m2 = __ldg(m + ks * 128 + 96);
+            const double* bu = Xu + (size_t)(ks * 4 + kk) * LDW + rw;
+            const double* bd = Xd + (size_t)(ks * 4 + kk) * LDW + rw;
+#pragma unroll
+            for (int j = 0; j < NT; ++j) {
+                const double xu = bu[8 * j], xd = bd[8 * j];
+                dense_dmma(au[j][0], au[j][1], mp, xu); dense_dmma(au[j][0], au[j][1], m1, xd);
+                dense_dmma(ad[j][0], ad[j][1], m1, xu); dense_dmma(ad[j][0], ad[j][1], mq, xd);
+                dense_dmma(t1[j][0], t1[j][1], m2, xu); dense_dmma(t2[j][0], t2[j][1], m2, xd);
+            }
+        }
+        const int g = node[mt * 8 + rw];
+        if (g < 0) continue;
+#pragma unroll
+        for (int j = 0; j < NT; ++j) {
+            const int v = v0 + 4 * j + kk;
+            if (v >= A.nvec) continue;
+            // Yu = Au - i T2,  Yd = Ad + i T1
+            double* yu = A.Y + ((2LL * g) * A.ldy + v) * 2;
+            double* yd = A.Y + ((2LL * g + 1) * A.ldy + v) * 2;
+            atomicAdd(yu, au[j][0] + t2[j][1]); atomicAdd(yu + 1, au[j][1] - t2[j][0]);
+            atomicAdd(yd, ad[j][0] - t1[j][1]); atomicAdd(yd + 1, ad[j][1] + t1[j][0]);
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+// step 4 of P:551-561, the nonlocal part, as separate kernels (the column kernel fuses the expansion; here the local part
+// is a different kernel). The coefficients C = P~^T X come from proj_gather_kernel (csf_kernels.cuh).
+
+// D = Delta C per atom, plain layout [crows][ldc] complex (row = atom_coff + 2 chi + spin), eq.76
+struct DeltaPlainParams {
+    const double2* C; double2* D; long long ldc; int nvec;
+    const long long* atom_coff; const int* atom_npj; const int* atom_type;
+    const double2* delta; const long long* delta_ptr;
+};
+
+__global__ void __launch_bounds__(256) delta_plain_kernel(const __grid_constant__ DeltaPlainParams A) {
+    const int atom = blockIdx.x;
+    const int v = blockIdx.y * 32 + (threadIdx.x & 31);
+    const int nr = 2 * A.atom_npj[atom];
+    const double2* Dl = A.delta + A.delta_ptr[A.atom_type[atom]];
+    const long long base = A.atom_coff[atom];
+    if (v >= A.nvec) return;
+    for (int r = threadIdx.x >> 5; r < nr; r += 8) {
+        double sr = 0.0, si = 0.0;
+        for (int q = 0; q < nr; ++q) {
+            const double2 d = __ldg(Dl + (long long)r * nr + q);
+            const double2 c = A.C[(base + q) * A.ldc + v];
+            sr = fma(d.x, c.x, sr); sr = fma(-d.y, c.y, sr);
+            si = fma(d.x, c.y, si); si = fma(d.y, c.x, si);
+        }
+        A.D[(base + r) * A.ldc + v] = make_double2(sr, si);
+    }
+}
+
+// Y[2 I + spin][v] += sum_chi P~[I, chi] D[atom; 2 chi + spin][v] over the entries (atom, node I) of one gather block;
+// P~ is read from g_pack, the fragment-ordered copy the gather kernel uses: [k-step of 4 entries][MT][(chi % 8) * 4 + entry % 4]
+struct ExpandPlainParams {
+    const double2* D; long long ldc;
+    double* Y; long long ldy; int nvec, mt;
+    const int* gb_atom; const int* gb_beg; const int* gb_end; const int* gb_k0;
+    const int* ent_node; const double* g_pack;
+    const long long* atom_coff; const int* atom_npj;
+};
+
+__global__ void __launch_bounds__(256) expand_plain_kernel(const __grid_constant__ ExpandPlainParams A) {
+    const int b = blockIdx.x, atom = A.gb_atom[b], beg = A.gb_beg[b], end = A.gb_end[b], k0 = A.gb_k0[b];
+    const int v = blockIdx.y * 32 + (threadIdx.x & 31);
+    const int npj = A.atom_npj[atom];
+    const long long base = A.atom_coff[atom];
+    if (v >= A.nvec) return;
+    for (int e = beg + (threadIdx.x >> 5); e < end; e += 8) {
+        const int I = A.ent_node[e];
+        const double* pk = A.g_pack + ((long long)(k0 + ((e - beg) >> 2)) * A.mt) * 32 + ((e - beg) & 3);
+        double ur = 0.0, ui = 0.0, dr = 0.0, di = 0.0;
+        for (int x = 0; x < npj; ++x) {
+            const double pv = __ldg(pk + (x >> 3) * 32 + (x & 7) * 4);
+            const double2 cu = A.D[(base + 2 * x) * A.ldc + v], cd = A.D[(base + 2 * x + 1) * A.ldc + v];
+            ur = fma(pv, cu.x, ur); ui = fma(pv, cu.y, ui); dr = fma(pv, cd.x, dr); di = fma(pv, cd.y, di);
+        }
+        double* yu = A.Y + ((2LL * I) * A.ldy + v) * 2;
+        double* yd = A.Y + ((2LL * I + 1) * A.ldy + v) * 2;
+        atomicAdd(yu, ur); atomicAdd(yu + 1, ui); atomicAdd(yd, dr); atomicAdd(yd + 1, di);
+    }
+}
+
+}  // namespace csf

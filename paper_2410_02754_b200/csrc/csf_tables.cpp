@@ -88,4 +88,35 @@ void build_dir(const Gll1D& g, double h, Dir1D* d) {
     for (int i = 0; i < n; ++i) for (int j = 0; j < n; ++j) d->A[i][j] = 0.5 * s[i] * (2.0 / h) * g.K[i][j] * s[j];
 }
 
+bool build_gauss_legendre(int nq, double* x, double* w) {
+    if (nq < 1 || nq > kMaxQ) return false;
+    const double pi = 3.14159265358979323846;
+    for (int i = 0; i < nq; ++i) {
+        double t = -std::cos(pi * (i + 0.75) / (nq + 0.5)), P = 0.0, dP = 1.0;
+        for (int it = 0; it < 100; ++it) {
+            legendre_pd(nq, t, &P, &dP);
+            const double dt = P / dP;
+            t -= dt;
+            if (std::fabs(dt) < 1e-16) break;
+        }
+        legendre_pd(nq, t, &P, &dP);
+        x[i] = t; w[i] = 2.0 / ((1.0 - t * t) * dP * dP);
+    }
+    for (int i = 0; i < nq / 2; ++i) {             // exact symmetry
+        const double a = 0.5 * (x[nq - 1 - i] - x[i]), ww = 0.5 * (w[i] + w[nq - 1 - i]);
+        x[i] = -a; x[nq - 1 - i] = a; w[i] = ww; w[nq - 1 - i] = ww;
+    }
+    if (nq % 2) x[nq / 2] = 0.0;
+    return true;
+}
+
+void lagrange_at_points(const Gll1D& g, int nq, const double* x, double* L) {
+    for (int i = 0; i < g.n; ++i)
+        for (int q = 0; q < nq; ++q) {
+            double v = 1.0;
+            for (int j = 0; j < g.n; ++j) if (j != i) v *= (x[q] - g.xi[j]) / (g.xi[i] - g.xi[j]);
+            L[i * nq + q] = v;
+        }
+}
+
 }  // namespace csf

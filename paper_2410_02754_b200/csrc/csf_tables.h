@@ -34,4 +34,11 @@ struct Dir1D {                // scaled 1-D operators of one mesh direction
 bool build_gll(int p, Gll1D* g);
 void build_dir(const Gll1D& g, double h, Dir1D* d);
 
+// Gauss-Legendre rule with nq points on [-1,1] (eq.44): x ascending = zeros of P_nq (Newton from the
+// Chebyshev guess), w = 2 / ((1 - x^2) P_nq'(x)^2). nq <= kMaxQ.
+constexpr int kMaxQ = 16;
+bool build_gauss_legendre(int nq, double* x, double* w);
+// L[i * nq + q] = l_i(x[q]): the Lagrange polynomials on the GLL nodes of g at nq arbitrary points (eq.82, one direction)
+void lagrange_at_points(const Gll1D& g, int nq, const double* x, double* L);
+
 }  // namespace csf
