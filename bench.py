@@ -350,6 +350,72 @@ def measure(cfg_index, mode_name, steps, warmup, args, ctxs):
     return res, live
 
 
+def measure_dense(args, peaks):
+    """One H apply through csf_apply_H_dense (eq.79-84: potential at n_q^3 Gauss-Legendre points, dense cell-level
+    matrices, FP64 tensor-core product) and through csf_apply_H (sum-factorised, nodal potential) on the same mesh, block and
+    projectors: config 3's cell size, order and atom density on a sub-mesh whose 4 n_p^6 doubles per cell fit the GPU."""
+    import torch
+    from paper_2410_02754_b200 import binding
+    base = synth.CONFIGS[3]
+    nc = min(args.dense_cells, base.ncell[0])
+    cfg = synth.scaled_config(base, (nc, nc, nc), max(1, round(base.natoms * nc ** 3 / (base.ncell[0] * base.ncell[1] * base.ncell[2]))), nvec=base.nvec)
+    ctx = binding.Csf(cfg.ncell, cfg.box, cfg.order, cfg.bc)
+    sysm = build_system(cfg, ctx)
+    nq = cfg.order + 3
+    pts = ctx.quadrature_points(nq)
+    k = [2.0 * np.pi / b for b in cfg.box]
+    vq = np.empty(pts.shape[:2] + (4,))
+    vq[..., 0] = -1.0 + 0.5 * np.cos(k[0] * pts[..., 0]) * np.cos(k[1] * pts[..., 1]) * np.cos(k[2] * pts[..., 2])
+    vq[..., 1] = 0.1 * np.sin(k[0] * pts[..., 0]); vq[..., 2] = 0.1 * np.sin(k[1] * pts[..., 1]); vq[..., 3] = 0.1 * np.cos(k[2] * pts[..., 2])
+    del pts
+    torch.cuda.synchronize(); t0 = time.perf_counter()
+    ctx.set_potential_quadrature(nq, vq)
+    ms_setup = (time.perf_counter() - t0) * 1e3
+    del vq
+    rows, nvec = 2 * ctx.M, cfg.nvec
+    gen = torch.Generator(device="cuda"); gen.manual_seed(777)
+    X = torch.empty((rows, nvec), dtype=torch.complex128, device="cuda"); torch.view_as_real(X).normal_(0.0, math.sqrt(0.5), generator=gen)
+    Y = torch.empty_like(X)
+    work = torch.empty(max(ctx.workspace_bytes(nvec), ctx.dense_workspace_bytes(nvec), 16), dtype=torch.uint8, device="cuda")
+    stream = torch.cuda.current_stream()
+
+    def timed(fn, reps):
+        for _ in range(2):
+            fn()
+        torch.cuda.synchronize()
+        e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(reps):
+            fn()
+        e1.record(stream); torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / reps
+
+    ms_sf = timed(lambda: ctx.apply_H(X, Y, nvec, nvec, work), 5)
+    ctx.profile_enable(True)
+    ms_dense = timed(lambda: ctx.apply_H_dense(X, Y, nvec, nvec, work), 3)
+    ms_cell, n_cell = ctx.profile_read(binding.KIND_CELL)
+    rest = {binding.KIND_NAMES[kd]: (lambda r: r[0] / max(r[1], 1))(ctx.profile_read(kd)) for kd in (binding.KIND_PGATHER, binding.KIND_DELTA, binding.KIND_AUX)}
+    ctx.profile_enable(False)
+    n3 = (cfg.order + 1) ** 3
+    E = cfg.ncell[0] * cfg.ncell[1] * cfg.ncell[2]
+    flops = 6.0 * 2.0 * 2.0 * n3 * n3 * nvec * E                       # six real n3 x n3 products on 2 nvec real columns per cell
+    mat_bytes = 4.0 * 8.0 * n3 * n3 * E
+    peak64 = SM_COUNT * FP64_FMA_PER_CLK_PER_SM * 2 * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6 / 1e12
+    ms_k = ms_cell / max(n_cell, 1)
+    out = {"note": "PAPER.md eq.79-84: potential at n_q^3 Gauss-Legendre points, dense 2x2-spin cell matrix applied with FP64 tensor-core tiles; "
+                   "beside it the sum-factorised csf_apply_H on the same mesh, block and projectors (nodal potential)",
+           "workload": f"{cfg.name}: {cfg.ncell[0]}^3 cells, order {cfg.order}, {cfg.natoms} atoms, {nvec} vectors, n_q = {nq}",
+           "cell_matrix_bytes": mat_bytes, "setup_ms": ms_setup,
+           "apply_dense_ms": ms_dense, "apply_sum_factorised_ms": ms_sf, "dense_over_sum_factorised": ms_dense / ms_sf,
+           "dense_kernel_ms": ms_k, "dense_kernel_tflops": flops / ms_k / 1e9, "dense_kernel_frac_of_fp64_peak": flops / ms_k / 1e9 / peak64,
+           "dense_kernel_matrix_gbs_if_read_once": mat_bytes / ms_k / 1e6,
+           "nonlocal_kernels_ms": {"proj_gather": rest["proj_gather"], "delta": rest["delta"], "expansion": rest["aux"]},
+           "units_per_s_dense": rows * nvec / (ms_dense * 1e-3), "units_per_s_sum_factorised": rows * nvec / (ms_sf * 1e-3),
+           "finite": bool(torch.isfinite(torch.view_as_real(Y[::4099])).all().item())}
+    del X, Y, work, ctx
+    return out
+
+
 def main_ours(args):
     import torch
     import torch.distributed as dist
@@ -480,6 +546,12 @@ def main_ours(args):
                            "warmup": r["warmup"], "roofline": r["roofline"], "step_roofline": r["step_roofline"], "clocks": r["clocks"], "finite": r["finite"],
                            "full_filter_extrapolated_s": r.get("full_filter_extrapolated_s"), "c_ov": r["config"].get("c_ov")})
 
+    # ---- the paper's own form of the local part (dense cell matrices, eq.84) beside the sum-factorised one
+    dense = None
+    if world == 1 and not args.no_dense and not (args.nvec or args.degree):
+        dense = measure_dense(args, peaks)
+        torch.cuda.empty_cache()
+
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         v, desc, cores, _ = run_oracle_sample(synth.CONFIGS[args.config])
@@ -490,7 +562,7 @@ def main_ours(args):
                "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": head["dtype"], "data": "synthetic", "config": head["config"],
                "clocks": head["clocks"], "e2e": e2e, "gpu_launches": head["gpu_launches"], "roofline": head["roofline"], "step_roofline": head["step_roofline"],
                "cpu_baseline": cpu, "finite": head["finite"], "full_filter_extrapolated_s": head.get("full_filter_extrapolated_s"), "other_configs": others,
-               "subspace": subspace}
+               "subspace": subspace, "dense_cell_matrix_path": dense}
         print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()
@@ -518,6 +590,8 @@ def main():
     ap.add_argument("--no-subspace", action="store_true", help="skip the Rayleigh-Ritz / density timings after the headline leg")
     ap.add_argument("--no-others", action="store_true", help="skip the other roofline-target legs (configs 2, 4 in FP64, config 4 in FP32-intermediate)")
     ap.add_argument("--other-steps", type=int, default=2, help="timed steps of each other leg")
+    ap.add_argument("--no-dense", action="store_true", help="skip the dense cell-matrix leg (SURVEY 8(f) NEXT-3)")
+    ap.add_argument("--dense-cells", type=int, default=16, help="cells per direction of the dense leg's sub-mesh of config 3")
     args = ap.parse_args()
     return main_reference(args) if args.impl == "reference" else main_ours(args)
 

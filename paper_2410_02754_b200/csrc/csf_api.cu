@@ -1279,8 +1279,8 @@ int csf_apply_H_dense(csf_ctx* c, const csf_c128* dX, csf_c128* dY, int64_t ld, 
     q.nvec = nvec; q.p = c->p; q.n3 = c->n * c->n * c->n; q.n3p = c->dense_n3p;
     q.ncx = c->ncell[0]; q.ncy = c->ncell[1]; q.ncz = c->ncell[2]; q.nfx = c->nfree[0]; q.nfy = c->nfree[1]; q.nfz = c->nfree[2];
     q.bcx = c->bc[0] == CSF_BC_DIRICHLET; q.bcy = c->bc[1] == CSF_BC_DIRICHLET; q.bcz = c->bc[2] == CSF_BC_DIRICHLET;
-    // 16 vectors per CTA where the X tile of the cell still leaves room for two CTAs per SM, 8 otherwise
-    const bool v16 = nvec > 8 && dense_smem<16>(q.n3p) <= 100 * 1024;
+    // 16 vectors per CTA where the X tile of the cell still leaves room for two CTAs per SM (up to order 5), 8 otherwise
+    const bool v16 = nvec > 8 && 2 * (dense_smem<16>(q.n3p) + 1024) <= 227 * 1024;
     const int vc = v16 ? 16 : 8;
     const size_t smem = v16 ? dense_smem<16>(q.n3p) : dense_smem<8>(q.n3p);
     if (smem > c->smem_optin) return fail(c, CSF_EUNSUPPORTED, "cell tile does not fit shared memory");

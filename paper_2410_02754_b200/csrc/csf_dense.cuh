@@ -97,15 +97,18 @@ __device__ __forceinline__ int dense_axis_node(int f, int nc, int p, int bc) {
     return (f == 0 || f == nc * p) ? -1 : f - 1;
 }
 
-// VC spinor vectors per CTA; the X tile of the cell is kept as two real arrays [n3p][2 VC + 8] (spin up, spin down;
-// the row stride 2 VC + 8 = 8 mod 16 doubles keeps the B-fragment reads free of bank conflicts)
-template <int VC> __host__ __device__ constexpr int dense_ldw() { return 2 * VC + 8; }
+// VC spinor vectors per CTA; the X tile of the cell is kept as two real arrays [n3p][LDW] (spin up, spin down). The B fragment
+// of a DMMA is read as (row k0 + lane % 4, column n0 + lane / 4): a half-warp must land in 16 different 8-byte banks, i.e.
+// the four rows must start 4 doubles apart mod 16. VC = 8: row stride 2 VC + 4 = 20. VC = 16: stride 32 with the column
+// XOR-ed by 4 (row % 4) instead of padding, so that the tile of an order-5 cell (110 KB) leaves room for two CTAs per SM.
+template <int VC> __host__ __device__ constexpr int dense_ldw() { return VC == 16 ? 32 : 2 * VC + 4; }
+template <int VC> __host__ __device__ constexpr int dense_col(int row, int col) { return VC == 16 ? (col ^ ((row & 3) * 4)) : col; }
 template <int VC> __host__ __device__ constexpr size_t dense_smem(int n3p) { return (size_t)2 * n3p * dense_ldw<VC>() * sizeof(double) + (size_t)n3p * sizeof(int); }
 
 // grid = cells x vector chunks (chunk fastest): the chunks of one cell run next to each other, so the cell's matrices (1.5 MB at order 5)
 // are fetched from HBM once and served from L2 to the other chunks. 8 warps, warp w takes the m-tiles w, w + 8, ...
 template <int VC>
-__global__ void __launch_bounds__(256) dense_cell_kernel(const __grid_constant__ DenseParams A) {
+__global__ void __launch_bounds__(256, 2) dense_cell_kernel(const __grid_constant__ DenseParams A) {
     constexpr int LDW = dense_ldw<VC>(), NT = VC / 4;          // n-tiles of 8 real columns = 4 complex vectors
     extern __shared__ __align__(16) unsigned char dense_raw[];
     double* Xu = reinterpret_cast<double*>(dense_raw);
@@ -133,14 +136,16 @@ __global__ void __launch_bounds__(256) dense_cell_kernel(const __grid_constant__
         const int g = node[a];
         double2 z = make_double2(0.0, 0.0);
         if (g >= 0 && v0 + c < A.nvec) z = A.X[(2LL * g + s) * A.ld + v0 + c];
-        double* o = (s ? Xd : Xu) + (size_t)a * LDW + 2 * c;
-        o[0] = z.x; o[1] = z.y;
+        *reinterpret_cast<double2*>((s ? Xd : Xu) + (size_t)a * LDW + dense_col<VC>(a, 2 * c)) = z;
     }
     __syncthreads();
     // step 2, cell-level product with the dense matrix; step 3, assembly
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int kk = lane & 3, rw = lane >> 2;
     const int mtn = A.n3p / 8, ksn = A.n3p / 4;
+    int cj[NT];                                                  // column of this lane's B element in n-tile j
+#pragma unroll
+    for (int j = 0; j < NT; ++j) cj[j] = dense_col<VC>(kk, 8 * j + rw);
     for (int mt = warp; mt < mtn; mt += 8) {
         double au[NT][2], ad[NT][2], t1[NT][2], t2[NT][2];       // P Xu + M1 Xd,  M1 Xu + Q Xd,  M2 Xu,  M2 Xd
 #pragma unroll
@@ -149,11 +154,11 @@ __global__ void __launch_bounds__(256) dense_cell_kernel(const __grid_constant__
 #pragma unroll 4
         for (int ks = 0; ks < ksn; ++ks) {
             const double mp = __ldg(m + ks * 128), mq = __ldg(m + ks * 128 + 32), m1 = __ldg(m + ks * 128 + 64), m2 = __ldg(m + ks * 128 + 96);
-            const double* bu = Xu + (size_t)(ks * 4 + kk) * LDW + rw;
-            const double* bd = Xd + (size_t)(ks * 4 + kk) * LDW + rw;
+            const double* bu = Xu + (size_t)(ks * 4 + kk) * LDW;
+            const double* bd = Xd + (size_t)(ks * 4 + kk) * LDW;
 #pragma unroll
             for (int j = 0; j < NT; ++j) {
-                const double xu = bu[8 * j], xd = bd[8 * j];
+                const double xu = bu[cj[j]], xd = bd[cj[j]];
                 dense_dmma(au[j][0], au[j][1], mp, xu); dense_dmma(au[j][0], au[j][1], m1, xd);
                 dense_dmma(ad[j][0], ad[j][1], m1, xu); dense_dmma(ad[j][0], ad[j][1], mq, xd);
                 dense_dmma(t1[j][0], t1[j][1], m2, xu); dense_dmma(t2[j][0], t2[j][1], m2, xd);
@@ -214,24 +219,39 @@ struct ExpandPlainParams {
     const long long* atom_coff; const int* atom_npj;
 };
 
+// grid (gather blocks, tiles of 32 vectors), 8 warps, lane = vector. D of the atom for these 32 vectors is staged in shared
+// memory once; a warp takes four entries at a time (one k-step of g_pack: the four P~ values of a projector are 32 consecutive bytes)
 __global__ void __launch_bounds__(256) expand_plain_kernel(const __grid_constant__ ExpandPlainParams A) {
+    __shared__ double2 Ds[64][32];
     const int b = blockIdx.x, atom = A.gb_atom[b], beg = A.gb_beg[b], end = A.gb_end[b], k0 = A.gb_k0[b];
-    const int v = blockIdx.y * 32 + (threadIdx.x & 31);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int v = blockIdx.y * 32 + lane;
     const int npj = A.atom_npj[atom];
     const long long base = A.atom_coff[atom];
+    for (int r = warp; r < 2 * npj; r += 8) Ds[r][lane] = v < A.nvec ? A.D[(base + r) * A.ldc + v] : make_double2(0.0, 0.0);
+    __syncthreads();
     if (v >= A.nvec) return;
-    for (int e = beg + (threadIdx.x >> 5); e < end; e += 8) {
-        const int I = A.ent_node[e];
-        const double* pk = A.g_pack + ((long long)(k0 + ((e - beg) >> 2)) * A.mt) * 32 + ((e - beg) & 3);
-        double ur = 0.0, ui = 0.0, dr = 0.0, di = 0.0;
+    for (int e = beg + 4 * warp; e < end; e += 32) {
+        const double2* pk = reinterpret_cast<const double2*>(A.g_pack + ((long long)(k0 + ((e - beg) >> 2)) * A.mt) * 32);
+        double ur[4] = {0.0, 0.0, 0.0, 0.0}, ui[4] = {0.0, 0.0, 0.0, 0.0}, dr[4] = {0.0, 0.0, 0.0, 0.0}, di[4] = {0.0, 0.0, 0.0, 0.0};
         for (int x = 0; x < npj; ++x) {
-            const double pv = __ldg(pk + (x >> 3) * 32 + (x & 7) * 4);
-            const double2 cu = A.D[(base + 2 * x) * A.ldc + v], cd = A.D[(base + 2 * x + 1) * A.ldc + v];
-            ur = fma(pv, cu.x, ur); ui = fma(pv, cu.y, ui); dr = fma(pv, cd.x, dr); di = fma(pv, cd.y, di);
+            const double2 p01 = __ldg(pk + (x >> 3) * 16 + (x & 7) * 2), p23 = __ldg(pk + (x >> 3) * 16 + (x & 7) * 2 + 1);
+            const double pv[4] = {p01.x, p01.y, p23.x, p23.y};
+            const double2 cu = Ds[2 * x][lane], cd = Ds[2 * x + 1][lane];
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                ur[q] = fma(pv[q], cu.x, ur[q]); ui[q] = fma(pv[q], cu.y, ui[q]);
+                dr[q] = fma(pv[q], cd.x, dr[q]); di[q] = fma(pv[q], cd.y, di[q]);
+            }
         }
-        double* yu = A.Y + ((2LL * I) * A.ldy + v) * 2;
-        double* yd = A.Y + ((2LL * I + 1) * A.ldy + v) * 2;
-        atomicAdd(yu, ur); atomicAdd(yu + 1, ui); atomicAdd(yd, dr); atomicAdd(yd + 1, di);
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            if (e + q >= end) break;
+            const long long I = A.ent_node[e + q];
+            double* yu = A.Y + ((2 * I) * A.ldy + v) * 2;
+            double* yd = A.Y + ((2 * I + 1) * A.ldy + v) * 2;
+            atomicAdd(yu, ur[q]); atomicAdd(yu + 1, ui[q]); atomicAdd(yd, dr[q]); atomicAdd(yd + 1, di[q]);
+        }
     }
 }
 
