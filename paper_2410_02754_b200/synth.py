@@ -237,6 +237,25 @@ def make_system(cfg: Config, coords: np.ndarray, mass: np.ndarray, with_projecto
     return System(cfg, pos, veff, bxyz, node_ptr, node_idx, nproj, pvals, atom_type, delta, delta_ptr, delta_off, rng)
 
 
+def bloch_pvals(sysm: System, coords: np.ndarray, kvec) -> np.ndarray:
+    """Complex projector entries P^{a,k}_{I chi} of eq.42 for Bloch vector k, same layout as `sysm.pvals`:
+    the collocated entry m_I p_chi(r_I - L_q - R_a) times e^{-i k.(r_I - L_q)}, with r_I - L_q = R_a + d and d the
+    minimum-image displacement the generator used for that support node (one image per node: r_c < L/2)."""
+    cfg = sysm.cfg
+    kvec = np.asarray(kvec, dtype=np.float64)
+    axes = grid_axes(cfg, coords)
+    out = np.zeros(sysm.pvals.size, dtype=np.complex128)
+    off = 0
+    for a in range(len(sysm.nproj)):
+        node, d = _local_patch(cfg, axes, sysm.positions[a], R_CUT_PROJ)
+        assert np.array_equal(node, sysm.node_idx[sysm.node_ptr[a]:sysm.node_ptr[a + 1]])
+        npj = int(sysm.nproj[a])
+        phase = np.exp(-1j * ((sysm.positions[a][None, :] + d) @ kvec))
+        blk = sysm.pvals[off:off + node.size * npj].reshape(node.size, npj) * phase[:, None]
+        out[off:off + node.size * npj] = blk.reshape(-1); off += node.size * npj
+    return out
+
+
 def random_block(rng, nrows, nvec) -> np.ndarray:
     """i.i.d. complex normal block, re and im ~ N(0, 1/2)."""
     return (rng.normal(scale=np.sqrt(0.5), size=(nrows, nvec)) + 1j * rng.normal(scale=np.sqrt(0.5), size=(nrows, nvec))).astype(np.complex128)
