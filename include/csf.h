@@ -236,12 +236,35 @@ int csf_quadrature_points(const csf_ctx* ctx, int nq, double* xyz_host);
  * Errors: CSF_EINVAL (NULL, nq out of range), CSF_ENOMEM when the matrices do not fit device memory, CSF_ECUDA. */
 int csf_set_potential_quadrature(csf_ctx* ctx, int nq, const double* vq_host);
 
-/* Bytes of device workspace csf_apply_H_dense needs for nvec vectors (projector coefficients; 0 without projectors). */
+/* Bytes of device workspace csf_filter_dense needs for nvec vectors (one block buffer + projector coefficients);
+ * csf_apply_H_dense is content with the same or less. */
 int csf_dense_workspace_bytes(const csf_ctx* ctx, int nvec, size_t* bytes);
 
 /* Y = Hhat X through the dense cell matrices (eq.84). Pointer rules and errors as csf_apply_H; CSF_ESTATE if
  * csf_set_potential_quadrature was never called. Enqueues only. */
 int csf_apply_H_dense(csf_ctx* ctx, const csf_c128* dX, csf_c128* dY, int64_t ld, int nvec, void* d_work, size_t work_bytes);
+
+/* csf_filter (eq.70, FP64) with every H apply going through the dense cell matrices: the filter for operators
+ * only the dense path holds (general quadrature rule, k-points). Arguments and errors as csf_filter. Enqueues only. */
+int csf_filter_dense(csf_ctx* ctx, const csf_c128* dX, csf_c128* dY, int64_t ld, int nvec,
+                     int degree, double a, double b, void* d_work, size_t work_bytes);
+
+/* ---- k-point (Bloch) Hamiltonian, on the dense path ------------------------------------------------
+ * PAPER.md:147-169 eq.21-24: H^k = e^{-ik.r} H e^{ik.r}; discretised (eq.40, eq.41-42)
+ *   H^k,loc  = int [1/2 grad N_I.grad N_J - i N_I k.grad N_J + (|k|^2/2 + V_eff) N_I N_J] d_ab + sum_d B^d N_I N_J sigma^d_ab
+ *   H^k,nloc = sum_a sum_{X X'} P^k_{I X} D^{X X'}_ab conj(P^k_{J X'}),  P^k_{I X} complex (Bloch phases e^{-ik.(r - L_q)})
+ * The gradient term is integrated exactly; |k|^2/2 is integrated with V_eff's rule (reading A19). The
+ * sum-factorised entry points (csf_apply_H, csf_filter, csf_filter_host, csf_rr_project, csf_lanczos, ...) hold the
+ * Gamma-point operator with real projectors and fail with CSF_ESTATE while a k-point or complex projectors are set. */
+
+/* Bloch vector k_host[3] (1/bohr); (0, 0, 0) switches the k-point terms off. Invalidates the cell matrices:
+ * csf_set_potential_quadrature must be called after it. Meaningful on periodic directions (not checked). */
+int csf_set_kpoint(csf_ctx* ctx, const double* k_host);
+
+/* csf_set_projectors with complex entries pvals[...] = P^{a,k}_{I X} of eq.42 (same layout; all host pointers). */
+int csf_set_projectors_complex(csf_ctx* ctx, int natoms, const int64_t* node_ptr, const int64_t* node_idx,
+                               const int* nproj, const csf_c128* pvals, const int* atom_type, int ntypes,
+                               const csf_c128* delta, const int64_t* delta_ptr);
 
 const char* csf_last_error(const csf_ctx* ctx);
 

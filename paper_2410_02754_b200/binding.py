@@ -20,7 +20,8 @@ EXPORTS = ["csf_create", "csf_destroy", "csf_set_stream", "csf_num_nodes", "csf_
            "csf_set_projectors", "csf_workspace_bytes", "csf_apply_H", "csf_apply_H_static", "csf_filter", "csf_filter_host", "csf_set_host_chunk",
            "csf_profile_enable", "csf_profile_read", "csf_probe_fp64_peak", "csf_probe_fp64_mixed", "csf_launch_count", "csf_column_lanes", "csf_set_variant", "csf_set_tuning", "csf_last_error",
            "csf_rr_workspace_bytes", "csf_rr_project", "csf_rr_solve", "csf_rr_rotate", "csf_density", "csf_lanczos_workspace_bytes", "csf_lanczos",
-           "csf_tridiag_extremes", "csf_quadrature_points", "csf_set_potential_quadrature", "csf_dense_workspace_bytes", "csf_apply_H_dense"]
+           "csf_tridiag_extremes", "csf_quadrature_points", "csf_set_potential_quadrature", "csf_dense_workspace_bytes", "csf_apply_H_dense",
+           "csf_filter_dense", "csf_set_kpoint", "csf_set_projectors_complex"]
 KIND_CELL, KIND_PGATHER, KIND_DELTA, KIND_AUX = 0, 1, 2, 3
 KIND_NAMES = ("cell", "proj_gather", "delta", "aux")
 
@@ -108,6 +109,24 @@ class Csf:
                                              _dp(pvals, C.c_double), _dp(atom_type, C.c_int), C.c_int(len(delta_ptr) - 1),
                                              delta.ctypes.data_as(C.c_void_p), _dp(delta_ptr, C.c_int64)))
 
+    def set_projectors_complex(self, node_ptr, node_idx, nproj, pvals, atom_type, delta, delta_ptr):
+        """set_projectors with complex entries P^{a,k}_{I chi} (eq.42); served by the dense path only."""
+        natoms = len(nproj)
+        if natoms == 0:
+            self._chk(self._L.csf_set_projectors_complex(self._h, C.c_int(0), None, None, None, None, None, C.c_int(0), None, None)); return
+        node_ptr = np.ascontiguousarray(node_ptr, dtype=np.int64); node_idx = np.ascontiguousarray(node_idx, dtype=np.int64)
+        nproj = np.ascontiguousarray(nproj, dtype=np.int32); pvals = np.ascontiguousarray(pvals, dtype=np.complex128)
+        atom_type = np.ascontiguousarray(atom_type, dtype=np.int32)
+        delta = np.ascontiguousarray(delta, dtype=np.complex128); delta_ptr = np.ascontiguousarray(delta_ptr, dtype=np.int64)
+        self._chk(self._L.csf_set_projectors_complex(self._h, C.c_int(natoms), _dp(node_ptr, C.c_int64), _dp(node_idx, C.c_int64), _dp(nproj, C.c_int),
+                                                     pvals.ctypes.data_as(C.c_void_p), _dp(atom_type, C.c_int), C.c_int(len(delta_ptr) - 1),
+                                                     delta.ctypes.data_as(C.c_void_p), _dp(delta_ptr, C.c_int64)))
+
+    def set_kpoint(self, kvec):
+        """Bloch vector (1/bohr); call set_potential_quadrature after it."""
+        k = np.ascontiguousarray(kvec, dtype=np.float64); assert k.shape == (3,)
+        self._chk(self._L.csf_set_kpoint(self._h, _dp(k, C.c_double)))
+
     def workspace_bytes(self, nvec, mode=CSF_FP64):
         b = C.c_size_t(); self._chk(self._L.csf_workspace_bytes(self._h, C.c_int(int(nvec)), C.c_int(mode), C.byref(b))); return int(b.value)
 
@@ -148,6 +167,10 @@ class Csf:
 
     def apply_H_dense(self, dX, dY, ld, nvec, d_work=0, work_bytes=0):
         self._chk(self._L.csf_apply_H_dense(self._h, self._ptr(dX), self._ptr(dY), C.c_int64(int(ld)), C.c_int(int(nvec)), self._ptr(d_work), self._nbytes(d_work, work_bytes)))
+
+    def filter_dense(self, dX, dY, ld, nvec, degree, a, b, d_work=0, work_bytes=0):
+        self._chk(self._L.csf_filter_dense(self._h, self._ptr(dX), self._ptr(dY), C.c_int64(int(ld)), C.c_int(int(nvec)), C.c_int(int(degree)),
+                                           C.c_double(float(a)), C.c_double(float(b)), self._ptr(d_work), self._nbytes(d_work, work_bytes)))
 
     def filter(self, dX, dY, ld, nvec, degree, a, b, mode=CSF_FP64, d_work=0, work_bytes=0):
         self._chk(self._L.csf_filter(self._h, self._ptr(dX), self._ptr(dY), C.c_int64(int(ld)), C.c_int(int(nvec)), C.c_int(int(degree)),

@@ -51,6 +51,8 @@ struct csf_ctx {
     Gll1D gll; Dir1D dir[3];
     bool have_pot = false;
     DevBuf d_col_order, d_vb;
+    double kpt[3] = {0.0, 0.0, 0.0}; bool kpt_on = false;      // Bloch vector of csf_set_kpoint (dense path only)
+    bool proj_complex = false; DevBuf d_g_pack_im, d_gk;         // Im P~ (csf_set_projectors_complex); S sum_d k_d G_d^(e) S in fragment order
     DevBuf d_cellmat; int dense_nq = 0, dense_n3p = 0;      // cell matrices of csf_set_potential_quadrature (fragment order, csf_dense.cuh)
     DevBuf d_inv_mass, d_occ;               // 1 / m_I (csf_density), occupation numbers of the last csf_density call
     DevBuf d_sub_ptr[kColMaxAuxWarps - 1], d_sub_desc[kColMaxAuxWarps - 1], d_a_pack[kColMaxAuxWarps - 1], d_ent_locf;     // [nq - 2]: nq expansion warps per CTA
@@ -185,6 +187,8 @@ int aux_warps(const csf_ctx* c, bool f32, int mode, int kind) { return kind == 2
 // src, dst: complex128 blocks, or complex64 blocks when f32 (CSF_FP32_INTERMEDIATE)
 int enqueue_step(csf_ctx* c, const void* src, long long ld, void* dst, long long ld_dst, int nvec, double sc, int rot, double shift,
                  double* dC, double* dCt, bool f32 = false) {
+    // the sum-factorised kernels hold the Gamma-point operator with real projectors only
+    if (c->kpt_on || c->proj_complex) return fail(c, CSF_ESTATE, "a k-point / complex projectors are set: only the dense path (csf_apply_H_dense, csf_filter_dense) serves them");
     const long long ldc = nvec;
     const int kind = column_kind(c); const bool ws = kind == 2;
     if (c->natoms > 0) {
@@ -459,14 +463,15 @@ int csf_set_potential(csf_ctx* c, const double* veff, const double* bxyz) {
     CSF_GUARD_END(c)
 }
 
-int csf_set_projectors(csf_ctx* c, int natoms, const int64_t* node_ptr, const int64_t* node_idx, const int* nproj,
-                       const double* pvals, const int* atom_type, int ntypes, const csf_c128* delta, const int64_t* delta_ptr) {
+// pvals_im: NULL, or the imaginary parts of complex projector entries (csf_set_projectors_complex; same layout as pvals)
+static int set_projectors_impl(csf_ctx* c, int natoms, const int64_t* node_ptr, const int64_t* node_idx, const int* nproj,
+                               const double* pvals, const double* pvals_im, const int* atom_type, int ntypes, const csf_c128* delta, const int64_t* delta_ptr) {
     CSF_GUARD_BEGIN
     if (!c) return CSF_EINVAL;
     if (natoms < 0) return fail(c, CSF_EINVAL, "natoms < 0");
     CSF_CUDA(c, cudaSetDevice(c->device));
     CSF_CUDA(c, cudaStreamSynchronize(c->stream));
-    c->natoms = 0; c->crows = 0; c->n_gather_blocks = 0;
+    c->natoms = 0; c->crows = 0; c->n_gather_blocks = 0; c->proj_complex = false;
     if (natoms == 0) return CSF_OK;
     if (!node_ptr || !node_idx || !nproj || !pvals || !atom_type || ntypes < 1 || !delta || !delta_ptr) return fail(c, CSF_EINVAL, "NULL projector argument");
     int npj_max = 0; bool uniform = true;
@@ -487,7 +492,7 @@ int csf_set_projectors(csf_ctx* c, int natoms, const int64_t* node_ptr, const in
     // owner cell and local index of every support node; sort each atom's entries by (cell, lz, ly, lx)
     struct Ent { int cell, lz, ly, lx; long long t; };
     std::vector<int> ent_node((size_t)nent), ent_locf((size_t)nent);
-    std::vector<double> ent_p((size_t)nent * npjp, 0.0);
+    std::vector<double> ent_p((size_t)nent * npjp, 0.0), ent_pi(pvals_im ? (size_t)nent * npjp : 0, 0.0);
     std::vector<long long> atom_coff(natoms); std::vector<int> atom_npj(nproj, nproj + natoms), atom_ty(atom_type, atom_type + natoms);
     std::vector<int> gb_atom, gb_beg, gb_end;
     struct Pair { int cell, atom; int off[kTabN + 1]; };
@@ -514,6 +519,7 @@ int csf_set_projectors(csf_ctx* c, int natoms, const int64_t* node_ptr, const in
             ent_node[e] = (int)I; ent_locf[e] = (ents[q].lz * p + ents[q].ly) * p + ents[q].lx;
             const double s = 1.0 / std::sqrt(mass[I]);
             for (int x = 0; x < nproj[a]; ++x) ent_p[(size_t)e * npjp + x] = s * pvals[pv_off + (t - t0) * nproj[a] + x];
+            if (pvals_im) for (int x = 0; x < nproj[a]; ++x) ent_pi[(size_t)e * npjp + x] = s * pvals_im[pv_off + (t - t0) * nproj[a] + x];
             if (q == 0 || ents[q].cell != ents[q - 1].cell) {
                 Pair pr; pr.cell = ents[q].cell; pr.atom = a;
                 for (int k = 0; k <= p; ++k) pr.off[k] = (int)e;
@@ -539,6 +545,15 @@ int csf_set_projectors(csf_ctx* c, int natoms, const int64_t* node_ptr, const in
             const size_t kstep = (size_t)atom_k0[a] + (e - node_ptr[a]) / 4; const int kq = (int)((e - node_ptr[a]) % 4);
             for (int x = 0; x < nproj[a]; ++x) g_pack[(kstep * mt + x / 8) * 32 + (x % 8) * 4 + kq] = ent_p[(size_t)e * npjp + x];
         }
+    if (pvals_im) {                             // Im P~ in the same order (dense path only)
+        std::vector<double> g_pack_im(g_pack.size(), 0.0);
+        for (int a = 0; a < natoms; ++a)
+            for (long long e = node_ptr[a]; e < node_ptr[a + 1]; ++e) {
+                const size_t kstep = (size_t)atom_k0[a] + (e - node_ptr[a]) / 4; const int kq = (int)((e - node_ptr[a]) % 4);
+                for (int x = 0; x < nproj[a]; ++x) g_pack_im[(kstep * mt + x / 8) * 32 + (x % 8) * 4 + kq] = ent_pi[(size_t)e * npjp + x];
+            }
+        CSF_CUDA(c, c->d_g_pack_im.upload(g_pack_im));
+    }
     // sub-pairs for the column kernels: every (cell, atom) pair split into the owned-node row ranges of the nq expansion
     // warps (entries of a pair are sorted by that index), grouped by (cell, warp)
     if (crows >= (1LL << 31)) return fail(c, CSF_EUNSUPPORTED, "too many projector rows");
@@ -587,7 +602,27 @@ int csf_set_projectors(csf_ctx* c, int natoms, const int64_t* node_ptr, const in
     CSF_CUDA(c, c->d_gb_k0.upload(gb_k0)); CSF_CUDA(c, c->d_g_pack.upload(g_pack)); CSF_CUDA(c, c->d_gb_atom.upload(gb_atom)); CSF_CUDA(c, c->d_gb_beg.upload(gb_beg)); CSF_CUDA(c, c->d_gb_end.upload(gb_end));
     c->natoms = natoms; c->crows = crows; c->npjp = npjp; c->npj_uniform = uniform ? nproj[0] : 0;
     c->n_gather_blocks = (int)gb_atom.size();
+    c->proj_complex = pvals_im != nullptr;
     return CSF_OK;
+    CSF_GUARD_END(c)
+}
+
+int csf_set_projectors(csf_ctx* c, int natoms, const int64_t* node_ptr, const int64_t* node_idx, const int* nproj,
+                       const double* pvals, const int* atom_type, int ntypes, const csf_c128* delta, const int64_t* delta_ptr) {
+    return set_projectors_impl(c, natoms, node_ptr, node_idx, nproj, pvals, nullptr, atom_type, ntypes, delta, delta_ptr);
+}
+
+int csf_set_projectors_complex(csf_ctx* c, int natoms, const int64_t* node_ptr, const int64_t* node_idx, const int* nproj,
+                               const csf_c128* pvals, const int* atom_type, int ntypes, const csf_c128* delta, const int64_t* delta_ptr) {
+    CSF_GUARD_BEGIN
+    if (!c) return CSF_EINVAL;
+    if (natoms <= 0 || !node_ptr || !nproj || !pvals) return set_projectors_impl(c, natoms, node_ptr, node_idx, nproj, nullptr, nullptr, atom_type, ntypes, delta, delta_ptr);
+    for (int a = 0; a < natoms; ++a) if (nproj[a] < 1 || node_ptr[a + 1] < node_ptr[a]) return fail(c, CSF_EINVAL, "bad nproj / node_ptr");
+    size_t n = 0;
+    for (int a = 0; a < natoms; ++a) n += (size_t)(node_ptr[a + 1] - node_ptr[a]) * nproj[a];
+    std::vector<double> re(n), im(n);
+    for (size_t i = 0; i < n; ++i) { re[i] = pvals[i].re; im[i] = pvals[i].im; }
+    return set_projectors_impl(c, natoms, node_ptr, node_idx, nproj, re.data(), im.data(), atom_type, ntypes, delta, delta_ptr);
     CSF_GUARD_END(c)
 }
 
@@ -1236,15 +1271,16 @@ int csf_set_potential_quadrature(csf_ctx* c, int nq, const double* vq) {
             kin[(size_t)(i + n * (j + n * k)) * n3p + i2 + n * (j2 + n * k2)] =
                 bz * by * c->dir[0].A[i][i2] + bz * c->dir[1].A[j][j2] * bx + c->dir[2].A[k][k2] * by * bx;
         }
-    DevBuf dNs, dwJ, dkin, dvq;
+    DevBuf dNs, dwJ, dkin, dvq; double cp_vshift = 0.0;
     CSF_CUDA(c, cudaStreamSynchronize(c->stream));
     CSF_CUDA(c, dNs.upload(Ns)); CSF_CUDA(c, dwJ.upload(wJ)); CSF_CUDA(c, dkin.upload(kin));
     CSF_CUDA(c, dvq.alloc((size_t)c->E * nq3 * 4 * sizeof(double)));
     CSF_CUDA(c, cudaMemcpy(dvq.p, vq, (size_t)c->E * nq3 * 4 * sizeof(double), cudaMemcpyHostToDevice));
+    cp_vshift = 0.5 * (c->kpt[0] * c->kpt[0] + c->kpt[1] * c->kpt[1] + c->kpt[2] * c->kpt[2]);      // |k|^2/2 stands beside V_eff in eq.40 (reading A19)
     if (c->d_cellmat.bytes != mat_bytes) { if (c->d_cellmat.alloc(mat_bytes) != cudaSuccess) { cudaGetLastError(); c->dense_nq = 0; return fail(c, CSF_ENOMEM, "cudaMalloc of the dense cell matrices failed"); } }
     CellMatParams cp{};
     cp.Ns = dNs.as<double>(); cp.wJ = dwJ.as<double>(); cp.kin = dkin.as<double>(); cp.vq = dvq.as<double>(); cp.out = c->d_cellmat.as<double>();
-    cp.nq3 = nq3; cp.n3 = n3; cp.n3p = n3p;
+    cp.nq3 = nq3; cp.n3 = n3; cp.n3p = n3p; cp.vshift = cp_vshift;
     const long long nblk = (long long)c->E * (n3p / 8);
     if (nblk > 0x7fffffffLL) return fail(c, CSF_EUNSUPPORTED, "grid too large");
     cellmat_build_kernel<<<(unsigned)nblk, 256, 0, c->stream>>>(cp);
@@ -1255,30 +1291,50 @@ int csf_set_potential_quadrature(csf_ctx* c, int nq, const double* vq) {
     CSF_GUARD_END(c)
 }
 
+int csf_set_kpoint(csf_ctx* c, const double* k) {
+    CSF_GUARD_BEGIN
+    if (!c || !k) return CSF_EINVAL;
+    CSF_CUDA(c, cudaSetDevice(c->device));
+    CSF_CUDA(c, cudaStreamSynchronize(c->stream));
+    for (int d = 0; d < 3; ++d) c->kpt[d] = k[d];
+    c->kpt_on = k[0] != 0.0 || k[1] != 0.0 || k[2] != 0.0;
+    c->dense_nq = 0;                          // the cell matrices carry |k|^2/2: csf_set_potential_quadrature must follow
+    if (!c->kpt_on) { c->d_gk.release(); return CSF_OK; }
+    // S sum_d k_d G_d^(e) S with G_x = Mz (x) My (x) Gx: the scaled 1-D mass B = diag(beta) - u u^T (csf_tables.h) and the scaled
+    // 1-D gradient C_ij = s_i w_i D_ij s_j (int l_i l_j' = w_i D_ij exactly; the (2/h)(h/2) of the derivative and the measure cancel)
+    const int n = c->n, n3 = n * n * n, n3p = (n3 + 7) / 8 * 8, ksn = n3p / 4;
+    auto Bm = [&](int d, int i, int j) { return (i == j ? c->dir[d].beta[i] : 0.0) - c->dir[d].u[i] * c->dir[d].u[j]; };
+    auto Cm = [&](int d, int i, int j) { return c->gll.w[i] * c->gll.D[i][j] / std::sqrt(c->dir[d].m1d[i] * c->dir[d].m1d[j]); };
+    std::vector<double> gk((size_t)n3p * n3p, 0.0);
+    for (int kz = 0; kz < n; ++kz) for (int j = 0; j < n; ++j) for (int i = 0; i < n; ++i)
+        for (int k2 = 0; k2 < n; ++k2) for (int j2 = 0; j2 < n; ++j2) for (int i2 = 0; i2 < n; ++i2) {
+            const double bx = Bm(0, i, i2), by = Bm(1, j, j2), bz = Bm(2, kz, k2);
+            const double v = k[0] * bz * by * Cm(0, i, i2) + k[1] * bz * Cm(1, j, j2) * bx + k[2] * Cm(2, kz, k2) * by * bx;
+            const int a = i + n * (j + n * kz), b = i2 + n * (j2 + n * k2);
+            gk[((size_t)(a / 8) * ksn + b / 4) * 32 + (a % 8) * 4 + b % 4] = v;
+        }
+    CSF_CUDA(c, c->d_gk.upload(gk));
+    return CSF_OK;
+    CSF_GUARD_END(c)
+}
+
 int csf_dense_workspace_bytes(const csf_ctx* c, int nvec, size_t* bytes) {
     if (!c || !bytes || nvec < 0) return CSF_EINVAL;
-    *bytes = c->natoms > 0 ? 2 * coef_bytes(c, nvec) : 0;
+    // one block buffer for the recurrence of csf_filter_dense + C (and the second gather of complex projectors) + Delta C
+    *bytes = block_bytes(c, nvec) + (c->natoms > 0 ? 3 * coef_bytes(c, nvec) : 0) + 256;
     return CSF_OK;
 }
 
-int csf_apply_H_dense(csf_ctx* c, const csf_c128* dX, csf_c128* dY, int64_t ld, int nvec, void* d_work, size_t work_bytes) {
-    CSF_GUARD_BEGIN
-    if (!c) return CSF_EINVAL;
-    if (!dX || !dY) return fail(c, CSF_EINVAL, "NULL block pointer");
-    if ((const void*)dX == (const void*)dY) return fail(c, CSF_EINVAL, "Y must not alias X");
-    if (nvec < 0 || ld < nvec) return fail(c, CSF_EINVAL, "need 0 <= nvec <= ld");
-    if (c->dense_nq == 0) return fail(c, CSF_ESTATE, "csf_set_potential_quadrature has not been called");
-    size_t need = 0; csf_dense_workspace_bytes(c, nvec, &need);
-    if (nvec > 0 && need > 0 && (!d_work || work_bytes < need)) return fail(c, CSF_EINVAL, "workspace too small");
-    if (nvec == 0) return CSF_OK;
-    CSF_CUDA(c, cudaSetDevice(c->device));
-    int rc = enqueue_zero(c, reinterpret_cast<double*>(dY), ld, nvec);
-    if (rc != CSF_OK) return rc;
+// dst += sc i^rot (Hhat^k - shift) src through the dense cell matrices; coef: 3 coef_bytes of workspace (unused without projectors)
+static int enqueue_dense_step(csf_ctx* c, const double2* src, long long ld, double* dst, long long ld_dst, int nvec, double sc, int rot, double shift, char* coef) {
+    const double frs[4] = {1.0, 0.0, -1.0, 0.0}, fis[4] = {0.0, 1.0, 0.0, -1.0};
+    const double fr = sc * frs[rot & 3], fi = sc * fis[rot & 3];
     DenseParams q{};
-    q.mat = c->d_cellmat.as<double>(); q.X = reinterpret_cast<const double2*>(dX); q.ld = ld; q.Y = reinterpret_cast<double*>(dY); q.ldy = ld;
+    q.mat = c->d_cellmat.as<double>(); q.X = src; q.ld = ld; q.Y = dst; q.ldy = ld_dst;
     q.nvec = nvec; q.p = c->p; q.n3 = c->n * c->n * c->n; q.n3p = c->dense_n3p;
     q.ncx = c->ncell[0]; q.ncy = c->ncell[1]; q.ncz = c->ncell[2]; q.nfx = c->nfree[0]; q.nfy = c->nfree[1]; q.nfz = c->nfree[2];
     q.bcx = c->bc[0] == CSF_BC_DIRICHLET; q.bcy = c->bc[1] == CSF_BC_DIRICHLET; q.bcz = c->bc[2] == CSF_BC_DIRICHLET;
+    q.fr = fr; q.fi = fi; q.gk = c->d_gk.as<double>();
     // 16 vectors per CTA where the X tile of the cell still leaves room for two CTAs per SM (up to order 5), 8 otherwise
     const bool v16 = nvec > 8 && 2 * (dense_smem<16>(q.n3p) + 1024) <= 227 * 1024;
     const int vc = v16 ? 16 : 8;
@@ -1289,48 +1345,129 @@ int csf_apply_H_dense(csf_ctx* c, const csf_c128* dX, csf_c128* dY, int64_t ld, 
     {
         static bool configured[64] = {};
         if (c->device >= 64 || !configured[c->device]) {
-            CSF_CUDA(c, cudaFuncSetAttribute(dense_cell_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_optin));
-            CSF_CUDA(c, cudaFuncSetAttribute(dense_cell_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_optin));
+            CSF_CUDA(c, cudaFuncSetAttribute(dense_cell_kernel<8, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_optin));
+            CSF_CUDA(c, cudaFuncSetAttribute(dense_cell_kernel<16, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_optin));
+            CSF_CUDA(c, cudaFuncSetAttribute(dense_cell_kernel<8, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_optin));
+            CSF_CUDA(c, cudaFuncSetAttribute(dense_cell_kernel<16, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_optin));
             if (c->device < 64) configured[c->device] = true;
         }
         ProfScope ps(c, CSF_KIND_CELL);
-        if (v16) dense_cell_kernel<16><<<(unsigned)nblk, 256, smem, c->stream>>>(q);
-        else dense_cell_kernel<8><<<(unsigned)nblk, 256, smem, c->stream>>>(q);
+        if (c->kpt_on) { if (v16) dense_cell_kernel<16, true><<<(unsigned)nblk, 256, smem, c->stream>>>(q); else dense_cell_kernel<8, true><<<(unsigned)nblk, 256, smem, c->stream>>>(q); }
+        else { if (v16) dense_cell_kernel<16, false><<<(unsigned)nblk, 256, smem, c->stream>>>(q); else dense_cell_kernel<8, false><<<(unsigned)nblk, 256, smem, c->stream>>>(q); }
     }
     CSF_CUDA(c, cudaGetLastError());
     c->launches += 1;
+    if (shift != 0.0) {
+        ProfScope ps(c, CSF_KIND_AUX);
+        caxpy_kernel<<<c->sm_count * 8, 256, 0, c->stream>>>(src, ld, reinterpret_cast<double2*>(dst), ld_dst, 2 * c->M, nvec, -fr * shift, -fi * shift);
+        CSF_CUDA(c, cudaGetLastError());
+        c->launches += 1;
+    }
     if (c->natoms == 0) return CSF_OK;
-    // step 4: Y += P~ Delta P~^T X
-    double* dC = static_cast<double*>(d_work);
-    double2* dD = reinterpret_cast<double2*>(static_cast<char*>(d_work) + coef_bytes(c, nvec));
+    // step 4: dst += f P~ Delta P~^+ src, P~ = Re + i Im
+    const size_t cb = coef_bytes(c, nvec);
+    double* dC = reinterpret_cast<double*>(coef);
+    double* dC2 = reinterpret_cast<double*>(coef + cb);
+    double2* dD = reinterpret_cast<double2*>(coef + 2 * cb);
     const long long ldc = nvec;
-    CSF_CUDA(c, cudaMemsetAsync(dC, 0, (size_t)c->crows * ldc * sizeof(double2), c->stream));
+    CSF_CUDA(c, cudaMemsetAsync(dC, 0, (c->proj_complex ? 2 : 1) * cb, c->stream));
     GatherParams gp{};
-    gp.src = dX; gp.ld = ld; gp.nvec = nvec;
+    gp.src = src; gp.ld = ld; gp.nvec = nvec;
     gp.gb_atom = c->d_gb_atom.as<int>(); gp.gb_beg = c->d_gb_beg.as<int>(); gp.gb_end = c->d_gb_end.as<int>();
     gp.ent_node = c->d_ent_node.as<int>(); gp.g_pack = c->d_g_pack.as<double>(); gp.gb_k0 = c->d_gb_k0.as<int>();
     gp.atom_coff = c->d_atom_coff.as<long long>(); gp.atom_npj = c->d_atom_npj.as<int>();
     gp.C = dC; gp.ldc = ldc;
     dim3 gg(c->n_gather_blocks, (nvec + 16 * kGatherNT - 1) / (16 * kGatherNT));
-    {
+    for (int part = 0; part < (c->proj_complex ? 2 : 1); ++part) {
+        if (part == 1) { gp.g_pack = c->d_g_pack_im.as<double>(); gp.C = dC2; }
         ProfScope ps(c, CSF_KIND_PGATHER);
         if (c->npjp <= 24) proj_gather_kernel<3, double><<<gg, 256, 0, c->stream>>>(gp);
         else proj_gather_kernel<4, double><<<gg, 256, 0, c->stream>>>(gp);
+        CSF_CUDA(c, cudaGetLastError());
+        c->launches += 1;
     }
-    CSF_CUDA(c, cudaGetLastError());
     DeltaPlainParams dp{};
-    dp.C = reinterpret_cast<const double2*>(dC); dp.D = dD; dp.ldc = ldc; dp.nvec = nvec;
+    dp.C = reinterpret_cast<const double2*>(dC); dp.C2 = c->proj_complex ? reinterpret_cast<const double2*>(dC2) : nullptr;
+    dp.D = dD; dp.ldc = ldc; dp.nvec = nvec; dp.fr = fr; dp.fi = fi;
     dp.atom_coff = c->d_atom_coff.as<long long>(); dp.atom_npj = c->d_atom_npj.as<int>(); dp.atom_type = c->d_atom_type.as<int>();
     dp.delta = c->d_delta.as<double2>(); dp.delta_ptr = c->d_delta_ptr.as<long long>();
     { ProfScope ps(c, CSF_KIND_DELTA); delta_plain_kernel<<<dim3(c->natoms, (nvec + 31) / 32), 256, 0, c->stream>>>(dp); }
     CSF_CUDA(c, cudaGetLastError());
     ExpandPlainParams ep{};
-    ep.D = dD; ep.ldc = ldc; ep.Y = reinterpret_cast<double*>(dY); ep.ldy = ld; ep.nvec = nvec; ep.mt = c->npjp <= 24 ? 3 : 4;
-    ep.gb_atom = gp.gb_atom; ep.gb_beg = gp.gb_beg; ep.gb_end = gp.gb_end; ep.gb_k0 = gp.gb_k0; ep.ent_node = gp.ent_node; ep.g_pack = gp.g_pack;
+    ep.D = dD; ep.ldc = ldc; ep.Y = dst; ep.ldy = ld_dst; ep.nvec = nvec; ep.mt = c->npjp <= 24 ? 3 : 4;
+    ep.gb_atom = gp.gb_atom; ep.gb_beg = gp.gb_beg; ep.gb_end = gp.gb_end; ep.gb_k0 = gp.gb_k0; ep.ent_node = gp.ent_node;
+    ep.g_pack = c->d_g_pack.as<double>(); ep.g_pack_im = c->d_g_pack_im.as<double>();
     ep.atom_coff = gp.atom_coff; ep.atom_npj = gp.atom_npj;
-    { ProfScope ps(c, CSF_KIND_AUX); expand_plain_kernel<<<dim3(c->n_gather_blocks, (nvec + 31) / 32), 256, 0, c->stream>>>(ep); }
+    {
+        ProfScope ps(c, CSF_KIND_AUX);
+        const dim3 eg(c->n_gather_blocks, (nvec + 31) / 32);
+        if (c->proj_complex) expand_plain_kernel<true><<<eg, 256, 0, c->stream>>>(ep); else expand_plain_kernel<false><<<eg, 256, 0, c->stream>>>(ep);
+    }
     CSF_CUDA(c, cudaGetLastError());
-    c->launches += 3;
+    c->launches += 2;
+    return CSF_OK;
+}
+
+static int check_dense_args(csf_ctx* c, const void* dX, const void* dY, int64_t ld, int nvec, const void* d_work, size_t work_bytes, size_t need) {
+    if (!dX || !dY) return fail(c, CSF_EINVAL, "NULL block pointer");
+    if (dX == dY) return fail(c, CSF_EINVAL, "Y must not alias X");
+    if (nvec < 0 || ld < nvec) return fail(c, CSF_EINVAL, "need 0 <= nvec <= ld");
+    if (c->dense_nq == 0) return fail(c, CSF_ESTATE, "csf_set_potential_quadrature has not been called (it must follow csf_set_kpoint)");
+    if (nvec > 0 && need > 0 && (!d_work || work_bytes < need)) return fail(c, CSF_EINVAL, "workspace too small");
+    return CSF_OK;
+}
+
+int csf_apply_H_dense(csf_ctx* c, const csf_c128* dX, csf_c128* dY, int64_t ld, int nvec, void* d_work, size_t work_bytes) {
+    CSF_GUARD_BEGIN
+    if (!c) return CSF_EINVAL;
+    // (one apply needs the coefficient buffers only; csf_dense_workspace_bytes also covers csf_filter_dense's block buffer)
+    int rc = check_dense_args(c, dX, dY, ld, nvec, d_work, work_bytes, c->natoms > 0 ? 3 * coef_bytes(c, std::max(nvec, 0)) : 0);
+    if (rc != CSF_OK || nvec == 0) return rc;
+    CSF_CUDA(c, cudaSetDevice(c->device));
+    rc = enqueue_zero(c, reinterpret_cast<double*>(dY), ld, nvec);
+    if (rc != CSF_OK) return rc;
+    char* coef = static_cast<char*>(d_work);
+    return enqueue_dense_step(c, reinterpret_cast<const double2*>(dX), ld, reinterpret_cast<double*>(dY), ld, nvec, 1.0, 0, 0.0, coef);
+    CSF_GUARD_END(c)
+}
+
+int csf_filter_dense(csf_ctx* c, const csf_c128* dX, csf_c128* dY, int64_t ld, int nvec, int degree, double a, double b, void* d_work, size_t work_bytes) {
+    CSF_GUARD_BEGIN
+    if (!c) return CSF_EINVAL;
+    if (degree < 0) return fail(c, CSF_EINVAL, "degree < 0");
+    if (!(a < b)) return fail(c, CSF_EINVAL, "need a < b");
+    size_t need = 0; csf_dense_workspace_bytes(c, std::max(nvec, 0), &need);
+    int rc = check_dense_args(c, dX, dY, ld, nvec, d_work, work_bytes, degree >= 1 ? need : 0);
+    if (rc != CSF_OK || nvec == 0) return rc;
+    CSF_CUDA(c, cudaSetDevice(c->device));
+    const long long rows = 2 * c->M;
+    const double cc = 0.5 * (a + b), ee = 0.5 * (b - a);
+    const double2* X = reinterpret_cast<const double2*>(dX);
+    double* Y = reinterpret_cast<double*>(dY);
+    if (degree == 0) {
+        { ProfScope ps(c, CSF_KIND_AUX); rot_copy_kernel<<<c->sm_count * 8, 256, 0, c->stream>>>(X, ld, reinterpret_cast<double2*>(Y), ld, rows, nvec, 0); }
+        CSF_CUDA(c, cudaGetLastError()); c->launches += 1;
+        return CSF_OK;
+    }
+    // the accumulate form of csf_filter: W_k = i^(m-k) T_k(H~) X, W_{k+1} = W_{k-1} + (-2i/e)(Hhat - c) W_k, W_m = T_m(H~) X
+    char* w = static_cast<char*>(d_work);
+    double* Wk = reinterpret_cast<double*>(w);
+    char* coef = w + block_bytes(c, nvec);
+    const bool even_m = (degree % 2 == 0);
+    double* buf0 = even_m ? Y : Wk;  const long long ld0 = even_m ? ld : nvec;
+    double* buf1 = even_m ? Wk : Y;  const long long ld1 = even_m ? nvec : ld;
+    if (degree >= 2) {
+        { ProfScope ps(c, CSF_KIND_AUX); rot_copy_kernel<<<c->sm_count * 8, 256, 0, c->stream>>>(X, ld, reinterpret_cast<double2*>(buf0), ld0, rows, nvec, degree & 3); }
+        CSF_CUDA(c, cudaGetLastError()); c->launches += 1;
+    }
+    rc = enqueue_zero(c, buf1, ld1, nvec); if (rc != CSF_OK) return rc;
+    rc = enqueue_dense_step(c, X, ld, buf1, ld1, nvec, 1.0 / ee, (degree + 3) & 3, cc, coef);
+    if (rc != CSF_OK) return rc;
+    for (int k = 1; k < degree; ++k) {
+        const bool odd = (k & 1);
+        rc = enqueue_dense_step(c, reinterpret_cast<const double2*>(odd ? buf1 : buf0), odd ? ld1 : ld0, odd ? buf0 : buf1, odd ? ld0 : ld1, nvec, 2.0 / ee, 3, cc, coef);
+        if (rc != CSF_OK) return rc;
+    }
     return CSF_OK;
     CSF_GUARD_END(c)
 }

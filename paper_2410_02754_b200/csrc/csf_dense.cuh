@@ -28,6 +28,7 @@ struct CellMatParams {
     const double* vq;        // [E][nq3][4]: V_eff, B_x, B_y, B_z at the quadrature points
     double* out;             // fragment order, see above
     int nq3, n3, n3p;
+    double vshift;           // added to V_eff at every quadrature point (|k|^2/2 of the k-point Hamiltonian)
 };
 
 constexpr int kCmChunk = 128;     // quadrature points staged per pass
@@ -48,7 +49,7 @@ __global__ void __launch_bounds__(256) cellmat_build_kernel(const __grid_constan
         for (int q0 = 0; q0 < A.nq3; q0 += kCmChunk) {
             const int nqc = min(kCmChunk, A.nq3 - q0);
             __syncthreads();
-            for (int t = threadIdx.x; t < nqc * 4; t += 256) f[t >> 2][t & 3] = A.wJ[q0 + (t >> 2)] * A.vq[(e * A.nq3 + q0 + (t >> 2)) * 4 + (t & 3)];
+            for (int t = threadIdx.x; t < nqc * 4; t += 256) f[t >> 2][t & 3] = A.wJ[q0 + (t >> 2)] * (A.vq[(e * A.nq3 + q0 + (t >> 2)) * 4 + (t & 3)] + ((t & 3) == 0 ? A.vshift : 0.0));
             for (int t = threadIdx.x; t < nqc * 8; t += 256) na[t >> 3][t & 7] = A.Ns[(long long)(q0 + (t >> 3)) * A.n3p + mt * 8 + (t & 7)];
             __syncthreads();
             if (b < A.n3p)
@@ -85,6 +86,8 @@ struct DenseParams {
     double* Y; long long ldy;          // [2M][ldy] complex128 as reals; Y += ...
     int nvec, p, n3, n3p;
     int ncx, ncy, ncz, nfx, nfy, nfz, bcx, bcy, bcz;      // bc: 0 periodic, 1 Dirichlet (boundary nodes removed)
+    double fr, fi;                     // Y += f (H^(e) X^(e)), f = fr + i fi (1 for a plain apply; sc i^rot for a recurrence step)
+    const double* gk;                  // KPT: S^(e) sum_d k_d G_d^(e) S^(e), G_d[a][b] = int N_a d_d N_b, fragment order [m-tile][k-step][32]; the same for all cells
 };
 
 __device__ __forceinline__ void dense_dmma(double& d0, double& d1, double a, double b) {
@@ -107,7 +110,9 @@ template <int VC> __host__ __device__ constexpr size_t dense_smem(int n3p) { ret
 
 // grid = cells x vector chunks (chunk fastest): the chunks of one cell run next to each other, so the cell's matrices (1.5 MB at order 5)
 // are fetched from HBM once and served from L2 to the other chunks. 8 warps, warp w takes the m-tiles w, w + 8, ...
-template <int VC>
+// KPT: the Bloch term -i k.grad of eq.40, spin-diagonal: Yu -= i Gk Xu, Yd -= i Gk Xd; it joins the two accumulators
+// that are multiplied by -+ i anyway: T2 = M2 Xd + Gk Xu, T1 = M2 Xu - Gk Xd.
+template <int VC, bool KPT>
 __global__ void __launch_bounds__(256, 2) dense_cell_kernel(const __grid_constant__ DenseParams A) {
     constexpr int LDW = dense_ldw<VC>(), NT = VC / 4;          // n-tiles of 8 real columns = 4 complex vectors
     extern __shared__ __align__(16) unsigned char dense_raw[];
@@ -151,9 +156,12 @@ __global__ void __launch_bounds__(256, 2) dense_cell_kernel(const __grid_constan
 #pragma unroll
         for (int j = 0; j < NT; ++j) { au[j][0] = au[j][1] = ad[j][0] = ad[j][1] = t1[j][0] = t1[j][1] = t2[j][0] = t2[j][1] = 0.0; }
         const double* m = A.mat + (((long long)e * mtn + mt) * ksn) * 128 + lane;
+        const double* mg = A.gk + ((long long)mt * ksn) * 32 + lane;
 #pragma unroll 4
         for (int ks = 0; ks < ksn; ++ks) {
             const double mp = __ldg(m + ks * 128), mq = __ldg(m + ks * 128 + 32), m1 = __ldg(m + ks * 128 + 64), m2 = __ldg(m + ks * 128 + 96);
+            double gp = 0.0, gn = 0.0;
+            if (KPT) { gp = __ldg(mg + ks * 32); gn = -gp; }
             const double* bu = Xu + (size_t)(ks * 4 + kk) * LDW;
             const double* bd = Xd + (size_t)(ks * 4 + kk) * LDW;
 #pragma unroll
@@ -162,6 +170,7 @@ __global__ void __launch_bounds__(256, 2) dense_cell_kernel(const __grid_constan
                 dense_dmma(au[j][0], au[j][1], mp, xu); dense_dmma(au[j][0], au[j][1], m1, xd);
                 dense_dmma(ad[j][0], ad[j][1], m1, xu); dense_dmma(ad[j][0], ad[j][1], mq, xd);
                 dense_dmma(t1[j][0], t1[j][1], m2, xu); dense_dmma(t2[j][0], t2[j][1], m2, xd);
+                if (KPT) { dense_dmma(t2[j][0], t2[j][1], gp, xu); dense_dmma(t1[j][0], t1[j][1], gn, xd); }
             }
         }
         const int g = node[mt * 8 + rw];
@@ -173,8 +182,9 @@ __global__ void __launch_bounds__(256, 2) dense_cell_kernel(const __grid_constan
             // Yu = Au - i T2,  Yd = Ad + i T1
             double* yu = A.Y + ((2LL * g) * A.ldy + v) * 2;
             double* yd = A.Y + ((2LL * g + 1) * A.ldy + v) * 2;
-            atomicAdd(yu, au[j][0] + t2[j][1]); atomicAdd(yu + 1, au[j][1] - t2[j][0]);
-            atomicAdd(yd, ad[j][0] - t1[j][1]); atomicAdd(yd + 1, ad[j][1] + t1[j][0]);
+            const double ur = au[j][0] + t2[j][1], ui = au[j][1] - t2[j][0], dr = ad[j][0] - t1[j][1], di = ad[j][1] + t1[j][0];
+            atomicAdd(yu, A.fr * ur - A.fi * ui); atomicAdd(yu + 1, A.fr * ui + A.fi * ur);
+            atomicAdd(yd, A.fr * dr - A.fi * di); atomicAdd(yd + 1, A.fr * di + A.fi * dr);
         }
     }
 }
@@ -186,6 +196,8 @@ __global__ void __launch_bounds__(256, 2) dense_cell_kernel(const __grid_constan
 // D = Delta C per atom, plain layout [crows][ldc] complex (row = atom_coff + 2 chi + spin), eq.76
 struct DeltaPlainParams {
     const double2* C; double2* D; long long ldc; int nvec;
+    const double2* C2;            // NULL, or the gather with Im P~: the coefficients are C - i C2 = (Re P~ + i Im P~)^+ X
+    double fr, fi;                // D = f Delta C
     const long long* atom_coff; const int* atom_npj; const int* atom_type;
     const double2* delta; const long long* delta_ptr;
 };
@@ -201,11 +213,12 @@ __global__ void __launch_bounds__(256) delta_plain_kernel(const __grid_constant_
         double sr = 0.0, si = 0.0;
         for (int q = 0; q < nr; ++q) {
             const double2 d = __ldg(Dl + (long long)r * nr + q);
-            const double2 c = A.C[(base + q) * A.ldc + v];
+            double2 c = A.C[(base + q) * A.ldc + v];
+            if (A.C2) { const double2 c2 = A.C2[(base + q) * A.ldc + v]; c.x += c2.y; c.y -= c2.x; }
             sr = fma(d.x, c.x, sr); sr = fma(-d.y, c.y, sr);
             si = fma(d.x, c.y, si); si = fma(d.y, c.x, si);
         }
-        A.D[(base + r) * A.ldc + v] = make_double2(sr, si);
+        A.D[(base + r) * A.ldc + v] = make_double2(A.fr * sr - A.fi * si, A.fr * si + A.fi * sr);
     }
 }
 
@@ -216,11 +229,13 @@ struct ExpandPlainParams {
     double* Y; long long ldy; int nvec, mt;
     const int* gb_atom; const int* gb_beg; const int* gb_end; const int* gb_k0;
     const int* ent_node; const double* g_pack;
+    const double* g_pack_im;      // CPLX: Im P~ in the same order
     const long long* atom_coff; const int* atom_npj;
 };
 
 // grid (gather blocks, tiles of 32 vectors), 8 warps, lane = vector. D of the atom for these 32 vectors is staged in shared
 // memory once; a warp takes four entries at a time (one k-step of g_pack: the four P~ values of a projector are 32 consecutive bytes)
+template <bool CPLX>
 __global__ void __launch_bounds__(256) expand_plain_kernel(const __grid_constant__ ExpandPlainParams A) {
     __shared__ double2 Ds[64][32];
     const int b = blockIdx.x, atom = A.gb_atom[b], beg = A.gb_beg[b], end = A.gb_end[b], k0 = A.gb_k0[b];
@@ -243,6 +258,16 @@ __global__ void __launch_bounds__(256) expand_plain_kernel(const __grid_constant
                 ur[q] = fma(pv[q], cu.x, ur[q]); ui[q] = fma(pv[q], cu.y, ui[q]);
                 dr[q] = fma(pv[q], cd.x, dr[q]); di[q] = fma(pv[q], cd.y, di[q]);
             }
+            if (CPLX) {                         // + i Im P~ (cu, cd)
+                const double2* pki = reinterpret_cast<const double2*>(A.g_pack_im + ((long long)(k0 + ((e - beg) >> 2)) * A.mt) * 32);
+                const double2 q01 = __ldg(pki + (x >> 3) * 16 + (x & 7) * 2), q23 = __ldg(pki + (x >> 3) * 16 + (x & 7) * 2 + 1);
+                const double pw[4] = {q01.x, q01.y, q23.x, q23.y};
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    ur[q] = fma(-pw[q], cu.y, ur[q]); ui[q] = fma(pw[q], cu.x, ui[q]);
+                    dr[q] = fma(-pw[q], cd.y, dr[q]); di[q] = fma(pw[q], cd.x, di[q]);
+                }
+            }
         }
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
@@ -252,6 +277,19 @@ __global__ void __launch_bounds__(256) expand_plain_kernel(const __grid_constant
             double* yd = A.Y + ((2 * I + 1) * A.ldy + v) * 2;
             atomicAdd(yu, ur[q]); atomicAdd(yu + 1, ui[q]); atomicAdd(yd, dr[q]); atomicAdd(yd + 1, di[q]);
         }
+    }
+}
+
+// dst += alpha src on complex128 blocks (the shift term -f c X of a recurrence step on the dense path)
+__global__ void __launch_bounds__(256) caxpy_kernel(const double2* __restrict__ src, long long ld, double2* __restrict__ dst, long long ld_dst,
+                                                    long long rows, int nvec, double ar, double ai) {
+    const long long total = rows * nvec;
+    for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < total; t += (long long)gridDim.x * blockDim.x) {
+        const long long r = t / nvec; const int v = (int)(t % nvec);
+        const double2 z = src[r * ld + v];
+        double2 o = dst[r * ld_dst + v];
+        o.x += ar * z.x - ai * z.y; o.y += ar * z.y + ai * z.x;
+        dst[r * ld_dst + v] = o;
     }
 }
 

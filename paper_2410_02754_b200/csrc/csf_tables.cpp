@@ -67,6 +67,7 @@ bool build_gll(int p, Gll1D* g) {
     double D[kMaxN][kMaxN];
     for (int q = 0; q < n; ++q) for (int i = 0; i < n; ++i) D[q][i] = (q == i) ? 0.0 : Lp[q] / (Lp[i] * (g->xi[q] - g->xi[i]));
     D[0][0] = -0.25 * p * (p + 1.0); D[p][p] = 0.25 * p * (p + 1.0);
+    for (int q = 0; q < n; ++q) for (int i = 0; i < n; ++i) g->D[q][i] = D[q][i];
     for (int i = 0; i < n; ++i) for (int j = 0; j < n; ++j) {
         double s = 0.0;
         for (int q = 0; q < n; ++q) s += D[q][i] * g->w[q] * D[q][j];

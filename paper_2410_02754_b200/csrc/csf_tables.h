@@ -22,6 +22,7 @@ struct Gll1D {
     int p = 0, n = 0;
     double xi[kMaxN], w[kMaxN], v[kMaxN], alpha = 0.0;
     double K[kMaxN][kMaxN];   // Khat
+    double D[kMaxN][kMaxN];   // D_qi = l_i'(xi_q); w_q D_qi = int l_q l_i' exactly (degree 2p - 1), the 1-D gradient matrix of eq.40's -i k.grad term
 };
 
 struct Dir1D {                // scaled 1-D operators of one mesh direction
