@@ -371,7 +371,6 @@ def measure_dense(args, peaks):
     torch.cuda.synchronize(); t0 = time.perf_counter()
     ctx.set_potential_quadrature(nq, vq)
     ms_setup = (time.perf_counter() - t0) * 1e3
-    del vq
     rows, nvec = 2 * ctx.M, cfg.nvec
     gen = torch.Generator(device="cuda"); gen.manual_seed(777)
     X = torch.empty((rows, nvec), dtype=torch.complex128, device="cuda"); torch.view_as_real(X).normal_(0.0, math.sqrt(0.5), generator=gen)
@@ -396,6 +395,16 @@ def measure_dense(args, peaks):
     ms_cell, n_cell = ctx.profile_read(binding.KIND_CELL)
     rest = {binding.KIND_NAMES[kd]: (lambda r: r[0] / max(r[1], 1))(ctx.profile_read(kd)) for kd in (binding.KIND_PGATHER, binding.KIND_DELTA, binding.KIND_AUX)}
     ctx.profile_enable(False)
+    # the same apply at a k-point (eq.40-42: Bloch term in the cell product, complex projectors)
+    kvec = np.array([0.21, -0.13, 0.08])
+    ctx.set_kpoint(kvec)
+    ctx.set_projectors_complex(sysm.node_ptr, sysm.node_idx, sysm.nproj, synth.bloch_pvals(sysm, ctx.node_coords(), kvec), sysm.atom_type, sysm.delta, sysm.delta_ptr)
+    ctx.set_potential_quadrature(nq, vq)
+    ctx.profile_enable(True)
+    ms_dense_k = timed(lambda: ctx.apply_H_dense(X, Y, nvec, nvec, work), 3)
+    ms_cell_k, n_cell_k = ctx.profile_read(binding.KIND_CELL)
+    ctx.profile_enable(False)
+    del vq
     n3 = (cfg.order + 1) ** 3
     E = cfg.ncell[0] * cfg.ncell[1] * cfg.ncell[2]
     flops = 6.0 * 2.0 * 2.0 * n3 * n3 * nvec * E                       # six real n3 x n3 products on 2 nvec real columns per cell
@@ -410,6 +419,10 @@ def measure_dense(args, peaks):
            "dense_kernel_ms": ms_k, "dense_kernel_tflops": flops / ms_k / 1e9, "dense_kernel_frac_of_fp64_peak": flops / ms_k / 1e9 / peak64,
            "dense_kernel_matrix_gbs_if_read_once": mat_bytes / ms_k / 1e6,
            "nonlocal_kernels_ms": {"proj_gather": rest["proj_gather"], "delta": rest["delta"], "expansion": rest["aux"]},
+           "kpoint": {"k": kvec.tolist(), "apply_dense_ms": ms_dense_k, "dense_kernel_ms": ms_cell_k / max(n_cell_k, 1),
+                      "dense_kernel_tflops": flops * 8.0 / 6.0 / (ms_cell_k / max(n_cell_k, 1)) / 1e9,
+                      "dense_kernel_frac_of_fp64_peak": flops * 8.0 / 6.0 / (ms_cell_k / max(n_cell_k, 1)) / 1e9 / peak64,
+                      "note": "eight real products per cell instead of six (the Bloch term -i k.grad), complex projector entries"},
            "units_per_s_dense": rows * nvec / (ms_dense * 1e-3), "units_per_s_sum_factorised": rows * nvec / (ms_sf * 1e-3),
            "finite": bool(torch.isfinite(torch.view_as_real(Y[::4099])).all().item())}
     del X, Y, work, ctx
