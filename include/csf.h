@@ -254,8 +254,10 @@ int csf_filter_dense(csf_ctx* ctx, const csf_c128* dX, csf_c128* dY, int64_t ld,
  *   H^k,loc  = int [1/2 grad N_I.grad N_J - i N_I k.grad N_J + (|k|^2/2 + V_eff) N_I N_J] d_ab + sum_d B^d N_I N_J sigma^d_ab
  *   H^k,nloc = sum_a sum_{X X'} P^k_{I X} D^{X X'}_ab conj(P^k_{J X'}),  P^k_{I X} complex (Bloch phases e^{-ik.(r - L_q)})
  * The gradient term is integrated exactly; |k|^2/2 is integrated with V_eff's rule (reading A19). The
- * sum-factorised entry points (csf_apply_H, csf_filter, csf_filter_host, csf_rr_project, csf_lanczos, ...) hold the
- * Gamma-point operator with real projectors and fail with CSF_ESTATE while a k-point or complex projectors are set. */
+ * sum-factorised entry points (csf_apply_H, csf_apply_H_static, csf_filter, csf_filter_host) hold the Gamma-point operator
+ * with real projectors and fail with CSF_ESTATE while a k-point or complex projectors are set. csf_rr_project and csf_lanczos
+ * apply the operator the context holds: in that state Hhat^k through the dense cell matrices (quadrature-rule potential), so
+ * that csf_lanczos -> csf_filter_dense -> csf_rr_project / _solve / _rotate -> csf_density is a whole ChFSI pass at a k-point. */
 
 /* Bloch vector k_host[3] (1/bohr); (0, 0, 0) switches the k-point terms off. Invalidates the cell matrices:
  * csf_set_potential_quadrature must be called after it. Meaningful on periodic directions (not checked). */

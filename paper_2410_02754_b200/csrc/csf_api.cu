@@ -330,7 +330,7 @@ int check_block_args(csf_ctx* c, const void* x, const void* y, long long ld, int
     if (!x || !y) return fail(c, CSF_EINVAL, "NULL block pointer");
     if (x == y) return fail(c, CSF_EINVAL, "Y must not alias X");
     if (nvec < 0 || ld < nvec) return fail(c, CSF_EINVAL, "need 0 <= nvec <= ld");
-    if (!c->have_pot) return fail(c, CSF_ESTATE, "csf_set_potential has not been called");
+    if (!c->have_pot && !(c->kpt_on || c->proj_complex)) return fail(c, CSF_ESTATE, "csf_set_potential has not been called");
     if (nvec > 0 && need > 0 && (!work || work_bytes < need)) return fail(c, CSF_EINVAL, "workspace too small");
     return CSF_OK;
 }
@@ -1014,9 +1014,23 @@ __global__ void __launch_bounds__(256) recip_kernel(const double* __restrict__ a
 
 extern "C" {
 
+static int enqueue_dense_step(csf_ctx* c, const double2* src, long long ld, double* dst, long long ld_dst, int nvec, double sc, int rot, double shift, char* coef);
+
+// Scratch of one H apply with whichever operator the context holds, and the apply itself (dst += Hhat src): the sum-factorised
+// Gamma-point operator, or, while a k-point / complex projectors are set, the dense-path operator Hhat^k (csf_dense.cuh)
+static size_t apply_scratch_bytes(const csf_ctx* c, int nvec) { return std::max(coef_bytes(c, nvec) + ctp_bytes(c, nvec), 3 * coef_bytes(c, nvec)); }
+static bool dense_only(const csf_ctx* c) { return c->kpt_on || c->proj_complex; }
+static int enqueue_apply(csf_ctx* c, const void* src, long long ld, double* dst, long long ld_dst, int nvec, char* scratch) {
+    if (dense_only(c)) {
+        if (c->dense_nq == 0) return fail(c, CSF_ESTATE, "csf_set_potential_quadrature has not been called (it must follow csf_set_kpoint)");
+        return enqueue_dense_step(c, static_cast<const double2*>(src), ld, dst, ld_dst, nvec, 1.0, 0, 0.0, scratch);
+    }
+    return enqueue_step(c, src, ld, dst, ld_dst, nvec, 1.0, 0, 0.0, reinterpret_cast<double*>(scratch), reinterpret_cast<double*>(scratch + coef_bytes(c, nvec)));
+}
+
 int csf_rr_workspace_bytes(const csf_ctx* c, int nvec, size_t* bytes) {
     if (!c || !bytes || nvec < 0) return CSF_EINVAL;
-    *bytes = block_bytes(c, nvec) + coef_bytes(c, nvec) + ctp_bytes(c, nvec) + rr_gram_bytes(nvec) + 256;
+    *bytes = block_bytes(c, nvec) + apply_scratch_bytes(c, nvec) + rr_gram_bytes(nvec) + 256;
     return CSF_OK;
 }
 
@@ -1030,11 +1044,10 @@ int csf_rr_project(csf_ctx* c, const csf_c128* dX, int64_t ld, int nvec, csf_c12
     CSF_CUDA(c, cudaSetDevice(c->device));
     char* w = static_cast<char*>(d_work);
     double* HX = reinterpret_cast<double*>(w);                                        // [2M][nvec] complex128
-    double* dC = reinterpret_cast<double*>(w + block_bytes(c, nvec));
-    double* dCt = reinterpret_cast<double*>(w + block_bytes(c, nvec) + coef_bytes(c, nvec));
-    double* dG = reinterpret_cast<double*>(w + block_bytes(c, nvec) + coef_bytes(c, nvec) + ctp_bytes(c, nvec));
+    char* scratch = w + block_bytes(c, nvec);
+    double* dG = reinterpret_cast<double*>(w + block_bytes(c, nvec) + apply_scratch_bytes(c, nvec));
     rc = enqueue_zero(c, HX, nvec, nvec); if (rc != CSF_OK) return rc;
-    rc = enqueue_step(c, reinterpret_cast<const double*>(dX), ld, HX, nvec, nvec, 1.0, 0, 0.0, dC, dCt); if (rc != CSF_OK) return rc;
+    rc = enqueue_apply(c, dX, ld, HX, nvec, nvec, scratch); if (rc != CSF_OK) return rc;
     const double* Xr = reinterpret_cast<const double*>(dX);
     rc = enqueue_gram(c, Xr, 2 * ld, HX, 2LL * nvec, nvec, dG, reinterpret_cast<double2*>(dHs), 1); if (rc != CSF_OK) return rc;      // Hs = X^dagger (Hhat X)
     return enqueue_gram(c, Xr, 2 * ld, Xr, 2 * ld, nvec, dG, reinterpret_cast<double2*>(dSs), 1);                                   // Ss = X^dagger X
@@ -1133,7 +1146,7 @@ int csf_density(csf_ctx* c, const csf_c128* dX, int64_t ld, int nvec, const doub
 
 int csf_lanczos_workspace_bytes(const csf_ctx* c, size_t* bytes) {
     if (!c || !bytes) return CSF_EINVAL;
-    *bytes = 3 * block_bytes(c, 1) + coef_bytes(c, 1) + ctp_bytes(c, 1) + 512;
+    *bytes = 3 * block_bytes(c, 1) + apply_scratch_bytes(c, 1) + 512;
     return CSF_OK;
 }
 
@@ -1141,15 +1154,15 @@ int csf_lanczos(csf_ctx* c, const csf_c128* d_v0, int k, double* alpha_host, dou
     if (!c) return CSF_EINVAL;
     CSF_GUARD_BEGIN
     if (!d_v0 || !alpha_host || !beta_host || k < 1) return fail(c, CSF_EINVAL, "bad argument");
-    if (!c->have_pot) return fail(c, CSF_ESTATE, "csf_set_potential has not been called");
+    if (!c->have_pot && !dense_only(c)) return fail(c, CSF_ESTATE, "csf_set_potential has not been called");
     size_t need = 0; csf_lanczos_workspace_bytes(c, &need);
     if (!d_work || work_bytes < need) return fail(c, CSF_EINVAL, "workspace too small");
     CSF_CUDA(c, cudaSetDevice(c->device));
     const long long n = 2 * c->M; const size_t vb = block_bytes(c, 1);
     char* w8 = static_cast<char*>(d_work);
     double2* v = reinterpret_cast<double2*>(w8); double2* vprev = reinterpret_cast<double2*>(w8 + vb); double2* w = reinterpret_cast<double2*>(w8 + 2 * vb);
-    double* dC = reinterpret_cast<double*>(w8 + 3 * vb); double* dCt = reinterpret_cast<double*>(w8 + 3 * vb + coef_bytes(c, 1));
-    double* scratch = reinterpret_cast<double*>(w8 + 3 * vb + coef_bytes(c, 1) + ctp_bytes(c, 1));
+    char* apply_scratch = w8 + 3 * vb;
+    double* scratch = reinterpret_cast<double*>(w8 + 3 * vb + apply_scratch_bytes(c, 1));
     const int grid = c->sm_count * 8;
     double hs[2] = {0.0, 0.0};
     // v = v0 / |v0|, vprev = 0
@@ -1164,7 +1177,7 @@ int csf_lanczos(csf_ctx* c, const csf_c128* d_v0, int k, double* alpha_host, dou
     double beta = 0.0; int done = 0;
     for (int j = 0; j < k; ++j) {
         int rc = enqueue_zero(c, reinterpret_cast<double*>(w), 1, 1); if (rc != CSF_OK) return rc;
-        rc = enqueue_step(c, reinterpret_cast<const double*>(v), 1, reinterpret_cast<double*>(w), 1, 1, 1.0, 0, 0.0, dC, dCt); if (rc != CSF_OK) return rc;
+        rc = enqueue_apply(c, v, 1, reinterpret_cast<double*>(w), 1, 1, apply_scratch); if (rc != CSF_OK) return rc;
         CSF_CUDA(c, cudaMemsetAsync(scratch, 0, 2 * sizeof(double), c->stream));
         lanczos_a_kernel<<<grid, 256, 0, c->stream>>>(w, vprev, v, beta, n, scratch);
         CSF_CUDA(c, cudaMemcpyAsync(hs, scratch, sizeof(double), cudaMemcpyDeviceToHost, c->stream));

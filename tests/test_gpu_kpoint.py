@@ -115,3 +115,31 @@ def test_state_rules_of_the_kpoint_calls():
     gpu.set_potential_quadrature(4, vq)
     gpu.apply_H(X, Y, 4, 4, work); gpu.apply_H_dense(X, Y, 4, 4, work)
     torch.cuda.synchronize()
+
+
+def test_rayleigh_ritz_and_lanczos_at_a_kpoint():
+    """csf_rr_project and csf_lanczos apply the operator the context holds: Hhat^k on the dense path here."""
+    import torch
+    from oracle import kpoint_oracle as KP
+    from oracle import subspace_oracle as S
+    from helpers import rel_fro
+    kvec = np.array([0.3, -0.2, 0.15])
+    ref0, gpu, s, vq, proj = _setup((5, 5, 5), (7.5, 7.5, 7.5), 3, (0, 0, 0), 2, kvec, 5)
+    apply = lambda Z: KP.apply_H_k(ref0, 5, vq, kvec, Z, proj)
+    N = 12
+    X = synth.random_block(s.rng, 2 * ref0.M, N)
+    dX = torch.from_numpy(X).cuda()
+    dHs = torch.empty((N, N), dtype=torch.complex128, device="cuda"); dSs = torch.empty_like(dHs); dQ = torch.empty_like(dHs)
+    work = torch.empty(gpu.rr_workspace_bytes(N), dtype=torch.uint8, device="cuda")
+    gpu.rr_project(dX, N, N, dHs, dSs, work)
+    torch.cuda.synchronize()
+    Hr, Sr = S.rr_project(apply, X)
+    assert rel_fro(dHs.cpu().numpy(), Hr) < 1e-11 and rel_fro(dSs.cpu().numpy(), Sr) < 1e-12
+    lam = gpu.rr_solve(dHs, dSs, N, dQ)
+    lam_ref, _ = S.rr_solve(Hr, Sr)
+    assert np.allclose(lam, lam_ref, rtol=0, atol=1e-9 * np.abs(lam_ref).max())
+    v0 = synth.random_block(s.rng, 2 * ref0.M, 1)
+    lw = torch.empty(gpu.lanczos_workspace_bytes(), dtype=torch.uint8, device="cuda")
+    al, be = gpu.lanczos(torch.from_numpy(v0).cuda(), 12, lw)
+    alr, ber = S.lanczos(apply, v0, 12)
+    assert np.allclose(al[:8], alr[:8], rtol=1e-10) and np.allclose(be[:8], ber[:8], rtol=1e-10)
