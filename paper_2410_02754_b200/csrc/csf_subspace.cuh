@@ -26,13 +26,15 @@ template <int N> __device__ __forceinline__ void sub_cp_wait() { asm volatile("c
 
 constexpr int kGT = 64;            // output tile edge (real columns) of gram / rotate
 constexpr int kGK = 32;            // rows (gram) / inner columns (rotate) per shared-memory slab
-constexpr int kGP = kGT + 8;       // padded row of a [k][64] slab: rows k, k+1 land on disjoint bank halves (2 wavefronts per LDS.64)
+constexpr int kGP = kGT + 4;       // padded row of a [k][64] slab: a DMMA fragment reads rows k .. k+3 at columns c .. c+7; with the rows 4 doubles
+                                   // apart mod 16 each half-warp covers 16 different 8-byte banks (2 wavefronts per LDS.64, the minimum)
 constexpr int kRP = kGK + 4;       // padded row of a [64][k] slab (rotate's A operand)
 constexpr size_t kGramSmem = (size_t)2 * 2 * kGK * kGP * sizeof(double);
 constexpr size_t kRotSmem = (size_t)2 * (kGT * kRP + kGK * kGP) * sizeof(double);
 
 // G[ca][cb] += sum_{r in this CTA's row range} A[r][ca] B[r][cb]; blockIdx.x = (tile m, tile n), blockIdx.y = row range.
-// sym: only tiles with n >= m (Hermitian result). 8 warps: warp w owns the 8 x 64 strip of m-tile w of the 64 x 64 tile.
+// sym: only tiles with n >= m (Hermitian result). 8 warps as 4 x 2: warp (wm, wn) owns the 16 x 32 block at (16 wm, 32 wn) of the
+// 64 x 64 tile: 2 A + 4 B fragment loads per 8 DMMAs (an 8 x 64 strip per warp takes 9, and the loads, not the tensor pipe, bound it).
 __global__ void __launch_bounds__(256) gram_kernel(const double* __restrict__ A, long long lda, const double* __restrict__ B, long long ldb,
                                                    int ncols, long long rows, long long rows_per_cta, double* __restrict__ G, int ldg, int sym) {
     extern __shared__ __align__(16) double sm[];
@@ -57,31 +59,39 @@ __global__ void __launch_bounds__(256) gram_kernel(const double* __restrict__ A,
         }
         sub_cp_commit();
     };
-    double c[8][2];
+    const int wm = warp >> 1, wn = warp & 1;
+    double c[2][4][2];
 #pragma unroll
-    for (int nt = 0; nt < 8; ++nt) { c[nt][0] = 0.0; c[nt][1] = 0.0; }
+    for (int mt = 0; mt < 2; ++mt)
+#pragma unroll
+        for (int nt = 0; nt < 4; ++nt) { c[mt][nt][0] = 0.0; c[mt][nt][1] = 0.0; }
     const long long nslab = (r1 - r0 + kGK - 1) / kGK;
     load_slab(0, r0);
     for (long long s = 0; s < nslab; ++s) {
         const int buf = (int)(s & 1);
         if (s + 1 < nslab) { load_slab(buf ^ 1, r0 + (s + 1) * kGK); sub_cp_wait<1>(); } else sub_cp_wait<0>();
         __syncthreads();
-        const double* as = As + buf * kGK * kGP + 8 * warp + (t >> 2);
-        const double* bs = Bs + buf * kGK * kGP + (t >> 2);
+        const double* as = As + buf * kGK * kGP + 16 * wm + (t >> 2);
+        const double* bs = Bs + buf * kGK * kGP + 32 * wn + (t >> 2);
 #pragma unroll
         for (int kk = 0; kk < kGK / 4; ++kk) {
-            const double a = as[(kk * 4 + (t & 3)) * kGP];
+            const double a0 = as[(kk * 4 + (t & 3)) * kGP], a1 = as[(kk * 4 + (t & 3)) * kGP + 8];
 #pragma unroll
-            for (int nt = 0; nt < 8; ++nt) sub_dmma(c[nt][0], c[nt][1], a, bs[(kk * 4 + (t & 3)) * kGP + 8 * nt]);
+            for (int nt = 0; nt < 4; ++nt) {
+                const double b = bs[(kk * 4 + (t & 3)) * kGP + 8 * nt];
+                sub_dmma(c[0][nt][0], c[0][nt][1], a0, b); sub_dmma(c[1][nt][0], c[1][nt][1], a1, b);
+            }
         }
         __syncthreads();
     }
-    const int gm = m0 + 8 * warp + (t >> 2);
-    if (gm < ncols) {
 #pragma unroll
-        for (int nt = 0; nt < 8; ++nt) {
-            const int gn = n0 + 8 * nt + 2 * (t & 3);
-            if (gn < ncols) { atomicAdd(G + (long long)gm * ldg + gn, c[nt][0]); atomicAdd(G + (long long)gm * ldg + gn + 1, c[nt][1]); }
+    for (int mt = 0; mt < 2; ++mt) {
+        const int gm = m0 + 16 * wm + 8 * mt + (t >> 2);
+        if (gm >= ncols) continue;
+#pragma unroll
+        for (int nt = 0; nt < 4; ++nt) {
+            const int gn = n0 + 32 * wn + 8 * nt + 2 * (t & 3);
+            if (gn < ncols) { atomicAdd(G + (long long)gm * ldg + gn, c[mt][nt][0]); atomicAdd(G + (long long)gm * ldg + gn + 1, c[mt][nt][1]); }
         }
     }
 }
@@ -132,31 +142,39 @@ __global__ void __launch_bounds__(256) rotate_kernel(const double* __restrict__ 
         }
         sub_cp_commit();
     };
-    double c[8][2];
+    const int wm = warp >> 1, wn = warp & 1;          // warp block 16 x 32, as in gram_kernel
+    double c[2][4][2];
 #pragma unroll
-    for (int nt = 0; nt < 8; ++nt) { c[nt][0] = 0.0; c[nt][1] = 0.0; }
+    for (int mt = 0; mt < 2; ++mt)
+#pragma unroll
+        for (int nt = 0; nt < 4; ++nt) { c[mt][nt][0] = 0.0; c[mt][nt][1] = 0.0; }
     const int nslab = (k2 + kGK - 1) / kGK;
     load_slab(0, 0);
     for (int s = 0; s < nslab; ++s) {
         const int buf = s & 1;
         if (s + 1 < nslab) { load_slab(buf ^ 1, (s + 1) * kGK); sub_cp_wait<1>(); } else sub_cp_wait<0>();
         __syncthreads();
-        const double* xs = Xs + (buf * kGT + 8 * warp + (t >> 2)) * kRP + (t & 3);
-        const double* qs = Qs + buf * kGK * kGP + (t >> 2);
+        const double* xs = Xs + (buf * kGT + 16 * wm + (t >> 2)) * kRP + (t & 3);
+        const double* qs = Qs + buf * kGK * kGP + 32 * wn + (t >> 2);
 #pragma unroll
         for (int kk = 0; kk < kGK / 4; ++kk) {
-            const double a = xs[kk * 4];
+            const double a0 = xs[kk * 4], a1 = xs[8 * kRP + kk * 4];
 #pragma unroll
-            for (int nt = 0; nt < 8; ++nt) sub_dmma(c[nt][0], c[nt][1], a, qs[(kk * 4 + (t & 3)) * kGP + 8 * nt]);
+            for (int nt = 0; nt < 4; ++nt) {
+                const double b = qs[(kk * 4 + (t & 3)) * kGP + 8 * nt];
+                sub_dmma(c[0][nt][0], c[0][nt][1], a0, b); sub_dmma(c[1][nt][0], c[1][nt][1], a1, b);
+            }
         }
         __syncthreads();
     }
-    const long long row = r0 + 8 * warp + (t >> 2);
-    if (row < rows) {
 #pragma unroll
-        for (int nt = 0; nt < 8; ++nt) {
-            const int gn = n0 + 8 * nt + 2 * (t & 3);
-            if (gn < k2) *reinterpret_cast<double2*>(U + row * ldu + gn) = make_double2(c[nt][0], c[nt][1]);
+    for (int mt = 0; mt < 2; ++mt) {
+        const long long row = r0 + 16 * wm + 8 * mt + (t >> 2);
+        if (row >= rows) continue;
+#pragma unroll
+        for (int nt = 0; nt < 4; ++nt) {
+            const int gn = n0 + 32 * wn + 8 * nt + 2 * (t & 3);
+            if (gn < k2) *reinterpret_cast<double2*>(U + row * ldu + gn) = make_double2(c[mt][nt][0], c[mt][nt][1]);
         }
     }
 }
