@@ -143,3 +143,33 @@ def test_rayleigh_ritz_and_lanczos_at_a_kpoint():
     al, be = gpu.lanczos(torch.from_numpy(v0).cuda(), 12, lw)
     alr, ber = S.lanczos(apply, v0, 12)
     assert np.allclose(al[:8], alr[:8], rtol=1e-10) and np.allclose(be[:8], ber[:8], rtol=1e-10)
+
+
+def test_bench_launch_configuration_on_sampled_columns():
+    """The launch configuration bench.py's dense leg times (order 5, cells of 1 bohr, 256 vectors = 16 chunks of 16 per cell, n_q = 8,
+    atoms with 18 projectors) on a 6^3-cell mesh, at a k-point with complex projectors: one H apply and a degree-6 filter of the whole
+    block on the GPU, the columns {0..3, 252..255} against the oracle."""
+    import torch
+    from oracle import kpoint_oracle as KP
+    from oracle import oracle as O
+    from oracle import dense_oracle as D
+    cfg = synth.scaled_config(synth.CONFIGS[3], (6, 6, 6), 4, nvec=256)
+    ref0 = O.RefCtx(cfg.ncell, cfg.box, cfg.order, cfg.bc); ref0.set_potential(np.zeros(ref0.M), None)
+    s = synth.make_system(cfg, ref0.node_coords(), ref0.mass_diag())
+    kvec = np.array([0.21, -0.13, 0.08]); nq = 8
+    pk = synth.bloch_pvals(s, ref0.node_coords(), kvec)
+    proj = (s.node_ptr, s.node_idx, s.nproj, pk, s.atom_type, s.delta, s.delta_ptr)
+    pts = D.quadrature_points(ref0, nq)
+    kk = [2 * np.pi / b for b in cfg.box]
+    vq = np.empty(pts.shape[:2] + (4,))
+    vq[..., 0] = -1.0 + 0.5 * np.cos(kk[0] * pts[..., 0]) * np.cos(kk[1] * pts[..., 1]) * np.cos(kk[2] * pts[..., 2])
+    vq[..., 1] = 0.1 * np.sin(kk[0] * pts[..., 0]); vq[..., 2] = 0.1 * np.sin(kk[1] * pts[..., 1]); vq[..., 3] = 0.1 * np.cos(kk[2] * pts[..., 2])
+    gpu = binding.Csf(cfg.ncell, cfg.box, cfg.order, cfg.bc)
+    gpu.set_projectors_complex(*proj); gpu.set_kpoint(kvec); gpu.set_potential_quadrature(nq, vq)
+    N = cfg.nvec
+    X = synth.random_block(s.rng, 2 * ref0.M, N)
+    cols = [0, 1, 2, 3, N - 4, N - 3, N - 2, N - 1]
+    apply = lambda Z: KP.apply_H_k(ref0, nq, vq, kvec, Z, proj)
+    assert_block_close(_dense(gpu, X)[:, cols], apply(X[:, cols]), TOL)
+    a, b = 6.0, 140.0
+    assert_block_close(_dense(gpu, X, filt=(6, a, b))[:, cols], KP.chebyshev_filter(apply, X[:, cols], 6, a, b), TOL)
