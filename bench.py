@@ -309,8 +309,14 @@ def measure(cfg_index, mode_name, steps, warmup, args, ctxs):
     t_hbm = (rm["bytes_column"] + rm["bytes_gather"]) * launch_units / (hbm * 1e9)
     t_alu = launch_units * (rm["flops_fp32"] / (peak32 * 1e12) + rm["flops_fp64"] / (peak64 * 1e12))
     roof = None
+    # csf_filter's fused half-block path: every column launch works on half the block and carries, in two extra warps, the
+    # projector gather of the other half (a5): its time, flops and bytes per H apply are those of two launches
+    fused = (not fp32) and (not args.no_projectors) and ctx.filter_fused_gather(nvec, mode)
+    per_apply = 2 if fused else 1
+    f_col = rm["flops_column"] + (72.0 * sysm.coverage if fused else 0.0)
+    b_col = rm["bytes_column"] + (rm["bytes_gather"] if fused else 0.0)
     if cell_n > 0:
-        t_cell = cell_ms / cell_n * 1e-3
+        t_cell = cell_ms / cell_n * per_apply * 1e-3
         if fp32:
             # the column kernel's own floors: 24 B/unit, its FP32 cell flops + the FP64 expansion (72 c_ov flops/unit)
             f32c = rm["flops_column"] - 72.0 * sysm.coverage
@@ -320,17 +326,19 @@ def measure(cfg_index, mode_name, steps, warmup, args, ctxs):
                     "unit": "TFLOP/s", "frac": t_floor / t_cell,
                     "peak_source": "mixed-pipe floor: FP32 cell flops at 148 SMs x 128 FMA/clk x 2 x %.0f MHz + FP64 expansion flops at half that, or 24 B/unit at the measured HBM copy rate, whichever is slower (DESIGN.md section 5)" % sm_max}
         else:
-            ach = rm["flops_column"] * launch_units / t_cell / 1e12
-            roof = {"kernel": "column_kernel (a1-a4, a7, a8)", "bound": "alu", "achieved": ach, "peak": peak64, "unit": "TFLOP/s", "frac": ach / peak64,
+            ach = f_col * launch_units / t_cell / 1e12
+            roof = {"kernel": "column_kernel with gather warps (a1-a5, a7, a8): two launches of half a block each per H apply" if fused else "column_kernel (a1-a4, a7, a8)",
+                    "bound": "alu", "achieved": ach, "peak": peak64, "unit": "TFLOP/s", "frac": ach / peak64,
                     "peak_source": "148 SMs x 64 FP64 FMA/clk x 2 x %.0f MHz (DESIGN.md; DFMA and DMMA share these units: 36.4 TF/s measured together)" % sm_max}
-        tr = ctxs["traffic"].get("cfg%d_%s" % (cfg.index, mode_name))
+        tr = ctxs["traffic"].get("cfg%d_%s%s" % (cfg.index, mode_name, "_fused" if fused else ""))
         roof.update({"traffic": (float(tr["dram_bytes_per_unit"]) * launch_units) if tr else None,
                      "traffic_source": tr["source"] if tr else None,
-                     "algorithmic_bytes": rm["bytes_column"] * launch_units, "flops_per_unit": rm["flops_column"],
+                     "algorithmic_bytes": b_col * launch_units, "flops_per_unit": f_col,
                      "flops_note": "algorithmic count of SURVEY 8(d) (cheapest algorithm implemented); the kernel executes fewer kinetic flops (shared z-planes are contracted once) and more projector flops (K 18 -> 20, partial row tiles)",
-                     "avg_launch_ms": t_cell * 1e3, "launches": cell_n, "share_of_step": cell_ms / ms_local,
-                     "hbm_achieved_gbs": rm["bytes_column"] * launch_units / t_cell / 1e9, "hbm_peak_gbs": hbm,
-                     "hbm_frac": rm["bytes_column"] * launch_units / t_cell / 1e9 / hbm,
+                     "avg_launch_ms": t_cell * 1e3 / per_apply, "launches": cell_n, "launches_per_apply": per_apply, "ms_per_apply": t_cell * 1e3,
+                     "share_of_step": cell_ms / ms_local,
+                     "hbm_achieved_gbs": b_col * launch_units / t_cell / 1e9, "hbm_peak_gbs": hbm,
+                     "hbm_frac": b_col * launch_units / t_cell / 1e9 / hbm,
                      "hbm_peak_source": "measured (MEASURED_PEAKS.json)" if peaks else "fallback"})
     t_apply = ms_per_step * 1e-3 / degree
     step = {"flops_per_unit": rm["flops_total"], "bytes_per_unit": rm["bytes_column"] + rm["bytes_gather"],
@@ -340,7 +348,7 @@ def measure(cfg_index, mode_name, steps, warmup, args, ctxs):
             "kernel_ms": {k: round(v[0] / steps, 3) for k, v in kinds.items()}}
     conf = workload_dict(cfg, sysm)
     conf.update({"block_vectors": nvec, "degree": degree, "bounds": [a, b], "lanczos_ritz": [tmin, tmax], "parallelism": f"replicas x{world}" if world > 1 else "single GPU",
-                 "mode": mode_name, "column_kernel_lanes": ctx.column_lanes(nvec, 1 if fp32 else 0), "setup_s": round(t_setup, 2)})
+                 "mode": mode_name, "column_kernel_lanes": ctx.column_lanes(nvec, 1 if fp32 else 0), "fused_gather": bool(fused), "setup_s": round(t_setup, 2)})
     res = {"value": value, "ms_per_step": ms_per_step, "steps": steps, "warmup": warmup, "dtype": "f32" if fp32 else "f64", "config": conf, "clocks": clocks,
            "gpu_launches": launches, "roofline": roof, "step_roofline": step, "finite": finite}
     if cfg.nstates > 0:

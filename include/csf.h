@@ -164,6 +164,16 @@ int csf_probe_fp64_mixed(int device, double* tflops_total);
  * parity-green but slower). Host-only query. */
 int csf_column_lanes(const csf_ctx* ctx, int nvec, int mode, int* lanes);
 
+/* Whether csf_filter runs a block of nvec vectors in `mode` on its fused half-block path (*fused = 1) or with one projector
+ * gather kernel per recurrence step (*fused = 0). Fused path (eq.84: the inner sum C^a = P^{a,T} X^(e') is all that a
+ * step needs from the other cells): complex128, order 5, 8 vectors per CTA, 18 projectors per atom, >= 64 vectors. The block is
+ * split into two halves (the first a multiple of 8 vectors) whose column steps alternate, and every column launch computes, in
+ * two extra warps, the projector coefficients the OTHER half needs next: the HBM-bound gather runs beside the latency-bound
+ * column step instead of after it. Results differ from the unfused path by summation order only.
+ * CSF_FUSED_GATHER=0 | 1 (read by csf_create) switches the path off | on for every block of >= 2 vectors (parity tests).
+ * Host-only query. */
+int csf_filter_fused_gather(const csf_ctx* ctx, int nvec, int mode, int* fused);
+
 /* Number of kernel launches (own kernels only, memsets excluded) enqueued by this context so far. */
 int csf_launch_count(const csf_ctx* ctx, int64_t* launches);
 

@@ -18,7 +18,7 @@ STATIC_SCRATCH_BYTES = 8 << 20          # CSF_STATIC_SCRATCH_BYTES of include/cs
 
 EXPORTS = ["csf_create", "csf_destroy", "csf_set_stream", "csf_num_nodes", "csf_node_coords", "csf_mass_diag", "csf_set_potential",
            "csf_set_projectors", "csf_workspace_bytes", "csf_apply_H", "csf_apply_H_static", "csf_filter", "csf_filter_host", "csf_set_host_chunk",
-           "csf_profile_enable", "csf_profile_read", "csf_probe_fp64_peak", "csf_probe_fp64_mixed", "csf_launch_count", "csf_column_lanes", "csf_set_variant", "csf_set_tuning", "csf_last_error",
+           "csf_profile_enable", "csf_profile_read", "csf_probe_fp64_peak", "csf_probe_fp64_mixed", "csf_launch_count", "csf_column_lanes", "csf_filter_fused_gather", "csf_set_variant", "csf_set_tuning", "csf_last_error",
            "csf_rr_workspace_bytes", "csf_rr_project", "csf_rr_solve", "csf_rr_rotate", "csf_density", "csf_lanczos_workspace_bytes", "csf_lanczos",
            "csf_tridiag_extremes", "csf_quadrature_points", "csf_set_potential_quadrature", "csf_dense_workspace_bytes", "csf_apply_H_dense",
            "csf_filter_dense", "csf_set_kpoint", "csf_set_projectors_complex"]
@@ -201,6 +201,9 @@ class Csf:
 
     def column_lanes(self, nvec, mode=0):
         n = C.c_int(); self._chk(self._L.csf_column_lanes(self._h, C.c_int(int(nvec)), C.c_int(int(mode)), C.byref(n))); return int(n.value)
+
+    def filter_fused_gather(self, nvec, mode=0):
+        n = C.c_int(); self._chk(self._L.csf_filter_fused_gather(self._h, C.c_int(int(nvec)), C.c_int(int(mode)), C.byref(n))); return bool(n.value)
 
     def launch_count(self):
         n = C.c_int64(); self._chk(self._L.csf_launch_count(self._h, C.byref(n))); return int(n.value)

@@ -41,6 +41,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
             (os.path.join(CSRC, "csf_tables.cpp"), os.path.join(objdir, "csf_tables.o"), [])]
     jobs += [(os.path.join(CSRC, "csf_column_p.cu"), os.path.join(objdir, f"csf_column_p{p}.o"), [f"-DCSF_P={p}"]) for p in range(1, 8)]
     jobs += [(os.path.join(CSRC, "csf_column_p.cu"), os.path.join(objdir, f"csf_column_wide_p{p}.o"), [f"-DCSF_P={p}", "-DCSF_WIDE=1"]) for p in (4, 5)]
+    # the wide order-5 FP64 kernel with two gather warps (fused projector gather of csf_filter's half-block path)
+    jobs += [(os.path.join(CSRC, "csf_column_p.cu"), os.path.join(objdir, "csf_column_wide_p5_g.o"), ["-DCSF_P=5", "-DCSF_WIDE=1", "-DCSF_GATHERW=2"])]
     jobs += [(os.path.join(CSRC, "csf_colws_p.cu"), os.path.join(objdir, f"csf_colws_p{p}.o"), [f"-DCSF_P={p}"]) for p in (4, 5)]
     with ThreadPoolExecutor(max_workers=min(12, os.cpu_count() or 2)) as ex:
         results = list(ex.map(lambda j: _run(["nvcc"] + cflags + j[2] + ["-c", j[0], "-o", j[1]]), jobs))

@@ -60,6 +60,7 @@ struct csf_ctx {
     int lanes_force = 0;                    // CSF_LANES=16|32 pins the column kernel variant (tests, sweeps); 0 = measured policy
     int kernel_force = 0;                   // CSF_KERNEL=wide|ws pins the 8-vector kernel of orders 4 and 5 (1 | 2)
     bool bulk_gather = true;                // CSF_GATHER=reg pins the register-load projector gather (tests run both)
+    int fused_gather = -1;                  // CSF_FUSED_GATHER=0|1: csf_filter's fused half-block path off | on for every block size; -1 = policy
     // projectors
     int natoms = 0, npj_uniform = 0, npjp = 0; long long crows = 0;
     DevBuf d_ent_node, d_atom_coff, d_atom_npj, d_atom_type, d_delta, d_delta_ptr, d_gb_atom, d_gb_beg, d_gb_end, d_gb_k0, d_g_pack;
@@ -183,15 +184,13 @@ int column_kind(const csf_ctx* c) {
 }
 int aux_warps(const csf_ctx* c, bool f32, int mode, int kind) { return kind == 2 ? kWsRoleWarps : col_aux_warps(c->p, f32, mode, kind == 1 ? 32 : 16); }
 
-// one step: dst += sc * i^rot * (Hhat - shift) src
-// src, dst: complex128 blocks, or complex64 blocks when f32 (CSF_FP32_INTERMEDIATE)
-int enqueue_step(csf_ctx* c, const void* src, long long ld, void* dst, long long ld_dst, int nvec, double sc, int rot, double shift,
-                 double* dC, double* dCt, bool f32 = false) {
-    // the sum-factorised kernels hold the Gamma-point operator with real projectors only
-    if (c->kpt_on || c->proj_complex) return fail(c, CSF_ESTATE, "a k-point / complex projectors are set: only the dense path (csf_apply_H_dense, csf_filter_dense) serves them");
+// What a column launch of the fused path carries for its gather warps: the block whose coefficients C = P~^T src they compute
+struct FusedGather { const void* src; long long ld; int nvec; double* dC; };
+
+// a5: C = P~^T src (cleared first) as a kernel of its own
+int enqueue_gather(csf_ctx* c, const void* src, long long ld, int nvec, double* dC, bool f32) {
     const long long ldc = nvec;
-    const int kind = column_kind(c); const bool ws = kind == 2;
-    if (c->natoms > 0) {
+    {
         CSF_CUDA(c, cudaMemsetAsync(dC, 0, (size_t)c->crows * ldc * sizeof(double2), c->stream));
         GatherParams gp{};
         gp.src = src; gp.ld = ld; gp.nvec = nvec;
@@ -202,8 +201,9 @@ int enqueue_step(csf_ctx* c, const void* src, long long ld, void* dst, long long
         dim3 gg(c->n_gather_blocks, (nvec + 16 * kGatherNT - 1) / (16 * kGatherNT));
         {
             ProfScope ps(c, CSF_KIND_PGATHER);
-            // complex128 blocks with 16-byte aligned rows: the bulk-copy kernel (src staged in shared memory by cp.async.bulk)
-            const bool bulk = !f32 && c->bulk_gather && ((uintptr_t)src & 15) == 0;
+            // blocks with 16-byte aligned rows: the bulk-copy kernel (src staged in shared memory by cp.async.bulk); complex64
+            // blocks have an even leading dimension (f32_block_bytes), so their rows qualify too
+            const bool bulk = c->bulk_gather && ((uintptr_t)src & 15) == 0 && (!f32 || ld % 2 == 0);
             if (bulk) {
                 static bool configured[64] = {};
                 int dev = 0; CSF_CUDA(c, cudaGetDevice(&dev));
@@ -211,9 +211,17 @@ int enqueue_step(csf_ctx* c, const void* src, long long ld, void* dst, long long
                     CSF_CUDA(c, cudaFuncSetAttribute(proj_gather_bulk_kernel<3, 2, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kGbSmem));
                     CSF_CUDA(c, cudaFuncSetAttribute(proj_gather_bulk_kernel<3, 3, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kGbSmem));
                     CSF_CUDA(c, cudaFuncSetAttribute(proj_gather_bulk_kernel<4, 4, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kGbSmem));
+                    CSF_CUDA(c, cudaFuncSetAttribute(proj_gather_bulk_kernel<3, 2, 2, float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gb_smem<float>()));
+                    CSF_CUDA(c, cudaFuncSetAttribute(proj_gather_bulk_kernel<3, 3, 0, float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gb_smem<float>()));
+                    CSF_CUDA(c, cudaFuncSetAttribute(proj_gather_bulk_kernel<4, 4, 0, float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gb_smem<float>()));
                     if (dev >= 0 && dev < 64) configured[dev] = true;
                 }
-                if (c->npj_uniform == 18) proj_gather_bulk_kernel<3, 2, 2><<<gg, 256, kGbSmem, c->stream>>>(gp);
+                if (f32) {
+                    if (c->npj_uniform == 18) proj_gather_bulk_kernel<3, 2, 2, float><<<gg, 256, gb_smem<float>(), c->stream>>>(gp);
+                    else if (c->npjp <= 24) proj_gather_bulk_kernel<3, 3, 0, float><<<gg, 256, gb_smem<float>(), c->stream>>>(gp);
+                    else proj_gather_bulk_kernel<4, 4, 0, float><<<gg, 256, gb_smem<float>(), c->stream>>>(gp);
+                }
+                else if (c->npj_uniform == 18) proj_gather_bulk_kernel<3, 2, 2><<<gg, 256, kGbSmem, c->stream>>>(gp);
                 else if (c->npjp <= 24) proj_gather_bulk_kernel<3, 3, 0><<<gg, 256, kGbSmem, c->stream>>>(gp);
                 else proj_gather_bulk_kernel<4, 4, 0><<<gg, 256, kGbSmem, c->stream>>>(gp);
             }
@@ -222,9 +230,20 @@ int enqueue_step(csf_ctx* c, const void* src, long long ld, void* dst, long long
             else { if (f32) proj_gather_kernel<4, float><<<gg, 256, 0, c->stream>>>(gp); else proj_gather_kernel<4, double><<<gg, 256, 0, c->stream>>>(gp); }
         }
         CSF_CUDA(c, cudaGetLastError());
+        c->launches += 1;
+    }
+    return CSF_OK;
+}
+
+// a6: C~ = Delta C, written in the fragment order of the column kernel's DMMA B operand; clear_ct: the padding rows of C~
+// must be zero (once per buffer and layout is enough)
+int enqueue_delta(csf_ctx* c, const double* dC, double* dCt, int nvec, double sc, bool clear_ct = true) {
+    const long long ldc = nvec;
+    const int kind = column_kind(c); const bool ws = kind == 2;
+    {
         DeltaParams dp{};
         const int lanes = column_info(c->p, kind).lanes, nchunks = (nvec + lanes / 4 - 1) / (lanes / 4);
-        CSF_CUDA(c, cudaMemsetAsync(dCt, 0, ctp_bytes(c, nvec), c->stream));
+        if (clear_ct) CSF_CUDA(c, cudaMemsetAsync(dCt, 0, ctp_bytes(c, nvec), c->stream));
         dp.C = reinterpret_cast<const double2*>(dC); dp.Ct = dCt; dp.ldc = ldc; dp.nvec = nvec;
         dp.lanes = lanes; dp.ks = c->npjp / 4; dp.nchunks = nchunks;
         dp.scale = ws ? sc : 1.0;          // the streaming kernel accumulates sc * (P~ C~) straight into its X tile
@@ -233,10 +252,18 @@ int enqueue_step(csf_ctx* c, const void* src, long long ld, void* dst, long long
         dim3 dg(c->natoms, (nvec + 31) / 32);
         { ProfScope ps(c, CSF_KIND_DELTA); delta_apply_kernel<<<dg, 256, 0, c->stream>>>(dp); }
         CSF_CUDA(c, cudaGetLastError());
-        c->launches += 2;
+        c->launches += 1;
     }
+    return CSF_OK;
+}
+
+// a1-a4, a7, a8: dst += sc * i^rot * (H_loc - shift + P~ C~) src; fg != nullptr: the launch also carries the projector
+// gather of another block (wide order-5 FP64 kernel with gather warps, csf_column.cuh col_gather_role)
+int enqueue_column(csf_ctx* c, const void* src, long long ld, void* dst, long long ld_dst, int nvec, double sc, int rot, double shift,
+                   double* dCt, bool f32, const FusedGather* fg) {
+    const int kind = column_kind(c); const bool ws = kind == 2;
     {
-        const ColInfo ci = column_info(c->p, kind);
+        const ColInfo ci = fg ? column_info_wide_p5_g() : column_info(c->p, kind);
         if (ci.smem > c->smem_optin) return fail(c, CSF_EUNSUPPORTED, "column tile does not fit shared memory");
         if (4 * ld >= (1LL << 31) || 4 * ld_dst >= (1LL << 31)) return fail(c, CSF_EUNSUPPORTED, "leading dimension too large");
         const int vpc = ci.lanes / 4;               // spinor vectors per CTA
@@ -294,13 +321,47 @@ int enqueue_step(csf_ctx* c, const void* src, long long ld, void* dst, long long
         long long nblocks = (long long)q.chunk_group * q.ncols * q.nseg * ngroups;
         if (nblocks > 0x7fffffffLL || (long long)q.nchunks * q.ncols * q.nseg > 0x7fffffffLL) return fail(c, CSF_EUNSUPPORTED, "grid too large");
         if (ws) nblocks = std::min<long long>((long long)q.nchunks * q.ncols * q.nseg, c->sm_count);      // persistent CTAs, one per SM
+        if (fg) {
+            // the gather warps' task list: (gather block, chunk of kCgVec vectors) of the OTHER block; its C is cleared here
+            ColGather& g = q.g;
+            g.src = static_cast<const double*>(fg->src); g.ld = fg->ld; g.nvec = fg->nvec;
+            g.gb_atom = c->d_gb_atom.as<int>(); g.gb_beg = c->d_gb_beg.as<int>(); g.gb_end = c->d_gb_end.as<int>(); g.gb_k0 = c->d_gb_k0.as<int>();
+            g.ent_node = c->d_ent_node.as<int>(); g.g_pack = c->d_g_pack.as<double>();
+            g.atom_coff = c->d_atom_coff.as<long long>(); g.atom_npj = c->d_atom_npj.as<int>();
+            g.C = fg->dC; g.ldc = fg->nvec;
+            g.nvc = (fg->nvec + kCgVec - 1) / kCgVec; g.ntasks = fg->dC ? c->n_gather_blocks * g.nvc : 0;
+            if (g.ntasks > 0) CSF_CUDA(c, cudaMemsetAsync(fg->dC, 0, (size_t)c->crows * g.ldc * sizeof(double2), c->stream));
+        }
         {
             ProfScope ps(c, CSF_KIND_CELL);
-            CSF_CUDA(c, launch_column(c->p, c->natoms > 0 ? c->npjp / 4 : 5, kmode, f32, kind, q, nblocks, c->stream));
+            if (fg) CSF_CUDA(c, launch_column_wide_p5_g(c->npjp / 4, kmode, f32, q, nblocks, c->stream));
+            else CSF_CUDA(c, launch_column(c->p, c->natoms > 0 ? c->npjp / 4 : 5, kmode, f32, kind, q, nblocks, c->stream));
         }
         c->launches += 1;
         return CSF_OK;
     }
+}
+
+// one step: dst += sc * i^rot * (Hhat - shift) src
+// src, dst: complex128 blocks, or complex64 blocks when f32 (CSF_FP32_INTERMEDIATE)
+int enqueue_step(csf_ctx* c, const void* src, long long ld, void* dst, long long ld_dst, int nvec, double sc, int rot, double shift,
+                 double* dC, double* dCt, bool f32 = false) {
+    // the sum-factorised kernels hold the Gamma-point operator with real projectors only
+    if (c->kpt_on || c->proj_complex) return fail(c, CSF_ESTATE, "a k-point / complex projectors are set: only the dense path (csf_apply_H_dense, csf_filter_dense) serves them");
+    if (c->natoms > 0) {
+        int rc = enqueue_gather(c, src, ld, nvec, dC, f32); if (rc != CSF_OK) return rc;
+        rc = enqueue_delta(c, dC, dCt, nvec, sc); if (rc != CSF_OK) return rc;
+    }
+    return enqueue_column(c, src, ld, dst, ld_dst, nvec, sc, rot, shift, dCt, f32, nullptr);
+}
+
+// The fused path of csf_filter (complex128, order 5, 8 vectors per CTA, 18 projectors per atom): the block is split into two
+// halves whose column steps alternate, and each column launch computes, in two extra warps, the projector coefficients the
+// OTHER half needs next. CSF_FUSED_GATHER=0 switches it off, =1 takes it for any block of >= 2 vectors (tests).
+bool fused_gather_ok(const csf_ctx* c, int nvec) {
+    if (c->fused_gather == 0 || column_kind(c) != 1 || c->p != 5 || c->natoms == 0 || c->npj_uniform != 18 || c->npjp != 20) return false;
+    if (column_info_wide_p5_g().smem > c->smem_optin) return false;
+    return nvec >= (c->fused_gather == 1 ? 2 : 64);
 }
 
 size_t f32_block_bytes(const csf_ctx* c, int nvec) { return ((size_t)2 * c->M * ((nvec + 1) & ~1) * sizeof(float2) + 255) / 256 * 256; }
@@ -381,6 +442,7 @@ int csf_create(csf_ctx** out, const int ncell[3], const double box[3], int order
     // CSF_LANES pins the column kernel variant for the parity tests (both variants against the oracle on every case)
     if (const char* e = std::getenv("CSF_LANES")) { int v = std::atoi(e); if (v == 16 || v == 32) c->lanes_force = v; }
     if (const char* e = std::getenv("CSF_GATHER")) c->bulk_gather = std::strcmp(e, "reg") != 0;
+    if (const char* e = std::getenv("CSF_FUSED_GATHER")) c->fused_gather = std::atoi(e) != 0 ? 1 : 0;
     if (const char* e = std::getenv("CSF_KERNEL")) c->kernel_force = std::strcmp(e, "ws") == 0 ? 2 : (std::strcmp(e, "wide") == 0 ? 1 : 0);
     const int B = 8;
     // traversal order of the (cx, cy) columns: 8x8 tiles, x fastest inside (neighbouring columns run together, so the
@@ -749,6 +811,39 @@ static int filter_enqueue(csf_ctx* c, const csf_c128* dX, csf_c128* dY, int64_t 
         CSF_CUDA(c, cudaGetLastError()); c->launches += 1;
     }
     rc = enqueue_zero(c, buf1, ld1, nvec); if (rc != CSF_OK) return rc;
+    if (fused_gather_ok(c, nvec)) {
+        // Two half-blocks (the first a multiple of 8 vectors), column steps alternating: K(h, k) = step k on half h. The gather
+        // warps of K(0, k) compute C of (1, k), those of K(1, k) C of (0, k + 1): both sources are complete by then, because
+        // the launches of one stream run in order. Only C of (0, 0) needs the gather kernel.
+        if (c->kpt_on || c->proj_complex) return fail(c, CSF_ESTATE, "a k-point / complex projectors are set: only the dense path (csf_apply_H_dense, csf_filter_dense) serves them");
+        const int nv0 = std::min(nvec - 1, ((nvec + 1) / 2 + 7) / 8 * 8), nvh[2] = {nv0, nvec - nv0}, voff[2] = {0, nv0};
+        double* hC[2] = {dC, dC + (size_t)c->crows * nv0 * 2};
+        double* hCt[2] = {dCt, reinterpret_cast<double*>(reinterpret_cast<char*>(dCt) + ctp_bytes(c, nv0))};
+        auto src_of = [&](int h, int k, long long* lds) -> const double* {
+            if (k == 0) { *lds = ld; return reinterpret_cast<const double*>(dX) + 2 * (size_t)voff[h]; }
+            const bool odd = (k & 1);
+            *lds = odd ? ld1 : ld0; return (odd ? buf1 : buf0) + 2 * (size_t)voff[h];
+        };
+        long long lds = 0;
+        const double* s00 = src_of(0, 0, &lds);
+        rc = enqueue_gather(c, s00, lds, nvh[0], hC[0], false); if (rc != CSF_OK) return rc;
+        rc = enqueue_delta(c, hC[0], hCt[0], nvh[0], 1.0); if (rc != CSF_OK) return rc;
+        for (int k = 0; k < degree; ++k) {
+            const bool odd = (k & 1);
+            double* dstb = (k == 0) ? buf1 : (odd ? buf0 : buf1); const long long ldd = (k == 0) ? ld1 : (odd ? ld0 : ld1);
+            const double sc = (k == 0 ? 1.0 : 2.0) / ee; const int rot = (k == 0) ? ((degree + 3) & 3) : 3;
+            for (int h = 0; h < 2; ++h) {
+                const int hn = 1 - h, kn = (h == 0) ? k : k + 1;         // whose coefficients this launch gathers
+                FusedGather fg{nullptr, 0, nvh[hn], nullptr};
+                if (kn < degree) { long long ldn = 0; fg.src = src_of(hn, kn, &ldn); fg.ld = ldn; fg.dC = hC[hn]; }
+                const double* srcp = src_of(h, k, &lds);
+                rc = enqueue_column(c, srcp, lds, dstb + 2 * (size_t)voff[h], ldd, nvh[h], sc, rot, cc, hCt[h], false, &fg);
+                if (rc != CSF_OK) return rc;
+                if (kn < degree) { rc = enqueue_delta(c, hC[hn], hCt[hn], nvh[hn], 1.0, kn == 0); if (rc != CSF_OK) return rc; }
+            }
+        }
+        return CSF_OK;
+    }
     // W_1 = (i^(m-1)/e)(Hhat - c) X
     rc = enqueue_step(c, reinterpret_cast<const double*>(dX), ld, buf1, ld1, nvec, 1.0 / ee, (degree + 3) & 3, cc, dC, dCt);
     if (rc != CSF_OK) return rc;
@@ -924,6 +1019,12 @@ int csf_column_lanes(const csf_ctx* c, int nvec, int mode, int* lanes) {
     if (!c || !lanes || nvec < 1 || (mode != CSF_FP64 && mode != CSF_FP32_INTERMEDIATE)) return CSF_EINVAL;
     const bool f32 = mode == CSF_FP32_INTERMEDIATE;
     *lanes = column_info(c->p, column_kind(c)).lanes;
+    return CSF_OK;
+}
+
+int csf_filter_fused_gather(const csf_ctx* c, int nvec, int mode, int* fused) {
+    if (!c || !fused || nvec < 1 || (mode != CSF_FP64 && mode != CSF_FP32_INTERMEDIATE)) return CSF_EINVAL;
+    *fused = (mode == CSF_FP64 && !c->kpt_on && !c->proj_complex && fused_gather_ok(c, nvec)) ? 1 : 0;
     return CSF_OK;
 }
 

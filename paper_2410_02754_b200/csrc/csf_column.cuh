@@ -66,6 +66,21 @@ __host__ __device__ constexpr int col_aux_row0(int nodes, int nq, int r) {
     return r * split < nodes ? r * split : nodes;
 }
 
+// Fused projector gather (csf_filter on half-blocks, FP64, order 5, 8 vectors per CTA): two extra warps of the column kernel
+// compute C = P~^T W for ANOTHER block of vectors (the half-block whose column step comes next) while the main warps work on
+// this one. The gather is HBM-bound and the column step latency-bound, so the two share an SM at little cost to either.
+// Tasks = (gather block of <= 256 support rows of one atom) x (chunk of kCgVec vectors), chunk fastest; CTA b takes tasks
+// b, b + gridDim.x, ...
+struct ColGather {
+    const double* src; long long ld; int nvec;                  // complex128 block [2M][ld], nvec live vectors
+    const int* gb_atom; const int* gb_beg; const int* gb_end;   // gather blocks over the entry list (as GatherParams)
+    const int* gb_k0;                                            // first k-step (4 entries) of the block in g_pack
+    const int* ent_node; const double* g_pack;                   // P~^T in A-fragment order [k-step][3][32]
+    const long long* atom_coff; const int* atom_npj;
+    double* C; long long ldc;                                    // [crows][ldc] complex128, cleared by the host, RED-added here
+    int ntasks, nvc;                                             // tasks in all, vector chunks per gather block
+};
+
 struct ColParams {
     // TMA descriptors (cuTensorMapEncodeTiled): src viewed as [nfz][nfy][2 nfx rows][2 nvec doubles], box = the owned
     // nodes of one cell x L/2 doubles per spin row; vb viewed as [nfz][nfy][4 nfx doubles], box = one cell's owned nodes
@@ -93,6 +108,7 @@ struct ColParams {
     const double* Ct;                    // C~ in B-fragment order: [atom][chunk][KS][L/8][32] (DeltaParams)
     int npjp;
     long long* prof;                     // WS_PROF builds of csf_colws.cuh: per (CTA, warp) cycle counters
+    ColGather g;                         // kernels with gather warps (GW > 0) only; ntasks = 0: nothing to gather
 };
 
 __device__ __forceinline__ double col_flip(double x, unsigned mask) {
@@ -123,6 +139,147 @@ __device__ __forceinline__ void col_dmma(double& d0, double& d1, double a, doubl
 __device__ __forceinline__ void col_bar_sync(int id, int count) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(count) : "memory"); }
 __device__ __forceinline__ void col_bar_arrive(int id, int count) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(count) : "memory"); }
 
+// gather warps (fused projector gather): each of the two warps (= spins) runs its own copy pipeline of kCgStages stages. A
+// stage is one k-step: 4 support rows x kCgVec complex128 of the warp's spin (512 bytes each) and the k-step's P~^T fragments
+// (the first 576 bytes of its 768 in g_pack: two DMMA tiles + the rows of projectors 16, 17). Laid out as
+// [row 0][row 2][P~^T][row 1][row 3], the rows k = 0..3 of a B fragment sit on two bank halves (576 = 64 mod 128).
+// Measured on the way here (config 3, cycles of a gather warp per k-step, 288 of them FP64-pipe time):
+//  * the whole staging area must stay under ~16.7 KB: with more, the CTA no longer fits the 196 KB shared-memory
+//    configuration, and the 228 KB one leaves the column step too little L1 (idle gather warps: 1617 against 1528 ms per block);
+//  * P~^T fragments loaded into registers one k-step ahead arrive late, and so does a support row's node index loaded right
+//    before its copy (the warp issues in order): fragments go through the pipeline, indices are fetched 32 rows at a time;
+//  * cp.async.bulk costs the issuing warp ~500 cycles per k-step whatever the number of requests (1 x 4 lanes, 3 x 1 lane and
+//    4 + 1 lanes all measured 530-640); plain 16-byte cp.async (LDGSTS, lane = 16-byte piece of a row) issues in ~400 and
+//    makes a task 25 % shorter, but loads the LSU that the main warps depend on: 1853 against 1818 ms per block. Bulk copies stay.
+#ifndef CSF_CG_STAGES
+#define CSF_CG_STAGES 3
+#endif
+constexpr int kCgStages = CSF_CG_STAGES, kCgVec = 32;
+constexpr int kCgRowBytes = kCgVec * 16;                                          // one spin of one support row
+constexpr int kCgABytes = 2 * 256 + 64;                                           // P~^T of one k-step as far as it is read
+constexpr int kCgStageBytes = 4 * kCgRowBytes + kCgABytes;
+constexpr int kCgWarpBytes = kCgStages * kCgStageBytes;
+constexpr size_t kCgBytes = (size_t)2 * kCgWarpBytes + 2 * kCgStages * 8;        // two warps + their full[s] mbarriers
+__host__ __device__ constexpr int col_cg_row(int k) { return (k >> 1) * kCgRowBytes + ((k & 1) ? 2 * kCgRowBytes + kCgABytes : 0); }
+constexpr int kCgAOff = 2 * kCgRowBytes;
+
+// ---------------------------------------------------------------------------------------------------------------
+// Gather role (a5 inside the column kernel): C[atom][2 chi + s][v] += sum_I P~_{I chi} src[(2I+s)][v] (eq.84 inner
+// sum) for the task list of this CTA. Two warps = the two spins, each with its own pipeline; a warp holds 8 n-tiles of 4
+// vectors. Support rows and P~^T fragments are staged in shared memory by cp.async.bulk (lanes 0-3 copy a row each, lane 4 the
+// fragments, all completing on the stage's mbarrier), projectors 0-15 go through DMMA m8n8k4 tiles (A = P~^T 8 x 4 in
+// fragment order, B = src 4 rows x 8 real lanes), 16 and 17 by plain FMAs — the arithmetic of
+// proj_gather_bulk_kernel<3, 2, 2> (csf_kernels.cuh), which serves 18 projectors per atom.
+// ---------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void col_gather_role(const ColGather& G, unsigned char* gsm, int gw, int wl) {
+    constexpr int MT = 3, MD = 2, NX = 2, NTG = kCgVec / 4;
+    unsigned char* const wsm = gsm + (size_t)gw * kCgWarpBytes;
+    const unsigned wsm_u = (unsigned)__cvta_generic_to_shared(wsm);
+    const unsigned mb0 = (unsigned)__cvta_generic_to_shared(gsm + (size_t)2 * kCgWarpBytes) + gw * (kCgStages * 8);      // full[s] of this warp
+    const int kk = wl & 3, rw = wl >> 2, spin = gw;
+    if (wl == 0) {
+#pragma unroll
+        for (int s = 0; s < kCgStages; ++s) asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(mb0 + 8 * s));
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncwarp();
+    int gbase = 0;                  // k-steps staged so far by this warp: stage and mbarrier phase continue across tasks
+    for (int task = blockIdx.x; task < G.ntasks; task += gridDim.x) {
+        const int gb = task / G.nvc, vc0 = (task % G.nvc) * kCgVec;
+        const int nv = min(kCgVec, G.nvec - vc0);
+        const int atom = __ldg(G.gb_atom + gb), e0 = __ldg(G.gb_beg + gb), e1 = __ldg(G.gb_end + gb);
+        const int nks = (e1 - e0 + 3) / 4;
+        const char* const srcb = reinterpret_cast<const char*>(G.src) + ((long long)spin * G.ld + vc0) * 16;
+        const char* const gpb = reinterpret_cast<const char*>(G.g_pack + (long long)__ldg(G.gb_k0 + gb) * (MT * 32));
+        // node indices of the support rows, 8 k-steps (32 rows) per coalesced load, two batches in registers: a copy must
+        // not wait for its row's index (the warp issues in order, and one round trip to L2 per k-step is what bounds it then)
+        auto load_idx = [&](int b) { const int e = e0 + 32 * b + wl; return e < e1 ? __ldg(G.ent_node + e) : 0; };
+        int idx0 = load_idx(0), idx1 = load_idx(1);
+        // stage k-step g of this task (called with g = 0, 1, 2, ... in order): lane k < 4 copies support row k (this warp's
+        // spin), lane 4 the P~^T fragments; the warp has finished reading the stage (program order + the warp-wide shuffle)
+        auto issue = [&](int g) {
+            const int s = (gbase + g) % kCgStages;
+            const int eg = e0 + 4 * g, rows_g = min(4, e1 - eg);
+            const unsigned sbase = wsm_u + (unsigned)(s * kCgStageBytes);
+            const int bt = g >> 3;
+            if ((g & 7) == 0 && g > 0) { if (bt & 1) idx0 = load_idx(bt + 1); else idx1 = load_idx(bt + 1); }      // batch bt - 1 is used up
+            const long long node = __shfl_sync(0xffffffffu, (bt & 1) ? idx1 : idx0, (g & 7) * 4 + (wl & 3));
+            if (wl == 0) asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mb0 + 8 * s), "r"((unsigned)(rows_g * nv * 16 + kCgABytes)) : "memory");
+            __syncwarp();
+            if (wl < rows_g) {
+                asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                             ::"r"(sbase + (unsigned)col_cg_row(wl)), "l"(srcb + 2 * node * G.ld * 16), "r"((unsigned)(nv * 16)), "r"(mb0 + 8 * s) : "memory");
+            } else if (wl == 4) {
+                asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                             ::"r"(sbase + (unsigned)kCgAOff), "l"(gpb + (long long)g * (MT * 256)), "r"((unsigned)kCgABytes), "r"(mb0 + 8 * s) : "memory");
+            }
+        };
+        for (int g = 0; g < kCgStages && g < nks; ++g) issue(g);
+        double acc[MD][NTG][2], accx[NX][NTG];
+#pragma unroll
+        for (int m = 0; m < MD; ++m)
+#pragma unroll
+            for (int nt = 0; nt < NTG; ++nt) { acc[m][nt][0] = 0.0; acc[m][nt][1] = 0.0; }
+#pragma unroll
+        for (int x = 0; x < NX; ++x)
+#pragma unroll
+            for (int nt = 0; nt < NTG; ++nt) accx[x][nt] = 0.0;
+        for (int g = 0; g < nks; ++g) {
+            {
+                const int gi = gbase + g; unsigned done = 0;
+                while (!done) asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }" : "=r"(done) : "r"(mb0 + 8 * (gi % kCgStages)), "r"((unsigned)((gi / kCgStages) & 1)) : "memory");
+            }
+            const unsigned char* st = wsm + ((gbase + g) % kCgStages) * kCgStageBytes;
+            const bool ok = e0 + 4 * g + kk < e1;               // rows past the block's end were not copied: stale data
+            const double* sb = reinterpret_cast<const double*>(st + col_cg_row(kk)) + rw;
+            const double* sa = reinterpret_cast<const double*>(st + kCgAOff);
+            double a[MD + NX], b[NTG];
+#pragma unroll
+            for (int m = 0; m < MD; ++m) a[m] = sa[m * 32 + wl];
+#pragma unroll
+            for (int x = 0; x < NX; ++x) a[MD + x] = sa[MD * 32 + x * 4 + kk];
+#pragma unroll
+            for (int nt = 0; nt < NTG; ++nt) b[nt] = (ok && nt * 4 + (rw >> 1) < nv) ? sb[nt * 8] : 0.0;
+#pragma unroll
+            for (int m = 0; m < MD; ++m)
+#pragma unroll
+                for (int nt = 0; nt < NTG; ++nt) col_dmma(acc[m][nt][0], acc[m][nt][1], a[m], b[nt]);
+#pragma unroll
+            for (int x = 0; x < NX; ++x)
+#pragma unroll
+                for (int nt = 0; nt < NTG; ++nt) accx[x][nt] = fma(a[MD + x], b[nt], accx[x][nt]);
+            if (g + kCgStages < nks) issue(g + kCgStages);
+        }
+        gbase += nks;
+        const long long coff = __ldg(G.atom_coff + atom);
+        const int npj = __ldg(G.atom_npj + atom);
+        // extra projectors: sum the four support rows of a k-step (lanes kk = 0..3), lane kk = 0 adds real lane rw of its vector
+#pragma unroll
+        for (int x = 0; x < NX; ++x)
+#pragma unroll
+            for (int nt = 0; nt < NTG; ++nt) {
+                double v = accx[x][nt];
+                v += __shfl_xor_sync(0xffffffffu, v, 1); v += __shfl_xor_sync(0xffffffffu, v, 2);
+                const int vv = vc0 + nt * 4 + (rw >> 1);
+                if (kk == 0 && 8 * MD + x < npj && vv < G.nvec) col_red(G.C + ((coff + 2 * (8 * MD + x) + spin) * G.ldc + vv) * 2 + (rw & 1), v);
+            }
+#pragma unroll
+        for (int m = 0; m < MD; ++m) {
+            const int chi = m * 8 + rw;
+            if (chi < npj) {
+#pragma unroll
+                for (int nt = 0; nt < NTG; ++nt) {
+                    const int v = vc0 + nt * 4 + kk;
+                    if (v < G.nvec) {
+                        double* cp = G.C + ((coff + 2 * chi + spin) * G.ldc + v) * 2;
+                        col_red(cp, acc[m][nt][0]); col_red(cp + 1, acc[m][nt][1]);
+                    }
+                }
+            }
+        }
+    }
+}
+
 // canonical representative of (i, j) under transposition and the centro flip (i, j) -> (N-1-i, N-1-j)
 template <int N> __host__ __device__ constexpr int col_canon(int i, int j) {
     int best = i * kColTab + j, c = j * kColTab + i;
@@ -150,11 +307,12 @@ __host__ __device__ constexpr int col_maxreg(int p, bool f32, int lanes, int aux
     return f32 ? (p == 4 ? 96 : 128) : (p == 4 ? 128 : 168);
 }
 
-template <typename T, int P, int L, int AUXW = 2> struct ColCfg {
+template <typename T, int P, int L, int AUXW = 2, int GW = 0> struct ColCfg {
     static constexpr int N = P + 1;
     static constexpr int NTM = (N * L + 31) / 32 * 32;               // main threads
     static constexpr int NAUX = 32 * AUXW;                           // auxiliary (expansion) threads
-    static constexpr int NT = NTM + NAUX;                            // threads per CTA
+    static constexpr int NTB = NTM + NAUX;                           // threads of the column step (named-barrier counts)
+    static constexpr int NT = NTB + 32 * GW;                         // threads per CTA (+ gather warps, highest warp ids)
     static constexpr int PLANE = N * N * L;                          // reals per ring plane and field
     static constexpr int EPLANE = P * P * L;
     static constexpr int VCELL = P * P * P * 4;                      // V, Bx, By, Bz of the owned nodes of one cell
@@ -164,14 +322,15 @@ template <typename T, int P, int L, int AUXW = 2> struct ColCfg {
     static constexpr size_t VBYTES = ((size_t)VCELL * sizeof(double) + 127) / 128 * 128;          // one potential stage
     static constexpr size_t VOFF = XOFF + kColXBuf * XBYTES;          // X and the stage are multi-buffered (cell t uses t % kColXBuf)
     static constexpr size_t MOFF = VOFF + kColXBuf * VBYTES;
-    static constexpr size_t SMEM = MOFF + 32;
+    static constexpr size_t GOFF = (MOFF + 32 + 127) / 128 * 128;    // gather stages (GW > 0)
+    static constexpr size_t SMEM = GW > 0 ? GOFF + kCgBytes : MOFF + 32;
 };
 
 // MODE 2: every node of the mesh is unconstrained (all directions periodic), nvec is a multiple of L/4 and the cells
 // are cubes (rho_y = rho_z = 1), so no load, store or RED needs a predicate and no rho multiply is issued.
-template <typename T, int P, int KS, int MODE, int L, int AUXW = col_aux_warps(P, sizeof(T) == 4, MODE, L)>
-__global__ void __launch_bounds__(ColCfg<T, P, L, AUXW>::NT) __maxnreg__(col_maxreg(P, sizeof(T) == 4, L, AUXW)) column_kernel(const __grid_constant__ ColParams A) {
-    using Cfg = ColCfg<T, P, L, AUXW>;
+template <typename T, int P, int KS, int MODE, int L, int AUXW = col_aux_warps(P, sizeof(T) == 4, MODE, L), int GW = 0>
+__global__ void __launch_bounds__(ColCfg<T, P, L, AUXW, GW>::NT) __maxnreg__(col_maxreg(P, sizeof(T) == 4, L, AUXW)) column_kernel(const __grid_constant__ ColParams A) {
+    using Cfg = ColCfg<T, P, L, AUXW, GW>;
     constexpr int kColAuxWarps = AUXW, kColAux = Cfg::NAUX;
     constexpr bool kMainTma = col_main_tma(P, L), kPot2 = P >= 5;
     using T2 = typename ColVec2<T>::type;
@@ -200,12 +359,21 @@ __global__ void __launch_bounds__(ColCfg<T, P, L, AUXW>::NT) __maxnreg__(col_max
     const int cidx = r % A.ncols; r /= A.ncols;
     const int seg = r % A.nseg; r /= A.nseg;
     const int chunk = r * A.chunk_group + cg;
-    if (chunk >= A.nchunks) return;
+    const bool live = chunk < A.nchunks;
+    if constexpr (GW == 0) { if (!live) return; }
+    else {
+        // gather warps (the LOWEST warp ids: the scheduler favours high ids, which belong to the main warps; with 4 expansion
+        // warps next, warps 0, 1 land on the SM sub-partitions that carry one main warp) work on their own task list, also in
+        // a CTA that has no column work
+        const int gwarp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
+        if (gwarp < GW) { col_gather_role(A.g, smem + Cfg::GOFF, gwarp, (int)(threadIdx.x & 31)); return; }
+        if (!live) return;
+    }
     const int col = A.col_order[cidx];
     const int cx = col % A.ncx, cy = col / A.ncx;
     const int cz0 = seg * A.seg_len;
     const int S = min(A.seg_len, A.ncz - cz0);
-    const int tid = threadIdx.x;
+    const int tid = (int)threadIdx.x - 32 * GW;          // thread index among the threads of the column step
     const int plane_nodes = A.nfx * A.nfy;
 
     if (tid == 0) {
@@ -213,7 +381,7 @@ __global__ void __launch_bounds__(ColCfg<T, P, L, AUXW>::NT) __maxnreg__(col_max
         for (int b = 0; b < kColXBuf; ++b) asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(mbar0 + 8 * b));
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    __syncthreads();
+    if constexpr (GW == 0) __syncthreads(); else col_bar_sync(0, Cfg::NTB);
 
     // warp-uniform role (broadcast from lane 0 so that the compiler knows the branch does not split a warp)
     const int warp_id = __shfl_sync(0xffffffffu, tid >> 5, 0);
@@ -249,7 +417,7 @@ __global__ void __launch_bounds__(ColCfg<T, P, L, AUXW>::NT) __maxnreg__(col_max
                 if (sp0 < sp1) { ds = __ldg(A.sub_desc + sp0); load_b(ds, b); }
             }
             if constexpr (!kMainTma) {
-                if (t >= kColXBuf) col_bar_sync(4 + xb, Cfg::NT);    // phase B(t - kColXBuf) has consumed this X buffer
+                if (t >= kColXBuf) col_bar_sync(4 + xb, Cfg::NTB);    // phase B(t - kColXBuf) has consumed this X buffer
                 if (aw == 0 && wl == 0) {
                     const int bx0 = cx * P - (A.bcx == 0 ? 0 : 1), by0 = cy * P - (A.bcy == 0 ? 0 : 1), bz0 = (cz0 + t) * P - (A.bcz == 0 ? 0 : 1);
                     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
@@ -346,7 +514,7 @@ __global__ void __launch_bounds__(ColCfg<T, P, L, AUXW>::NT) __maxnreg__(col_max
                 }
             }
             __threadfence_block();
-            col_bar_arrive(2 + xb, Cfg::NT);                     // X(t) is complete
+            col_bar_arrive(2 + xb, Cfg::NTB);                     // X(t) is complete
         }
         return;
     }
@@ -480,7 +648,7 @@ __global__ void __launch_bounds__(ColCfg<T, P, L, AUXW>::NT) __maxnreg__(col_max
         }
         if (t + 1 < S) load_plane(plane_of(t + 1));          // in flight during phase B
         col_bar_sync(1, NTM);                                 // ring written
-        col_bar_sync(2 + t % kColXBuf, Cfg::NT);              // X(t) complete
+        col_bar_sync(2 + t % kColXBuf, Cfg::NTB);              // X(t) complete
         const T* X = reinterpret_cast<const T*>(xbase + (t % kColXBuf) * Cfg::XBYTES);
         // ------------------------------------------------------------------ phase B
         if (q_on) {
@@ -533,7 +701,7 @@ __global__ void __launch_bounds__(ColCfg<T, P, L, AUXW>::NT) __maxnreg__(col_max
             }
         }
         if constexpr (!kMainTma)
-            if (t + kColXBuf < S) col_bar_arrive(4 + t % kColXBuf, Cfg::NT);   // this X buffer is free
+            if (t + kColXBuf < S) col_bar_arrive(4 + t % kColXBuf, Cfg::NTB);   // this X buffer is free
         col_bar_sync(1, NTM);                                 // ring and X(t) free
         if constexpr (kMainTma)
             if (mtid == 0 && t + kColXBuf < S) issue_tma(t + kColXBuf);

@@ -19,6 +19,9 @@ CSF_DECL_COL(1) CSF_DECL_COL(2) CSF_DECL_COL(3) CSF_DECL_COL(4) CSF_DECL_COL(5) 
     ColInfo column_info_wide_p##P();
 CSF_DECL_COLWIDE(4) CSF_DECL_COLWIDE(5)
 #undef CSF_DECL_COLWIDE
+// wide kernel of order 5 with two gather warps (fused projector gather of another block, ColParams::g; FP64, KS = 5)
+cudaError_t launch_column_wide_p5_g(int ks, int mode, bool f32, const ColParams& cp, long long nblocks, cudaStream_t s);
+ColInfo column_info_wide_p5_g();
 // warp-specialised kernel (csf_colws.cuh: 8 vectors per CTA, persistent CTAs), orders 4 and 5
 #define CSF_DECL_COLW(P) \
     cudaError_t launch_column_ws_p##P(int ks, int mode, bool f32, const ColParams& cp, int nctas, cudaStream_t s); \

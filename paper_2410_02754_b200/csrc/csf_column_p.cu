@@ -22,12 +22,18 @@ constexpr int kLanes = CSF_P <= 6 ? 16 : 8;      // order 7 does not fit shared 
 #define CSF_FN(name) CSF_CAT(CSF_CAT(name, _p), CSF_P)
 #endif
 
+#ifdef CSF_GATHERW
+constexpr int kGatherWarps = CSF_GATHERW;        // translation unit of the kernels with gather warps (FP64, KS = 5 only)
+#else
+constexpr int kGatherWarps = 0;
+#endif
+
 template <typename T, int KS, int MODE>
 cudaError_t launch_t(const ColParams& cp, long long nblocks, cudaStream_t s) {
     // the opt-in to > 48 KB of dynamic shared memory belongs to the device's context: remember it per device
     static bool configured[64] = {};
-    auto kern = column_kernel<T, CSF_P, KS, MODE, kLanes>;
-    using Cfg = ColCfg<T, CSF_P, kLanes, col_aux_warps(CSF_P, sizeof(T) == 4, MODE, kLanes)>;
+    auto kern = column_kernel<T, CSF_P, KS, MODE, kLanes, col_aux_warps(CSF_P, sizeof(T) == 4, MODE, kLanes), kGatherWarps>;
+    using Cfg = ColCfg<T, CSF_P, kLanes, col_aux_warps(CSF_P, sizeof(T) == 4, MODE, kLanes), kGatherWarps>;
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return e;
@@ -49,10 +55,20 @@ cudaError_t launch_real(int ks, int mode, const ColParams& cp, long long nblocks
 }
 }  // namespace
 
+#ifdef CSF_GATHERW
+// column step + fused projector gather of another block (ColParams::g): complex128 blocks, 18 projectors per atom (KS = 5)
+cudaError_t CSF_CAT(CSF_FN(launch_column), _g)(int ks, int mode, bool f32, const ColParams& cp, long long nblocks, cudaStream_t s) {
+    if (f32 || ks != 5) return cudaErrorInvalidValue;
+    return mode == 2 ? launch_t<double, 5, 2>(cp, nblocks, s) : mode == 1 ? launch_t<double, 5, 1>(cp, nblocks, s) : launch_t<double, 5, 0>(cp, nblocks, s);
+}
+
+ColInfo CSF_CAT(CSF_FN(column_info), _g)() { return ColInfo{kLanes, ColCfg<double, CSF_P, kLanes, col_aux_warps(CSF_P, false, 2, kLanes), kGatherWarps>::SMEM}; }
+#else
 cudaError_t CSF_FN(launch_column)(int ks, int mode, bool f32, const ColParams& cp, long long nblocks, cudaStream_t s) {
     return f32 ? launch_real<float>(ks, mode, cp, nblocks, s) : launch_real<double>(ks, mode, cp, nblocks, s);
 }
 
 ColInfo CSF_FN(column_info)() { return ColInfo{kLanes, ColCfg<double, CSF_P, kLanes>::SMEM}; }
+#endif
 
 }  // namespace csf

@@ -149,13 +149,21 @@ __global__ void __launch_bounds__(256, 2) proj_gather_kernel(const __grid_consta
 // ---------------------------------------------------------------------------------------------------
 constexpr int kGbRows = 16;                       // support rows per stage (4 k-steps)
 constexpr int kGbStages = 3;
-constexpr int kGbRowBytes = 2 * 1024 + 64;        // both spins x 64 vectors x 16 B, + 64 B of skew
-constexpr size_t kGbSmem = (size_t)kGbStages * kGbRows * kGbRowBytes + 64;
+// bytes of a staged row: both spins x 64 vectors of complex<T>, + a skew that spreads the four rows of a B fragment over the
+// banks (complex128: 64 bytes = two bank halves of 64-byte pieces; complex64: 32 bytes = four quarters of 32-byte pieces)
+template <typename T> __host__ __device__ constexpr int gb_row_bytes() { return 2 * 64 * 2 * (int)sizeof(T) + (sizeof(T) == 8 ? 64 : 32); }
+template <typename T> __host__ __device__ constexpr size_t gb_smem() { return (size_t)kGbStages * kGbRows * gb_row_bytes<T>() + 64; }
+constexpr int kGbRowBytes = gb_row_bytes<double>();
+constexpr size_t kGbSmem = gb_smem<double>();
 
-template <int MT, int MD, int NX>
+// T = real type of the block (double: complex128 rows; float: the complex64 blocks of CSF_FP32_INTERMEDIATE, converted when
+// the B fragments are read; the accumulation stays FP64). Complex64 rows are copied up to an even vector count (the blocks
+// have an even leading dimension, so the pad column exists; its values never reach a fragment).
+template <int MT, int MD, int NX, typename T = double>
 __global__ void __launch_bounds__(256, 2) proj_gather_bulk_kernel(const __grid_constant__ GatherParams A) {
+    constexpr int RB = gb_row_bytes<T>(), SPB = 64 * 2 * (int)sizeof(T), EB = 2 * (int)sizeof(T);      // row, spin half, complex element
     extern __shared__ __align__(128) unsigned char gsm[];
-    const unsigned mb0 = (unsigned)__cvta_generic_to_shared(gsm + (size_t)kGbStages * kGbRows * kGbRowBytes);      // full[s], empty[s]
+    const unsigned mb0 = (unsigned)__cvta_generic_to_shared(gsm + (size_t)kGbStages * kGbRows * RB);      // full[s], empty[s]
     const int tid = threadIdx.x, wl = tid & 31, warp = tid >> 5;
     const int kk = wl & 3, rw = wl >> 2;
     const int spin = warp & 1;
@@ -182,14 +190,15 @@ __global__ void __launch_bounds__(256, 2) proj_gather_bulk_kernel(const __grid_c
             unsigned done = 0;
             while (!done) asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }" : "=r"(done) : "r"(mb0 + 8 * (kGbStages + s)), "r"((unsigned)((g / kGbStages - 1) & 1)) : "memory");
         }
-        if (wl == 0) asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mb0 + 8 * s), "r"((unsigned)(rows_g * 2 * nv * 16)) : "memory");
+        const int cpb = ((nv * EB + 15) / 16) * 16;                     // bytes per (row, spin) copy
+        if (wl == 0) asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mb0 + 8 * s), "r"((unsigned)(rows_g * 2 * cpb)) : "memory");
         __syncwarp();
         const int row = wl >> 1, sp = wl & 1;
         if (row < rows_g) {
             const long long node = __ldg(A.ent_node + eg + row);
-            const char* src = static_cast<const char*>(A.src) + ((2 * node + sp) * A.ld + vc0) * 16;
-            const unsigned dst = (unsigned)__cvta_generic_to_shared(gsm + ((size_t)s * kGbRows + row) * kGbRowBytes + sp * 1024);
-            asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst), "l"(src), "r"((unsigned)(nv * 16)), "r"(mb0 + 8 * s) : "memory");
+            const char* src = static_cast<const char*>(A.src) + ((2 * node + sp) * A.ld + vc0) * EB;
+            const unsigned dst = (unsigned)__cvta_generic_to_shared(gsm + ((size_t)s * kGbRows + row) * RB + sp * SPB);
+            asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst), "l"(src), "r"((unsigned)cpb), "r"(mb0 + 8 * s) : "memory");
         }
     };
     if (warp == 0)
@@ -223,14 +232,14 @@ __global__ void __launch_bounds__(256, 2) proj_gather_bulk_kernel(const __grid_c
             unsigned done = 0;
             while (!done) asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }" : "=r"(done) : "r"(mb0 + 8 * s), "r"((unsigned)((g / kGbStages) & 1)) : "memory");
         }
-        const double* sb = reinterpret_cast<const double*>(gsm + (size_t)s * kGbRows * kGbRowBytes + spin * 1024) + (vloc + (rw >> 1)) * 2 + (rw & 1);
+        const T* sb = reinterpret_cast<const T*>(gsm + (size_t)s * kGbRows * RB + spin * SPB) + (vloc + (rw >> 1)) * 2 + (rw & 1);
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
             const bool ok = eg + 4 * q + kk < e1;
             double b[kGatherNT];
 #pragma unroll
             for (int nt = 0; nt < kGatherNT; ++nt)
-                b[nt] = (ok && vloc + nt * 4 + (rw >> 1) < nv) ? sb[(size_t)(4 * q + kk) * (kGbRowBytes / 8) + nt * 8] : 0.0;
+                b[nt] = (ok && vloc + nt * 4 + (rw >> 1) < nv) ? (double)sb[(size_t)(4 * q + kk) * (RB / (int)sizeof(T)) + nt * 8] : 0.0;
 #pragma unroll
             for (int m = 0; m < MD; ++m)
 #pragma unroll

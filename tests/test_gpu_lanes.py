@@ -1,5 +1,6 @@
 """Every column-kernel variant against the oracle: the cell-per-iteration kernel with 4 vectors per CTA (16 lanes) and with 8
-(32 lanes, orders 4 and 5), and the warp-specialised streaming kernel (csf_colws.cuh, orders 4 and 5, 32 lanes). By default
+(32 lanes, orders 4 and 5), the warp-specialised streaming kernel (csf_colws.cuh, orders 4 and 5, 32 lanes) and the fused
+half-block path of csf_filter (order 5: column kernel with gather warps; CSF_FUSED_GATHER=1 forces it at small sizes). By default
 libcsf picks the variant; CSF_LANES / CSF_KERNEL pin it at csf_create, so every case below runs
 through each kernel."""
 import numpy as np
@@ -12,11 +13,16 @@ from test_gpu_parity import TOL, TOL32, _cfg, gpu_filter32
 pytestmark = pytest.mark.gpu
 
 
-@pytest.fixture(params=[16, 32, "ws"])
+@pytest.fixture(params=[16, 32, "ws", "fused"])
 def lanes(request, monkeypatch):
-    """16: 4 vectors per CTA; 32: 8 vectors per CTA (cell-per-iteration kernel); "ws": the warp-specialised streaming kernel."""
+    """16: 4 vectors per CTA; 32: 8 vectors per CTA (cell-per-iteration kernel); "ws": the warp-specialised streaming kernel;
+    "fused": csf_filter's half-block path (order 5, complex128: the column kernel with two gather warps that compute the
+    projector coefficients of the other half-block) forced for every block size, which the policy takes from 64 vectors on."""
     if request.param == "ws":
         monkeypatch.setenv("CSF_KERNEL", "ws")
+    elif request.param == "fused":
+        monkeypatch.setenv("CSF_LANES", "32")
+        monkeypatch.setenv("CSF_FUSED_GATHER", "1")
     else:
         monkeypatch.setenv("CSF_LANES", str(request.param))
     return request.param
@@ -110,3 +116,47 @@ def test_column_lanes_query(monkeypatch):
     monkeypatch.delenv("CSF_LANES")
     monkeypatch.setenv("CSF_KERNEL", "ws")
     assert binding.Csf((2, 2, 2), (4.0, 4.0, 4.0), 4, (0, 0, 0)).column_lanes(16, binding.CSF_FP64) == 32
+
+
+def test_fused_gather_policy_and_agreement(monkeypatch):
+    """csf_filter_fused_gather reports the path a block takes (policy: complex128, order 5, 18 projectors per atom, >= 64
+    vectors; CSF_FUSED_GATHER pins it), and the fused and the unfused path give the oracle's result on the same block — a
+    block wide enough for the policy to choose the fused path by itself, split 40 + 27 (ragged second half)."""
+    from paper_2410_02754_b200 import binding
+    for v in ("CSF_LANES", "CSF_KERNEL", "CSF_FUSED_GATHER"):
+        monkeypatch.delenv(v, raising=False)
+    cfg = synth.scaled_config(synth.CONFIGS[3], (4, 4, 4), 2, nvec=67, degree=7)
+    ref, gpu, s = setup_pair(cfg)
+    assert gpu.filter_fused_gather(67, binding.CSF_FP64) and gpu.filter_fused_gather(64, binding.CSF_FP64)
+    assert not gpu.filter_fused_gather(63, binding.CSF_FP64) and not gpu.filter_fused_gather(67, binding.CSF_FP32_INTERMEDIATE)
+    a, b, _, _ = bounds.lanczos_bounds(lambda v: ref.apply_H(v), 2 * ref.M)
+    X = synth.random_block(s.rng, 2 * ref.M, 67)
+    Yref = ref.filter(X, 7, a, b)
+    Yf = gpu_filter(gpu, X, 7, a, b, ld=70)
+    assert_block_close(Yf, Yref, TOL)
+    monkeypatch.setenv("CSF_FUSED_GATHER", "0")
+    ref2, gpu2, _ = setup_pair(cfg)
+    assert not gpu2.filter_fused_gather(67, binding.CSF_FP64)
+    Yu = gpu_filter(gpu2, X, 7, a, b, ld=70)
+    assert_block_close(Yu, Yref, TOL)
+    assert rel_fro(Yf, Yu) < 1e-13
+    monkeypatch.setenv("CSF_FUSED_GATHER", "1")
+    p4 = binding.Csf((2, 2, 2), (4.0, 4.0, 4.0), 4, (0, 0, 0))
+    assert not p4.filter_fused_gather(256, binding.CSF_FP64)          # order 4 has no kernel with gather warps
+
+
+@pytest.mark.parametrize("gather", ["reg", "bulk"])
+@pytest.mark.parametrize("base,ncell,natoms,nvec,degree", [(2, (4, 4, 8), 3, 24, 6), (4, (6, 6, 6), 4, 13, 8)])
+def test_both_projector_gather_kernels(monkeypatch, gather, base, ncell, natoms, nvec, degree):
+    """The projector gather (a5) has two kernels: src rows staged in shared memory by bulk copies (the default for complex128
+    and complex64 blocks alike) and plain register loads (CSF_GATHER=reg pins it). Both against the oracle, both precision
+    modes, full and ragged blocks (13 vectors: the complex64 rows are copied up to the even pad column)."""
+    monkeypatch.setenv("CSF_GATHER", gather)
+    cfg = synth.scaled_config(synth.CONFIGS[base], ncell, natoms, nvec=nvec, degree=degree)
+    ref, gpu, s = setup_pair(cfg)
+    a, b, _, _ = bounds.lanczos_bounds(lambda v: ref.apply_H(v), 2 * ref.M)
+    X = synth.random_block(s.rng, 2 * ref.M, nvec)
+    Yref = ref.filter(X, degree, a, b)
+    assert_block_close(gpu_filter(gpu, X, degree, a, b), Yref, TOL)
+    assert_block_close(gpu_filter32(gpu, X, degree, a, b), Yref, TOL32)
+    assert_block_close(gpu_apply_H(gpu, X, ld=nvec + 3), ref.apply_H(X), TOL)

@@ -74,12 +74,14 @@ def test_single_cell_periodic_directions():
     assert_block_close(gpu_apply_H(gpu, X), ref.apply_H(X), TOL)
 
 
-def test_generic_projector_counts():
-    """Atoms with different numbers of projectors take the generic (non-18) code path."""
+@pytest.mark.parametrize("counts", [(5, 1, 7), (26, 3, 30)])
+def test_generic_projector_counts(counts):
+    """Atoms with different numbers of projectors take the generic (non-18) code paths: up to 24 projectors (three tensor
+    tiles per k-step) and up to 32 (four), in the gather, Delta and expansion kernels, both precision modes."""
     cfg = _cfg((3, 3, 3), (4.0, 4.0, 4.0), 3, (0, 0, 0), 0, nvec=6)
     ref, gpu, s = setup_pair(cfg, with_projectors=False)
     rng = np.random.default_rng(4); M = ref.M
-    nproj = np.array([5, 1, 7], dtype=np.int32); node_ptr = [0]; idx = []; pv = []; dl = []; dptr = [0]
+    nproj = np.array(counts, dtype=np.int32); node_ptr = [0]; idx = []; pv = []; dl = []; dptr = [0]
     for a, npj in enumerate(nproj):
         sel = np.sort(rng.choice(M, 60 + 10 * a, replace=False)); idx.append(sel); node_ptr.append(node_ptr[-1] + len(sel))
         pv.append(rng.normal(size=(len(sel), npj)).reshape(-1))
@@ -88,6 +90,10 @@ def test_generic_projector_counts():
     ref.set_projectors(*args); gpu.set_projectors(*args)
     X = synth.random_block(s.rng, 2 * M, cfg.nvec)
     assert_block_close(gpu_apply_H(gpu, X), ref.apply_H(X), TOL)
+    a, b, _, _ = bounds.lanczos_bounds(lambda v: ref.apply_H(v), 2 * M)
+    Yref = ref.filter(X[:, :5], 5, a, b)
+    assert_block_close(gpu_filter(gpu, X[:, :5], 5, a, b, ld=6), Yref, TOL)
+    assert_block_close(gpu_filter32(gpu, X[:, :5], 5, a, b, ld=6), Yref, TOL32)
 
 
 @pytest.mark.parametrize("degree", [0, 1, 2, 3, 8, 9])
