@@ -884,7 +884,19 @@ int csf_filter_host(csf_ctx* c, const csf_c128* hX, csf_c128* hY, int64_t ld, in
     if (nvec == 0) return CSF_OK;
     CSF_CUDA(c, cudaSetDevice(c->device));
     const int chunk = std::min(c->host_chunk, nvec);
-    const int nch = (nvec + chunk - 1) / chunk;
+    // Column chunks. What the pipeline cannot hide is the host->device copy of the first chunk and the device->host copy of the
+    // last one, so a block of at least three chunks starts with chunks of 1/4 and 3/4 the size (the first a multiple of 8
+    // columns) and ends with the same two in reverse: the copy of the second chunk still fits under the filter of the first.
+    std::vector<int> csz;
+    {
+        const int q4 = std::max(8, chunk / 4 / 8 * 8);
+        int mid = nvec;
+        const bool ramp = nvec >= 3 * chunk && q4 < chunk;
+        if (ramp) { csz.push_back(q4); csz.push_back(chunk - q4); mid -= 2 * chunk; }
+        for (; mid > 0; mid -= chunk) csz.push_back(std::min(chunk, mid));
+        if (ramp) { csz.push_back(chunk - q4); csz.push_back(q4); }
+    }
+    const int nch = (int)csz.size();
     size_t wb = 0;
     int rc = csf_workspace_bytes(c, chunk, mode, &wb); if (rc != CSF_OK) return fail(c, rc, "unsupported mode");
     const size_t rows = (size_t)2 * c->M, cb = rows * chunk * sizeof(double2);
@@ -907,8 +919,9 @@ int csf_filter_host(csf_ctx* c, const csf_c128* hX, csf_c128* hY, int64_t ld, in
     // an error inside the pipeline must not return while copies into the caller's host memory are in flight
     auto drain = [&]() { cudaStreamSynchronize(c->hs_in); cudaStreamSynchronize(c->stream); cudaStreamSynchronize(c->hs_out); };
 #define CSF_CUDA_H(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) { drain(); return cuda_fail(c, e__, #call); } } while (0)
-    for (int i = 0; i < nch; ++i) {
-        const int s = i & 1, v0 = i * chunk, nv = std::min(chunk, nvec - v0);
+    int v0 = 0;
+    for (int i = 0; i < nch; v0 += csz[i], ++i) {
+        const int s = i & 1, nv = csz[i];
         const size_t wbytes = (size_t)nv * sizeof(double2);
         if (i >= 2) CSF_CUDA_H(cudaStreamWaitEvent(c->hs_in, c->ev_cmp[s], 0));
         CSF_CUDA_H(cudaMemcpy2DAsync(c->h_x[s].p, wbytes, hX + v0, (size_t)ld * sizeof(double2), wbytes, rows, cudaMemcpyHostToDevice, c->hs_in));
@@ -1058,19 +1071,26 @@ int enqueue_gram(csf_ctx* c, const double* A, long long lda, const double* B, lo
     static bool configured[64] = {};
     int dev = 0; CSF_CUDA(c, cudaGetDevice(&dev));
     if (dev < 0 || dev >= 64 || !configured[dev]) {
-        CSF_CUDA(c, cudaFuncSetAttribute(gram_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kGramSmem));
+        CSF_CUDA(c, cudaFuncSetAttribute(gram_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)GramCfg<64>::SMEM));
+        CSF_CUDA(c, cudaFuncSetAttribute(gram_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)GramCfg<128>::SMEM));
         CSF_CUDA(c, cudaFuncSetAttribute(rotate_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRotSmem));
         if (dev >= 0 && dev < 64) configured[dev] = true;
     }
-    const long long rows = 2 * c->M; const int nc = 2 * nvec, nt = (nc + kGT - 1) / kGT;
+    // 128 x 128 output tiles for blocks of >= 128 vectors (twice the flops per byte read from L2), 64 x 64 below
+    const int tt = (nvec >= 128 && GramCfg<128>::SMEM <= c->smem_optin) ? 128 : 64;
+    const long long rows = 2 * c->M; const int nc = 2 * nvec, nt = (nc + tt - 1) / tt;
     CSF_CUDA(c, cudaMemsetAsync(dG, 0, (size_t)nc * nc * sizeof(double), c->stream));
-    // row ranges: enough CTAs for ~4 waves of 2 CTAs per SM over the (upper-triangle) tiles
+    // row ranges: enough CTAs for ~4 waves of resident CTAs (two per SM with 64-wide tiles, one with 128) over the (upper-triangle) tiles
     const int tiles = sym ? nt * (nt + 1) / 2 : nt * nt;
-    long long nsplit = std::max<long long>(1, std::min<long long>((8LL * c->sm_count + tiles - 1) / tiles, (rows + 4 * kGK - 1) / (4 * kGK)));
+    long long nsplit = std::max<long long>(1, std::min<long long>(((tt == 128 ? 4LL : 8LL) * c->sm_count + tiles - 1) / tiles, (rows + 4 * kGK - 1) / (4 * kGK)));
     nsplit = std::min<long long>(nsplit, 65535);
     const long long rpc = ((rows + nsplit - 1) / nsplit + kGK - 1) / kGK * kGK;
     dim3 grid(nt * nt, (unsigned)((rows + rpc - 1) / rpc));
-    { ProfScope ps(c, CSF_KIND_AUX); gram_kernel<<<grid, 256, kGramSmem, c->stream>>>(A, lda, B, ldb, nc, rows, rpc, dG, nc, sym); }
+    {
+        ProfScope ps(c, CSF_KIND_AUX);
+        if (tt == 128) gram_kernel<128><<<grid, 256, GramCfg<128>::SMEM, c->stream>>>(A, lda, B, ldb, nc, rows, rpc, dG, nc, sym);
+        else gram_kernel<64><<<grid, 256, GramCfg<64>::SMEM, c->stream>>>(A, lda, B, ldb, nc, rows, rpc, dG, nc, sym);
+    }
     CSF_CUDA(c, cudaGetLastError());
     gram_finish_kernel<<<(nvec * nvec + 255) / 256, 256, 0, c->stream>>>(dG, nc, nvec, dOut, nvec, sym);
     CSF_CUDA(c, cudaGetLastError());
