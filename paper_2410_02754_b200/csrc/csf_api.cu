@@ -885,16 +885,17 @@ int csf_filter_host(csf_ctx* c, const csf_c128* hX, csf_c128* hY, int64_t ld, in
     CSF_CUDA(c, cudaSetDevice(c->device));
     const int chunk = std::min(c->host_chunk, nvec);
     // Column chunks. What the pipeline cannot hide is the host->device copy of the first chunk and the device->host copy of the
-    // last one, so a block of at least three chunks starts with chunks of 1/4 and 3/4 the size (the first a multiple of 8
-    // columns) and ends with the same two in reverse: the copy of the second chunk still fits under the filter of the first.
+    // last one, so a block of at least three chunks starts and ends with half a chunk (a multiple of 8 columns). Not less:
+    // narrow blocks filter slowly (config 3: 6.9 ms per column at 64 columns and more, 7.8 at 48, 11.5 at 16), and a quarter
+    // chunk at both ends measured no gain at all.
     std::vector<int> csz;
     {
-        const int q4 = std::max(8, chunk / 4 / 8 * 8);
+        const int q2 = chunk / 2 / 8 * 8;
         int mid = nvec;
-        const bool ramp = nvec >= 3 * chunk && q4 < chunk;
-        if (ramp) { csz.push_back(q4); csz.push_back(chunk - q4); mid -= 2 * chunk; }
+        const bool ramp = nvec >= 3 * chunk && q2 >= 8;
+        if (ramp) { csz.push_back(q2); mid -= 2 * q2; }
         for (; mid > 0; mid -= chunk) csz.push_back(std::min(chunk, mid));
-        if (ramp) { csz.push_back(chunk - q4); csz.push_back(q4); }
+        if (ramp) csz.push_back(q2);
     }
     const int nch = (int)csz.size();
     size_t wb = 0;
@@ -1071,26 +1072,21 @@ int enqueue_gram(csf_ctx* c, const double* A, long long lda, const double* B, lo
     static bool configured[64] = {};
     int dev = 0; CSF_CUDA(c, cudaGetDevice(&dev));
     if (dev < 0 || dev >= 64 || !configured[dev]) {
-        CSF_CUDA(c, cudaFuncSetAttribute(gram_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)GramCfg<64>::SMEM));
-        CSF_CUDA(c, cudaFuncSetAttribute(gram_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)GramCfg<128>::SMEM));
+        CSF_CUDA(c, cudaFuncSetAttribute(gram_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kGramSmem));
         CSF_CUDA(c, cudaFuncSetAttribute(rotate_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRotSmem));
         if (dev >= 0 && dev < 64) configured[dev] = true;
     }
-    // 128 x 128 output tiles for blocks of >= 128 vectors (twice the flops per byte read from L2), 64 x 64 below
-    const int tt = (nvec >= 128 && GramCfg<128>::SMEM <= c->smem_optin) ? 128 : 64;
-    const long long rows = 2 * c->M; const int nc = 2 * nvec, nt = (nc + tt - 1) / tt;
+    const long long rows = 2 * c->M; const int nc = 2 * nvec, nt = (nc + kGT - 1) / kGT;
     CSF_CUDA(c, cudaMemsetAsync(dG, 0, (size_t)nc * nc * sizeof(double), c->stream));
-    // row ranges: enough CTAs for ~4 waves of resident CTAs (two per SM with 64-wide tiles, one with 128) over the (upper-triangle) tiles
+    // row ranges: enough CTAs for ~4 waves of 2 CTAs per SM over the (upper-triangle) tiles
+    // (128 x 128 output tiles — 32 x 64 per warp, twice the flops per byte read from L2, but 168 registers and 135 KB of shared
+    // memory, i.e. one CTA of 8 warps per SM — measured 253 against 212 ms for the two projections at config 3: dropped)
     const int tiles = sym ? nt * (nt + 1) / 2 : nt * nt;
-    long long nsplit = std::max<long long>(1, std::min<long long>(((tt == 128 ? 4LL : 8LL) * c->sm_count + tiles - 1) / tiles, (rows + 4 * kGK - 1) / (4 * kGK)));
+    long long nsplit = std::max<long long>(1, std::min<long long>((8LL * c->sm_count + tiles - 1) / tiles, (rows + 4 * kGK - 1) / (4 * kGK)));
     nsplit = std::min<long long>(nsplit, 65535);
     const long long rpc = ((rows + nsplit - 1) / nsplit + kGK - 1) / kGK * kGK;
     dim3 grid(nt * nt, (unsigned)((rows + rpc - 1) / rpc));
-    {
-        ProfScope ps(c, CSF_KIND_AUX);
-        if (tt == 128) gram_kernel<128><<<grid, 256, GramCfg<128>::SMEM, c->stream>>>(A, lda, B, ldb, nc, rows, rpc, dG, nc, sym);
-        else gram_kernel<64><<<grid, 256, GramCfg<64>::SMEM, c->stream>>>(A, lda, B, ldb, nc, rows, rpc, dG, nc, sym);
-    }
+    { ProfScope ps(c, CSF_KIND_AUX); gram_kernel<<<grid, 256, kGramSmem, c->stream>>>(A, lda, B, ldb, nc, rows, rpc, dG, nc, sym); }
     CSF_CUDA(c, cudaGetLastError());
     gram_finish_kernel<<<(nvec * nvec + 255) / 256, 256, 0, c->stream>>>(dG, nc, nvec, dOut, nvec, sym);
     CSF_CUDA(c, cudaGetLastError());

@@ -29,80 +29,68 @@ constexpr int kGK = 32;            // rows (gram) / inner columns (rotate) per s
 constexpr int kGP = kGT + 4;       // padded row of a [k][64] slab: a DMMA fragment reads rows k .. k+3 at columns c .. c+7; with the rows 4 doubles
                                    // apart mod 16 each half-warp covers 16 different 8-byte banks (2 wavefronts per LDS.64, the minimum)
 constexpr int kRP = kGK + 4;       // padded row of a [64][k] slab (rotate's A operand)
+constexpr size_t kGramSmem = (size_t)2 * 2 * kGK * kGP * sizeof(double);
 constexpr size_t kRotSmem = (size_t)2 * (kGT * kRP + kGK * kGP) * sizeof(double);
 
 // G[ca][cb] += sum_{r in this CTA's row range} A[r][ca] B[r][cb]; blockIdx.x = (tile m, tile n), blockIdx.y = row range.
-// sym: only tiles with n >= m (Hermitian result). TT = output tile edge: 64, or 128 for blocks of >= 128 vectors. 8 warps as
-// 4 x 2: warp (wm, wn) owns the (TT/4) x (TT/2) block at (TT/4 wm, TT/2 wn) of the tile. TT = 64: 16 x 32 per warp, 2 A + 4 B
-// fragment loads per 8 DMMAs (an 8 x 64 strip per warp takes 9, and the loads, not the tensor pipe, bound it); every CTA
-// re-reads its two 64-column strips of the block from L2 at 8 flops per byte (4.6 TB/s at the FP64 peak: the L2 <-> SM fabric
-// binds, 26 TF/s measured). TT = 128: 32 x 64 per warp, 4 A + 8 B loads per 32 DMMAs, 16 flops per byte.
-template <int TT> struct GramCfg {
-    static constexpr int GP = TT + 4;              // padded slab row (rows 4 doubles apart mod 16: see kGP)
-    static constexpr size_t SMEM = (size_t)2 * 2 * kGK * GP * sizeof(double);
-    static constexpr int MT = TT / 32, NT = TT / 16;   // m8 / n8 fragment tiles per warp
-};
-template <int TT>
+// sym: only tiles with n >= m (Hermitian result). 8 warps as 4 x 2: warp (wm, wn) owns the 16 x 32 block at (16 wm, 32 wn) of the
+// 64 x 64 tile: 2 A + 4 B fragment loads per 8 DMMAs (an 8 x 64 strip per warp takes 9, and the loads, not the tensor pipe, bound it).
 __global__ void __launch_bounds__(256) gram_kernel(const double* __restrict__ A, long long lda, const double* __restrict__ B, long long ldb,
                                                    int ncols, long long rows, long long rows_per_cta, double* __restrict__ G, int ldg, int sym) {
     extern __shared__ __align__(16) double sm[];
-    constexpr int GP = GramCfg<TT>::GP, MT = GramCfg<TT>::MT, NT = GramCfg<TT>::NT;
-    const int ntile = (ncols + TT - 1) / TT;
+    const int ntile = (ncols + kGT - 1) / kGT;
     const int tm = blockIdx.x / ntile, tn = blockIdx.x % ntile;
     if (sym && tn < tm) return;
     const long long r0 = (long long)blockIdx.y * rows_per_cta, r1 = min(rows, r0 + rows_per_cta);
     if (r0 >= r1) return;
-    double* As = sm;                                  // [2][kGK][GP]
-    double* Bs = sm + 2 * kGK * GP;
+    double* As = sm;                                  // [2][kGK][kGP]
+    double* Bs = sm + 2 * kGK * kGP;
     const int tid = threadIdx.x, warp = tid >> 5, t = tid & 31;
-    const int m0 = tm * TT, n0 = tn * TT;
+    const int m0 = tm * kGT, n0 = tn * kGT;
     auto load_slab = [&](int buf, long long rs) {
-        // 32 rows x TT doubles = 16 TT 16-byte pieces per operand, TT / 16 per thread
+        // 32 rows x 64 doubles = 1024 16-byte pieces per operand, 4 per thread
 #pragma unroll
-        for (int q = 0; q < TT / 16; ++q) {
-            const int piece = tid + 256 * q, rr = piece / (TT / 2), cc = (piece % (TT / 2)) * 2;
+        for (int q = 0; q < 4; ++q) {
+            const int piece = tid + 256 * q, rr = piece >> 5, cc = (piece & 31) * 2;
             const long long row = rs + rr;
             const bool ra = row < r1;
-            sub_cp16(As + (buf * kGK + rr) * GP + cc, A + (ra ? row : r0) * lda + min(m0 + cc, ncols - 2), (ra && m0 + cc < ncols) ? 16 : 0);
-            sub_cp16(Bs + (buf * kGK + rr) * GP + cc, B + (ra ? row : r0) * ldb + min(n0 + cc, ncols - 2), (ra && n0 + cc < ncols) ? 16 : 0);
+            sub_cp16(As + (buf * kGK + rr) * kGP + cc, A + (ra ? row : r0) * lda + min(m0 + cc, ncols - 2), (ra && m0 + cc < ncols) ? 16 : 0);
+            sub_cp16(Bs + (buf * kGK + rr) * kGP + cc, B + (ra ? row : r0) * ldb + min(n0 + cc, ncols - 2), (ra && n0 + cc < ncols) ? 16 : 0);
         }
         sub_cp_commit();
     };
     const int wm = warp >> 1, wn = warp & 1;
-    double c[MT][NT][2];
+    double c[2][4][2];
 #pragma unroll
-    for (int mt = 0; mt < MT; ++mt)
+    for (int mt = 0; mt < 2; ++mt)
 #pragma unroll
-        for (int nt = 0; nt < NT; ++nt) { c[mt][nt][0] = 0.0; c[mt][nt][1] = 0.0; }
+        for (int nt = 0; nt < 4; ++nt) { c[mt][nt][0] = 0.0; c[mt][nt][1] = 0.0; }
     const long long nslab = (r1 - r0 + kGK - 1) / kGK;
     load_slab(0, r0);
     for (long long s = 0; s < nslab; ++s) {
         const int buf = (int)(s & 1);
         if (s + 1 < nslab) { load_slab(buf ^ 1, r0 + (s + 1) * kGK); sub_cp_wait<1>(); } else sub_cp_wait<0>();
         __syncthreads();
-        const double* as = As + buf * kGK * GP + (TT / 4) * wm + (t >> 2);
-        const double* bs = Bs + buf * kGK * GP + (TT / 2) * wn + (t >> 2);
+        const double* as = As + buf * kGK * kGP + 16 * wm + (t >> 2);
+        const double* bs = Bs + buf * kGK * kGP + 32 * wn + (t >> 2);
 #pragma unroll
         for (int kk = 0; kk < kGK / 4; ++kk) {
-            double a[MT];
+            const double a0 = as[(kk * 4 + (t & 3)) * kGP], a1 = as[(kk * 4 + (t & 3)) * kGP + 8];
 #pragma unroll
-            for (int mt = 0; mt < MT; ++mt) a[mt] = as[(kk * 4 + (t & 3)) * GP + 8 * mt];
-#pragma unroll
-            for (int nt = 0; nt < NT; ++nt) {
-                const double b = bs[(kk * 4 + (t & 3)) * GP + 8 * nt];
-#pragma unroll
-                for (int mt = 0; mt < MT; ++mt) sub_dmma(c[mt][nt][0], c[mt][nt][1], a[mt], b);
+            for (int nt = 0; nt < 4; ++nt) {
+                const double b = bs[(kk * 4 + (t & 3)) * kGP + 8 * nt];
+                sub_dmma(c[0][nt][0], c[0][nt][1], a0, b); sub_dmma(c[1][nt][0], c[1][nt][1], a1, b);
             }
         }
         __syncthreads();
     }
 #pragma unroll
-    for (int mt = 0; mt < MT; ++mt) {
-        const int gm = m0 + (TT / 4) * wm + 8 * mt + (t >> 2);
+    for (int mt = 0; mt < 2; ++mt) {
+        const int gm = m0 + 16 * wm + 8 * mt + (t >> 2);
         if (gm >= ncols) continue;
 #pragma unroll
-        for (int nt = 0; nt < NT; ++nt) {
-            const int gn = n0 + (TT / 2) * wn + 8 * nt + 2 * (t & 3);
+        for (int nt = 0; nt < 4; ++nt) {
+            const int gn = n0 + 32 * wn + 8 * nt + 2 * (t & 3);
             if (gn < ncols) { atomicAdd(G + (long long)gm * ldg + gn, c[mt][nt][0]); atomicAdd(G + (long long)gm * ldg + gn + 1, c[mt][nt][1]); }
         }
     }

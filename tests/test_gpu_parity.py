@@ -170,7 +170,7 @@ def test_error_codes():
 @pytest.mark.parametrize("chunk,nvec,ld", [(8, 20, 24), (64, 16, 16), (5, 5, 5), (4, 9, 9), (32, 100, 104), (16, 48, 48)])
 def test_filter_host_pipeline_matches_oracle(chunk, nvec, ld, cfg0_oracle):
     """The end-to-end entry point: host buffers staged in column chunks (H2D / filter / D2H on three streams); blocks of at
-    least three chunks start and end with a small chunk (32, 100: chunks 8, 24, 32, 4, 24, 8; 16, 48: 8, 8, 16, 8, 8)."""
+    least three chunks start and end with half a chunk (32, 100: chunks 16, 32, 32, 4, 16; 16, 48: 8, 16, 16, 8)."""
     import torch
     ref, a, b = (cfg0_oracle[k] for k in ("ctx", "a", "b"))
     _, gpu, s = setup_pair(synth.CONFIGS[0])
