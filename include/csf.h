@@ -170,7 +170,7 @@ int csf_column_lanes(const csf_ctx* ctx, int nvec, int mode, int* lanes);
  * split into two halves (the first a multiple of 8 vectors) whose column steps alternate, and every column launch computes, in
  * two extra warps, the projector coefficients the OTHER half needs next: the HBM-bound gather runs beside the latency-bound
  * column step instead of after it. Results differ from the unfused path by summation order only.
- * CSF_FUSED_GATHER=0 | 1 (read by csf_create) switches the path off | on for every block of >= 2 vectors (parity tests).
+ * CSF_FUSED_GATHER=0 | 1 (read by csf_create) switches the path off | on for every block of >= 9 vectors (parity tests).
  * Host-only query. */
 int csf_filter_fused_gather(const csf_ctx* ctx, int nvec, int mode, int* fused);
 

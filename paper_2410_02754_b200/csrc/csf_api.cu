@@ -357,11 +357,12 @@ int enqueue_step(csf_ctx* c, const void* src, long long ld, void* dst, long long
 
 // The fused path of csf_filter (complex128, order 5, 8 vectors per CTA, 18 projectors per atom): the block is split into two
 // halves whose column steps alternate, and each column launch computes, in two extra warps, the projector coefficients the
-// OTHER half needs next. CSF_FUSED_GATHER=0 switches it off, =1 takes it for any block of >= 2 vectors (tests).
+// OTHER half needs next. CSF_FUSED_GATHER=0 switches it off, =1 takes it for any block of >= 9 vectors (tests).
 bool fused_gather_ok(const csf_ctx* c, int nvec) {
     if (c->fused_gather == 0 || column_kind(c) != 1 || c->p != 5 || c->natoms == 0 || c->npj_uniform != 18 || c->npjp != 20) return false;
     if (column_info_wide_p5_g().smem > c->smem_optin) return false;
-    return nvec >= (c->fused_gather == 1 ? 2 : 64);
+    // (from 9 vectors on the first half is a multiple of 8 vectors, which keeps the two halves' C~ blocks inside ctp_bytes(nvec))
+    return nvec >= (c->fused_gather == 1 ? 9 : 64);
 }
 
 size_t f32_block_bytes(const csf_ctx* c, int nvec) { return ((size_t)2 * c->M * ((nvec + 1) & ~1) * sizeof(float2) + 255) / 256 * 256; }

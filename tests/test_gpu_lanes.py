@@ -143,6 +143,11 @@ def test_fused_gather_policy_and_agreement(monkeypatch):
     monkeypatch.setenv("CSF_FUSED_GATHER", "1")
     p4 = binding.Csf((2, 2, 2), (4.0, 4.0, 4.0), 4, (0, 0, 0))
     assert not p4.filter_fused_gather(256, binding.CSF_FP64)          # order 4 has no kernel with gather warps
+    # forced on, the path starts at 9 vectors (halves of 8 + 1: the first half must be a multiple of 8 vectors)
+    ref3, gpu3, _ = setup_pair(cfg)
+    assert gpu3.filter_fused_gather(9, binding.CSF_FP64) and not gpu3.filter_fused_gather(8, binding.CSF_FP64)
+    for n in (8, 9, 10):
+        assert_block_close(gpu_filter(gpu3, X[:, :n], 7, a, b, ld=12), Yref[:, :n], TOL)
 
 
 @pytest.mark.parametrize("gather", ["reg", "bulk"])
