@@ -54,6 +54,9 @@ constexpr int kColXBuf = 2;
 #ifndef CSF_WIDE_AUXW
 #define CSF_WIDE_AUXW 4
 #endif
+#ifndef CSF_PREFB_MIN
+#define CSF_PREFB_MIN 128
+#endif
 constexpr int kColMaxAuxWarps = 6;
 constexpr int col_aux_warps(int p, bool f32, int mode, int lanes = 16) {
     if (lanes == 32) return (p == 5 && !f32) ? CSF_WIDE_AUXW : (p == 4 ? 3 : 2);
@@ -394,6 +397,7 @@ __global__ void __launch_bounds__(ColCfg<T, P, L, AUXW, GW>::NT) __maxnreg__(col
         const int aw = warp_id, wl = tid & 31;
         const int kk = wl & 3, rw = wl >> 2;
         constexpr int TMAX = (P * P * P + 7) / 8, TCH = TMAX < 5 ? TMAX : ((L == 32 && col_maxreg(P, sizeof(T) == 4, L, AUXW) <= 128) ? 3 : 5);   // wide kernels capped at 128 registers: fewer tiles in flight
+        constexpr bool kPrefB = col_maxreg(P, sizeof(T) == 4, L, AUXW) > CSF_PREFB_MIN;
         const int xr0 = col_aux_row0(P * P * P, kColAuxWarps, aw), xr1 = col_aux_row0(P * P * P, kColAuxWarps, aw + 1);
         auto load_b = [&](const int4& ds, double (&bb)[KS][L / 8]) {
             const double* cb = A.Ct + ((long long)ds.x * A.nchunks + chunk) * (KS * (L / 8) * 32) + wl;
@@ -472,8 +476,10 @@ __global__ void __launch_bounds__(ColCfg<T, P, L, AUXW, GW>::NT) __maxnreg__(col
                 for (int sp = sp0; sp < sp1; ++sp) {
                     // A fragments of up to TCH tiles at once (one exposed round trip), next sub-pair's B meanwhile
                     const int e0 = ds.z, e1 = ds.w;
-                    int4 dn = ds; double bn[KS][L / 8];
-                    if (sp + 1 < sp1) { dn = __ldg(A.sub_desc + sp + 1); load_b(dn, bn); }
+                    // (kernels capped at 128 registers prefetch the next descriptor only: its C~ fragments are requested
+                    // together with its first P~ tiles, which is one exposed round trip either way, and 40 registers less)
+                    int4 dn = ds; double bn[kPrefB ? KS : 1][kPrefB ? L / 8 : 1];
+                    if (sp + 1 < sp1) { dn = __ldg(A.sub_desc + sp + 1); if constexpr (kPrefB) load_b(dn, bn); }
                     for (int eb = e0; eb < e1; eb += 8 * TCH) {
                         double a[TCH][KS]; int loc[TCH];
 #pragma unroll
@@ -506,10 +512,12 @@ __global__ void __launch_bounds__(ColCfg<T, P, L, AUXW, GW>::NT) __maxnreg__(col
                     __syncwarp();          // the next sub-pair of this warp may touch the same rows from other lanes
                     if (sp + 1 < sp1) {
                         ds = dn;
+                        if constexpr (kPrefB) {
 #pragma unroll
-                        for (int s = 0; s < KS; ++s)
+                            for (int s = 0; s < KS; ++s)
 #pragma unroll
-                            for (int nt = 0; nt < L / 8; ++nt) b[s][nt] = bn[s][nt];
+                                for (int nt = 0; nt < L / 8; ++nt) b[s][nt] = bn[kPrefB ? s : 0][kPrefB ? nt : 0];
+                        } else load_b(ds, b);
                     }
                 }
             }
