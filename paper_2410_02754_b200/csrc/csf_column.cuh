@@ -55,7 +55,7 @@ constexpr int kColXBuf = 2;
 #define CSF_WIDE_AUXW 4
 #endif
 #ifndef CSF_PREFB_MIN
-#define CSF_PREFB_MIN 128
+#define CSF_PREFB_MIN 168
 #endif
 constexpr int kColMaxAuxWarps = 6;
 constexpr int col_aux_warps(int p, bool f32, int mode, int lanes = 16) {
