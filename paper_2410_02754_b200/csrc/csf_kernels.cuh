@@ -182,7 +182,9 @@ __global__ void __launch_bounds__(256, 2) proj_gather_bulk_kernel(const __grid_c
     }
     __syncthreads();
     const int ngroups = (e1 - e0 + kGbRows - 1) / kGbRows;
-    // warp 0 issues the copies of a stage: lane = (row, spin)
+    // one warp issues the copies of a stage: lane = (row, spin); warp w issues groups w, w + 8, ... and holds the node index of its
+    // next group's row (a copy must not wait for an index load)
+    int nodep; { const int en = e0 + warp * kGbRows + (wl >> 1); nodep = en < e1 ? __ldg(A.ent_node + en) : 0; }
     auto issue = [&](int g) {
         const int s = g % kGbStages;
         const int eg = e0 + g * kGbRows, rows_g = min(kGbRows, e1 - eg);
@@ -194,15 +196,18 @@ __global__ void __launch_bounds__(256, 2) proj_gather_bulk_kernel(const __grid_c
         if (wl == 0) asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mb0 + 8 * s), "r"((unsigned)(rows_g * 2 * cpb)) : "memory");
         __syncwarp();
         const int row = wl >> 1, sp = wl & 1;
+        const long long node = nodep;
+        { const int en = eg + 8 * kGbRows + row; nodep = en < e1 ? __ldg(A.ent_node + en) : 0; }      // this warp's next group: g + 8
         if (row < rows_g) {
-            const long long node = __ldg(A.ent_node + eg + row);
             const char* src = static_cast<const char*>(A.src) + ((2 * node + sp) * A.ld + vc0) * EB;
             const unsigned dst = (unsigned)__cvta_generic_to_shared(gsm + ((size_t)s * kGbRows + row) * RB + sp * SPB);
             asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst), "l"(src), "r"((unsigned)cpb), "r"(mb0 + 8 * s) : "memory");
         }
     };
-    if (warp == 0)
-        for (int g = 0; g < kGbStages && g < ngroups; ++g) issue(g);
+    // the copies of group g are issued by warp g mod 8: a bulk copy costs the issuing warp ~500 cycles, and a fixed issuing warp
+    // falls behind by that much in every group and sets the pace of the CTA through the stage barriers
+    for (int g = 0; g < kGbStages && g < ngroups; ++g)
+        if (warp == (g & 7)) issue(g);
     double acc[MD][kGatherNT][2];
     double accx[NX > 0 ? NX : 1][kGatherNT];
 #pragma unroll
@@ -251,7 +256,7 @@ __global__ void __launch_bounds__(256, 2) proj_gather_bulk_kernel(const __grid_c
         }
         __syncwarp();
         if (wl == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(mb0 + 8 * (kGbStages + s)) : "memory");
-        if (warp == 0 && g + kGbStages < ngroups) issue(g + kGbStages);
+        if (warp == ((g + kGbStages) & 7) && g + kGbStages < ngroups) issue(g + kGbStages);
     }
     const long long coff = A.atom_coff[atom];
     const int v0 = vc0 + vloc;
