@@ -165,3 +165,22 @@ def test_both_projector_gather_kernels(monkeypatch, gather, base, ncell, natoms,
     assert_block_close(gpu_filter(gpu, X, degree, a, b), Yref, TOL)
     assert_block_close(gpu_filter32(gpu, X, degree, a, b), Yref, TOL32)
     assert_block_close(gpu_apply_H(gpu, X, ld=nvec + 3), ref.apply_H(X), TOL)
+
+
+def test_filter_host_with_fused_chunks(monkeypatch):
+    """csf_filter_host on an order-5 mesh with a block wide enough for its 64-column chunks to take the fused half-block path by
+    the policy itself (200 columns: chunks of 32, 64, 64, 8, 32; the half chunks at both ends and the remainder run unfused)."""
+    import torch
+    for v in ("CSF_LANES", "CSF_KERNEL", "CSF_FUSED_GATHER"):
+        monkeypatch.delenv(v, raising=False)
+    cfg = synth.scaled_config(synth.CONFIGS[3], (4, 4, 4), 2, nvec=200, degree=5)
+    ref, gpu, s = setup_pair(cfg)
+    a, b, _, _ = bounds.lanczos_bounds(lambda v: ref.apply_H(v), 2 * ref.M)
+    X = synth.random_block(s.rng, 2 * ref.M, 200)
+    hX = torch.zeros((2 * ref.M, 204), dtype=torch.complex128).pin_memory(); hX[:, :200] = torch.from_numpy(X)
+    hY = torch.full((2 * ref.M, 204), 7.0 + 3.0j, dtype=torch.complex128).pin_memory()
+    gpu.set_host_chunk(64)
+    gpu.filter_host(hX, hY, 204, 200, 5, a, b)
+    out = hY.numpy()
+    assert_block_close(out[:, :200], ref.filter(X, 5, a, b), TOL)
+    assert np.all(out[:, 200:] == 7.0 + 3.0j), "padding columns were touched"
