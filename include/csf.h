@@ -166,7 +166,7 @@ int csf_column_lanes(const csf_ctx* ctx, int nvec, int mode, int* lanes);
 
 /* Whether csf_filter runs a block of nvec vectors in `mode` on its fused half-block path (*fused = 1) or with one projector
  * gather kernel per recurrence step (*fused = 0). Fused path (eq.84: the inner sum C^a = P^{a,T} X^(e') is all that a
- * step needs from the other cells): complex128, order 5, 8 vectors per CTA, 18 projectors per atom, >= 64 vectors. The block is
+ * step needs from the other cells): complex128, order 5, 8 vectors per CTA, 18 projectors per atom, a multiple of 64 vectors. The block is
  * split into two halves (the first a multiple of 8 vectors) whose column steps alternate, and every column launch computes, in
  * two extra warps, the projector coefficients the OTHER half needs next: the HBM-bound gather runs beside the latency-bound
  * column step instead of after it. Results differ from the unfused path by summation order only.

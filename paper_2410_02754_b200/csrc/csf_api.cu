@@ -362,7 +362,10 @@ bool fused_gather_ok(const csf_ctx* c, int nvec) {
     if (c->fused_gather == 0 || column_kind(c) != 1 || c->p != 5 || c->natoms == 0 || c->npj_uniform != 18 || c->npjp != 20) return false;
     if (column_info_wide_p5_g().smem > c->smem_optin) return false;
     // (from 9 vectors on the first half is a multiple of 8 vectors, which keeps the two halves' C~ blocks inside ctp_bytes(nvec))
-    return nvec >= (c->fused_gather == 1 ? 9 : 64);
+    if (c->fused_gather == 1) return nvec >= 9;
+    // policy: both halves whole gather tasks of 32 vectors (a block of 96 = 48 + 48 pads the gather warps' work by a third and
+    // measured 761 against 711 ms at config 3; 64 = 32 + 32 breaks even, 256 = 128 + 128 gains 3-7 %)
+    return nvec >= 64 && nvec % 64 == 0;
 }
 
 size_t f32_block_bytes(const csf_ctx* c, int nvec) { return ((size_t)2 * c->M * ((nvec + 1) & ~1) * sizeof(float2) + 255) / 256 * 256; }

@@ -119,27 +119,28 @@ def test_column_lanes_query(monkeypatch):
 
 
 def test_fused_gather_policy_and_agreement(monkeypatch):
-    """csf_filter_fused_gather reports the path a block takes (policy: complex128, order 5, 18 projectors per atom, >= 64
-    vectors; CSF_FUSED_GATHER pins it), and the fused and the unfused path give the oracle's result on the same block — a
-    block wide enough for the policy to choose the fused path by itself, split 40 + 27 (ragged second half)."""
+    """csf_filter_fused_gather reports the path a block takes (policy: complex128, order 5, 18 projectors per atom, a multiple
+    of 64 vectors; CSF_FUSED_GATHER pins it), and the fused and the unfused path give the oracle's result on the same blocks:
+    64 vectors (the policy's own choice, halves 32 + 32) and 67 (forced, split 40 + 27 with a ragged second half)."""
     from paper_2410_02754_b200 import binding
     for v in ("CSF_LANES", "CSF_KERNEL", "CSF_FUSED_GATHER"):
         monkeypatch.delenv(v, raising=False)
     cfg = synth.scaled_config(synth.CONFIGS[3], (4, 4, 4), 2, nvec=67, degree=7)
     ref, gpu, s = setup_pair(cfg)
-    assert gpu.filter_fused_gather(67, binding.CSF_FP64) and gpu.filter_fused_gather(64, binding.CSF_FP64)
-    assert not gpu.filter_fused_gather(63, binding.CSF_FP64) and not gpu.filter_fused_gather(67, binding.CSF_FP32_INTERMEDIATE)
+    assert gpu.filter_fused_gather(64, binding.CSF_FP64) and gpu.filter_fused_gather(256, binding.CSF_FP64)
+    assert not gpu.filter_fused_gather(63, binding.CSF_FP64) and not gpu.filter_fused_gather(96, binding.CSF_FP64)
+    assert not gpu.filter_fused_gather(64, binding.CSF_FP32_INTERMEDIATE)
     a, b, _, _ = bounds.lanczos_bounds(lambda v: ref.apply_H(v), 2 * ref.M)
     X = synth.random_block(s.rng, 2 * ref.M, 67)
     Yref = ref.filter(X, 7, a, b)
-    Yf = gpu_filter(gpu, X, 7, a, b, ld=70)
-    assert_block_close(Yf, Yref, TOL)
+    Yp = gpu_filter(gpu, X[:, :64], 7, a, b, ld=70)                     # the policy's fused path
+    assert_block_close(Yp, Yref[:, :64], TOL)
     monkeypatch.setenv("CSF_FUSED_GATHER", "0")
     ref2, gpu2, _ = setup_pair(cfg)
-    assert not gpu2.filter_fused_gather(67, binding.CSF_FP64)
+    assert not gpu2.filter_fused_gather(64, binding.CSF_FP64)
     Yu = gpu_filter(gpu2, X, 7, a, b, ld=70)
     assert_block_close(Yu, Yref, TOL)
-    assert rel_fro(Yf, Yu) < 1e-13
+    assert rel_fro(Yp, Yu[:, :64]) < 1e-13
     monkeypatch.setenv("CSF_FUSED_GATHER", "1")
     p4 = binding.Csf((2, 2, 2), (4.0, 4.0, 4.0), 4, (0, 0, 0))
     assert not p4.filter_fused_gather(256, binding.CSF_FP64)          # order 4 has no kernel with gather warps
@@ -148,6 +149,9 @@ def test_fused_gather_policy_and_agreement(monkeypatch):
     assert gpu3.filter_fused_gather(9, binding.CSF_FP64) and not gpu3.filter_fused_gather(8, binding.CSF_FP64)
     for n in (8, 9, 10):
         assert_block_close(gpu_filter(gpu3, X[:, :n], 7, a, b, ld=12), Yref[:, :n], TOL)
+    Yf = gpu_filter(gpu3, X, 7, a, b, ld=70)                             # 67 = 40 + 27
+    assert_block_close(Yf, Yref, TOL)
+    assert rel_fro(Yf, Yu) < 1e-13
 
 
 @pytest.mark.parametrize("gather", ["reg", "bulk"])
