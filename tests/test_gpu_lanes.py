@@ -17,7 +17,7 @@ pytestmark = pytest.mark.gpu
 def lanes(request, monkeypatch):
     """16: 4 vectors per CTA; 32: 8 vectors per CTA (cell-per-iteration kernel); "ws": the warp-specialised streaming kernel;
     "fused": csf_filter's half-block path (order 5, complex128: the column kernel with two gather warps that compute the
-    projector coefficients of the other half-block) forced for every block size, which the policy takes from 64 vectors on."""
+    projector coefficients of the other half-block) forced for every block size, which the policy takes for blocks that are multiples of 64 vectors."""
     if request.param == "ws":
         monkeypatch.setenv("CSF_KERNEL", "ws")
     elif request.param == "fused":
